@@ -1,0 +1,171 @@
+/* dex.h — C ABI of the B200-native Depth Exploration Decoding (DEX) step library.
+ *
+ * One thing lives behind this boundary: the expand -> exit -> commit -> collapse step of
+ * DEX (arxiv/paper_2606_29223), PAPER.md:143-190 (Alg. 1) and PAPER.md:196-208 (Sec. 3.2),
+ * with greedy DECS decoding, PAPER.md:454-482 (Alg. 2).  Every call below is hand-written
+ * CUDA for sm_100a; there is no CPU fallback.
+ *
+ * Conventions
+ *   - plain C, opaque handle, every call returns int32_t: DEX_OK or a negative DEX_E* code;
+ *     dex_last_error() returns a static/ctx-owned string.  Nothing throws or aborts.
+ *   - Ownership: ALL device memory (weights, workspace) is allocated by the caller and only
+ *     borrowed; it must outlive the context.  The library never calls cudaMalloc.  It owns
+ *     host-side bookkeeping and one small pinned host buffer for step results.
+ *   - "device" / "host" is stated for every pointer.  All device pointers must be 16-byte
+ *     aligned; the workspace 1024-byte aligned.
+ *   - The CUDA stream is the caller's (cudaStream_t passed as void*); all work of a call is
+ *     enqueued on it; calls that return results synchronise that stream before returning.
+ *   - Not thread-safe per context.
+ */
+#ifndef DEX_B200_H
+#define DEX_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define DEX_OK          0
+#define DEX_EINVAL     -1   /* bad argument / config (e.g. depth set violates Def. 4)   */
+#define DEX_ECAPACITY  -2   /* workspace, max_ctx, max_seqs or row capacity exceeded     */
+#define DEX_ESTATE     -3   /* call not legal in the current FSM state                   */
+#define DEX_ECUDA      -4   /* a CUDA runtime / driver call failed (see dex_last_error)  */
+
+#define DEX_MAX_DEPTHS  8   /* |X| <= 8: the range the paper evaluates    */
+
+/* dex_step flags */
+#define DEX_STEP_AUTOCOLLAPSE 1u  /* commit + collapse inside the step (Alg. 1 lines 9-13) */
+
+typedef struct dex_ctx dex_ctx;
+
+/* Model + runtime shape.  Llama-style pre-norm decoder (BASELINE.json:configs; reading R13
+ * in DESIGN.md): RMSNorm, rotate-half RoPE, GQA, SwiGLU, untied embed / LM head, no biases;
+ * every exit depth is decoded by the shared final RMSNorm + LM head. */
+typedef struct dex_config {
+  int32_t n_layers;      /* L                                                             */
+  int32_t d_model;       /* d, multiple of 8                                              */
+  int32_t n_heads;
+  int32_t n_kv_heads;    /* divides n_heads                                               */
+  int32_t head_dim;      /* 64 or 128                                                     */
+  int32_t d_ffn;         /* multiple of 8                                                 */
+  int32_t vocab;
+  float   rms_eps;
+  float   rope_theta;
+  int32_t max_seqs;      /* independent sequences (lattices) batched into the same launches */
+  int32_t max_ctx;       /* max committed positions per sequence (prompt + generated)     */
+  int32_t page_size;     /* committed-KV page, positions; multiple of 64                  */
+  int32_t decs;          /* 1: Alg. 2 masking of shallower slot-chain proposals; 0: plain argmax */
+  int32_t eos_id;        /* -1: none (stop rule = max length only)      */
+  int32_t debug_taps;    /* 1: keep per-layer hidden rows / anchor logits for dex_debug_read */
+  int32_t act_planes;    /* 1: activations enter the MMAs as bf16; 2: as bf16 hi+lo pair  */
+  int32_t use_graph;     /* 1: replay the step as a CUDA graph                            */
+} dex_config;
+
+/* Device pointers to the packed tensors (row-major, "out x in"; layout = dex_synth/gen.py):
+ *   embed [V,d] bf16, lm_head [V,d] bf16, wqkv [L,(nh+2nkv)*hd,d] bf16 (q heads, k heads, v heads),
+ *   wo [L,d,nh*hd] bf16, wgu [L,2,ffn,d] bf16 (gate, up), wdn [L,d,ffn] bf16,
+ *   norm_attn [L,d] f32, norm_ffn [L,d] f32, norm_final [d] f32. */
+typedef struct dex_weights {
+  const void*  embed;
+  const void*  lm_head;
+  const void*  wqkv;
+  const void*  wo;
+  const void*  wgu;
+  const void*  wdn;
+  const float* norm_attn;
+  const float* norm_ffn;
+  const float* norm_final;
+} dex_weights;
+
+/* Per-sequence record of one round of Alg. 1 (host memory). */
+typedef struct dex_step_result {
+  int32_t active;            /* sequence took part in this round                           */
+  int32_t committed;         /* 1 if the anchor reached final depth and a token was committed */
+  int32_t token;             /* y = u_{N-1}; -1 if none                     */
+  int32_t match_k;           /* selected anchor branch b_k (N-1 = fallback); -1 if none    */
+  int32_t q_before;          /* FSM state entering the round                               */
+  int32_t q_after;           /* FSM state leaving it (after collapse / advance)            */
+  int32_t exit_rows;         /* new lattice nodes decoded this round (2^q)                 */
+  int32_t critical_layers;   /* max |Pi_m| over live stages (paper's charged depth)        */
+  int64_t layer_evals;       /* sum_m rows_m * |Pi_m| executed this round                  */
+  int32_t rows_per_stage[DEX_MAX_DEPTHS];
+  int32_t anchor_tokens[DEX_MAX_DEPTHS]; /* u_0..u_{N-1} when the anchor is at final depth */
+  float   ref_top1;          /* final-depth anchor's best and second-best logit            */
+  float   ref_top2;
+  int32_t n_tokens;          /* committed tokens incl. prompt after the round              */
+  int32_t done;              /* eos hit or max_ctx reached                                 */
+} dex_step_result;
+
+/* Bytes of device workspace dex_init needs (committed KV pages, slot KV, hidden rows,
+ * activation planes, split-K partials, row tables, FSM, exit scratch).  host: cfg, depths, out. */
+int32_t dex_workspace_bytes(const dex_config* cfg, const int32_t* depths, int32_t n_depths,
+                            size_t* out_bytes);
+
+/* Create a context.  depths (host): the exploration set X = {d_0 < ... < d_{N-1} = L}
+ * (Def. 4), strictly increasing, in [1,L], last == L, N <= DEX_MAX_DEPTHS;
+ * DEX_EINVAL otherwise.  depths = {L} IS the autoregressive baseline.  w (host struct of
+ * device pointers), workspace (device, >= dex_workspace_bytes, 1024-aligned), stream
+ * (cudaStream_t).  Builds TMA descriptors, RoPE tables, zeroes the FSM. */
+int32_t dex_init(dex_ctx** out, const dex_config* cfg, const dex_weights* w,
+                 const int32_t* depths, int32_t n_depths,
+                 void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* S <- init(x, {E_k})  (Alg. 1 line 2; reading R3): resets sequence `seq`,
+ * fills the committed K/V of prompt[0..n-2] at all layers (chunks of <=128 causal rows
+ * through the same segment kernels), makes prompt[n-1] the first root-slot input, q <- 0.
+ * prompt: host int32[n], 1 <= n <= max_ctx.  Returns after the work is enqueued. */
+int32_t dex_prefill(dex_ctx* ctx, int32_t seq, const int32_t* prompt, int32_t n);
+
+/* One round of Alg. 1 (lines 5-16) for every active sequence: expand all frontier nodes
+ * through their next stage (one grouped launch per layer op), DECS-decode all new nodes,
+ * insert into B; if the anchor reached final depth: validate_and_commit and, with
+ * DEX_STEP_AUTOCOLLAPSE, collapse; else advance.  Without the flag a sequence whose anchor
+ * reached final depth is left pending and must be finished with dex_collapse before the
+ * next dex_step (DEX_ESTATE otherwise).  out: host dex_step_result[max_seqs].  Returns
+ * after the results are visible on the host. */
+int32_t dex_step(dex_ctx* ctx, uint32_t flags, dex_step_result* out);
+
+/* collapse(B, S, q, b) as a primitive (Alg. 1 line 13): commit `token`
+ * for sequence `seq`, append the root slot's K/V of all L layers to the committed pages,
+ * keep the sub-tree consistent with anchor branch `branch_k` (N-1 = fallback: nothing
+ * survives) and compact B, frontier hidden rows and slot K/V in place.  DEX_ESTATE unless a
+ * commit is pending; DEX_EINVAL if branch_k < N-1 and B[anchor(branch_k)] != token.
+ * Used by tests and by the parity harness to teacher-force the oracle's token (R17). */
+int32_t dex_collapse(dex_ctx* ctx, int32_t seq, int32_t branch_k, int32_t token);
+
+/* Committed tokens of a sequence (prompt included) -> host int32[cap]; *n_out = count. */
+int32_t dex_get_tokens(dex_ctx* ctx, int32_t seq, int32_t* out, int32_t cap, int32_t* n_out);
+
+/* Debug taps (cfg.debug_taps = 1 only; DEX_ESTATE otherwise).  dst: HOST buffers.
+ *   DEX_TAP_HIDDEN : a = node id of the last round (level q_before) -> float[len_m * d],
+ *                    residual stream after each layer of that node's stage
+ *   DEX_TAP_LOGITS : final-depth anchor logits of the last round -> float[vocab]
+ *                    (recomputed by a plain CUDA-core kernel from the anchor's exit row)
+ *   DEX_TAP_B      : explore buffer B of `seq` -> int32[2^N - 1] (-1 = empty)
+ *   DEX_TAP_FSM    : int32[4] = {q, ctx_len, n_tokens, pending}                         */
+#define DEX_TAP_HIDDEN 1
+#define DEX_TAP_LOGITS 2
+#define DEX_TAP_B      3
+#define DEX_TAP_FSM    4
+int32_t dex_debug_read(dex_ctx* ctx, int32_t what, int32_t seq, int32_t a, void* dst, size_t dst_bytes);
+
+/* Kernel-level tap for parity tests of the weight-streaming GEMM:
+ * y[rows,out] (host f32) = x[rows,k] (host f32, split to bf16 planes on device) . W[out,k]^T
+ * with W = weight kind `which` (0 qkv, 1 o, 2 gate/up, 3 down, 4 lm_head) of layer `layer`,
+ * through exactly the launch configuration dex_step uses.  rows <= 128. */
+int32_t dex_debug_gemm(dex_ctx* ctx, int32_t which, int32_t layer, const float* x, int32_t rows, float* y);
+
+/* Per-kernel-class device time of the last dex_step in microseconds (CUDA events around each
+ * phase; only when cfg.debug_taps = 1, which disables graph replay): float[8] =
+ * {bookkeeping, gemm, glue(norm/rope/silu), attention, exit, commit+collapse, 0, total}. */
+int32_t dex_debug_phase_us(dex_ctx* ctx, float* out8);
+
+int32_t dex_destroy(dex_ctx* ctx);
+const char* dex_last_error(const dex_ctx* ctx);   /* ctx may be NULL: last global error */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DEX_B200_H */

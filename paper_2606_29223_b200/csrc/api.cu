@@ -1,0 +1,771 @@
+// api.cu — the C ABI of include/dex.h: context, workspace carving, TMA descriptors, page
+// allocator, launch sequence of one DEX round (Alg. 1 lines 5-16), prefill,
+// collapse primitive, debug taps.  Host logic only; every step of the path runs in the kernels.
+#include <algorithm>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <map>
+#include <memory>
+#include <string>
+#include <vector>
+
+#include "common.cuh"
+
+namespace dexk {
+cudaError_t gemm_init();
+cudaError_t launch_gemm(const CUtensorMap&, const CUtensorMap&, const GemmArgs&, int, size_t, cudaStream_t);
+cudaError_t launch_rows_decode(const Dev&, const Plan&, cudaStream_t);
+cudaError_t launch_rows_prefill(const Dev&, int, int, int, cudaStream_t);
+cudaError_t launch_seq_init(const Dev&, int, int, cudaStream_t);
+cudaError_t launch_rope_table(const Dev&, double, int, cudaStream_t);
+cudaError_t launch_gather_norm(const Dev&, const Plan&, int, cudaStream_t);
+cudaError_t launch_add_norm(const Dev&, const Plan&, int, int, int, int, size_t, cudaStream_t);
+cudaError_t launch_rope_kv(const Dev&, const Plan&, int, int, int, size_t, cudaStream_t);
+cudaError_t launch_silu_mul(const Dev&, const Plan&, int, int, int, size_t, cudaStream_t);
+cudaError_t launch_attn(const Dev&, const Plan&, int, int, int, cudaStream_t);
+cudaError_t launch_decide(const Dev&, const Plan&, int, cudaStream_t);
+cudaError_t launch_set_cmd(const Dev&, int, int, int, cudaStream_t);
+cudaError_t launch_collapse(const Dev&, const Plan&, int, cudaStream_t);
+cudaError_t launch_tap_logits(const Dev&, int, float*, cudaStream_t);
+cudaError_t launch_debug_rows(const Dev&, int, cudaStream_t);
+cudaError_t launch_debug_split(const float*, __nv_bfloat16*, int, int, size_t, int, cudaStream_t);
+cudaError_t launch_debug_sum(const float*, float*, int, int, int, int, size_t, cudaStream_t);
+}  // namespace dexk
+
+using namespace dexk;
+
+namespace {
+
+std::string g_last_error;
+
+struct OpCfg {          // one projection: Y = X . W^T
+  CUtensorMap tmW;
+  int out, k, n_tiles, ksplit, kbps, kb_total;
+};
+struct RingCfg {        // shared-memory ring of the GEMM for a plan
+  int x_cap, n_stages, acc_cols;
+  size_t smem;
+};
+struct HostSeq {
+  int active = 0, q = 0, ctx_len = 0, n_tok = 0, pending = 0, done = 0;
+  int anchor_tokens[DEX_MAX_DEPTHS];
+  int last_q_before = 0;
+  std::vector<int> pages;
+};
+enum Phase { PH_BOOK = 0, PH_GEMM, PH_GLUE, PH_ATTN, PH_EXIT, PH_COMMIT, PH_N };
+
+}  // namespace
+
+struct dex_ctx {
+  dex_config cfg;
+  Dev D;
+  Plan dec_plan, pre_plan, exit_plan;
+  RingCfg dec_ring, pre_ring, exit_ring;
+  OpCfg op[5];                        // qkv, o, gate/up, down, lm_head
+  CUtensorMap tmX[4];                 // act_a, act_o, act_f, act_e
+  cudaStream_t stream;
+  int n_sms;
+  std::vector<HostSeq> seqs;
+  std::vector<int> free_pages;
+  std::vector<int> page_table_host;
+  dex_step_result* result_host;       // pinned, mapped
+  float* dbg_stage;                   // device staging for debug taps (taps only)
+  size_t dbg_floats;
+  size_t part_split_stride;
+  std::map<long long, cudaGraphExec_t> graphs;
+  std::string err;
+  // phase timing (taps only)
+  std::vector<std::pair<cudaEvent_t, cudaEvent_t>> ev[PH_N];
+  size_t ev_used[PH_N];
+  float phase_us[8];
+};
+
+namespace {
+
+int fail(dex_ctx* c, int code, const char* fmt, ...) {
+  char buf[512];
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(buf, sizeof buf, fmt, ap);
+  va_end(ap);
+  g_last_error = buf;
+  if (c) c->err = buf;
+  return code;
+}
+#define CU(c, call)                                                                      \
+  do {                                                                                   \
+    cudaError_t e_ = (call);                                                             \
+    if (e_ != cudaSuccess) return fail(c, DEX_ECUDA, "%s: %s", #call, cudaGetErrorString(e_)); \
+  } while (0)
+
+size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+int round16i(int v) { return (v + 15) & ~15; }
+
+int validate(const dex_config* cfg, const int32_t* depths, int32_t n) {
+  if (!cfg || !depths) return fail(nullptr, DEX_EINVAL, "null config / depths");
+  if (n < 1 || n > DEX_MAX_DEPTHS) return fail(nullptr, DEX_EINVAL, "n_depths must be in [1,%d]", DEX_MAX_DEPTHS);
+  for (int i = 0; i < n; ++i) {
+    if (depths[i] < 1 || depths[i] > cfg->n_layers || (i && depths[i] <= depths[i - 1]))
+      return fail(nullptr, DEX_EINVAL, "exploration set must be strictly increasing in [1,L] (Def. 4)");
+  }
+  if (depths[n - 1] != cfg->n_layers) return fail(nullptr, DEX_EINVAL, "exploration set must end at L (Def. 4)");
+  if (cfg->head_dim != 64 && cfg->head_dim != 128) return fail(nullptr, DEX_EINVAL, "head_dim must be 64 or 128");
+  if (cfg->n_kv_heads < 1 || cfg->n_heads % cfg->n_kv_heads) return fail(nullptr, DEX_EINVAL, "n_kv_heads must divide n_heads");
+  if (cfg->d_model % 8 || cfg->d_ffn % 8) return fail(nullptr, DEX_EINVAL, "d_model and d_ffn must be multiples of 8");
+  if (cfg->page_size < 64 || cfg->page_size % 64) return fail(nullptr, DEX_EINVAL, "page_size must be a multiple of 64");
+  if (cfg->max_seqs < 1 || cfg->max_seqs > 8) return fail(nullptr, DEX_EINVAL, "max_seqs must be in [1,8]");
+  if (cfg->max_ctx < 2) return fail(nullptr, DEX_EINVAL, "max_ctx too small");
+  if (cfg->act_planes != 1 && cfg->act_planes != 2) return fail(nullptr, DEX_EINVAL, "act_planes must be 1 or 2");
+  if (cfg->vocab < 2) return fail(nullptr, DEX_EINVAL, "vocab too small");
+  if (cfg->max_seqs * cap_of(n, 0) > 256) return fail(nullptr, DEX_ECAPACITY, "max_seqs * 2^(N-2) rows exceed 256 per stage");
+  return DEX_OK;
+}
+
+void choose_split(OpCfg& o, bool allow_split) {
+  o.n_tiles = (o.out + kTileM - 1) / kTileM;
+  o.kb_total = (o.k + kTileK - 1) / kTileK;
+  int S = 1;
+  if (allow_split)
+    while (S < 8 && o.n_tiles * S < 256 && S * 2 <= o.kb_total) S *= 2;
+  o.kbps = (o.kb_total + S - 1) / S;
+  o.ksplit = (o.kb_total + o.kbps - 1) / o.kbps;
+}
+
+// Shape-only quantities shared by dex_workspace_bytes and dex_init.
+struct Layout {
+  int N, R_dec, R_cap, part_ld, s_max, max_chunks, n_slots, n_nodes, pages_per_seq, n_pages, max_len, ref_tiles;
+  Plan dec, pre, ext;
+  OpCfg op[5];
+  size_t off[40];
+  size_t total;
+  size_t dbg_floats;
+};
+enum Buf {
+  B_SEQS, B_TOKENS, B_B, B_PT, B_ROWS, B_GNB, B_ENB, B_KEY, B_REFT, B_CMD, B_KPOOL, B_VPOOL, B_KSLOT, B_VSLOT,
+  B_XCUR, B_XFRONT, B_ACTA, B_ACTO, B_ACTF, B_ACTE, B_PART, B_QBUF, B_APART, B_ROPE, B_TAPH, B_DBG, B_COUNT
+};
+
+void make_layout(const dex_config& c, const int32_t* depths, int n, Layout& L) {
+  memset(&L, 0, sizeof(Layout));
+  L.N = n;
+  L.n_nodes = (1 << n) - 1;
+  L.n_slots = 1 << (n - 1);
+  int base = 0;
+  L.dec.n_grp = n;
+  L.max_len = 0;
+  for (int m = 0; m < n; ++m) {
+    L.dec.row_base[m] = base;
+    L.dec.rows_cap[m] = round16i(c.max_seqs * cap_of(n, m));
+    L.dec.layer_lo[m] = m ? depths[m - 1] : 0;
+    L.dec.layer_len[m] = depths[m] - L.dec.layer_lo[m];
+    L.max_len = std::max(L.max_len, L.dec.layer_len[m]);
+    base += L.dec.rows_cap[m];
+  }
+  L.R_dec = base;
+  L.R_cap = round16i(std::max(L.R_dec, kPrefillRows));
+  L.pre.n_grp = 1;
+  L.pre.row_base[0] = 0;
+  L.pre.rows_cap[0] = kPrefillRows;
+  L.pre.layer_lo[0] = 0;
+  L.pre.layer_len[0] = c.n_layers;
+  L.ext.n_grp = (L.R_dec + 255) / 256;
+  for (int g = 0; g < L.ext.n_grp; ++g) {
+    L.ext.row_base[g] = 256 * g;
+    L.ext.rows_cap[g] = std::min(256, L.R_dec - 256 * g);
+    L.ext.layer_lo[g] = 0;
+    L.ext.layer_len[g] = 1;
+  }
+  const int qkv_out = (c.n_heads + 2 * c.n_kv_heads) * c.head_dim;
+  const int outs[5] = {qkv_out, c.d_model, 2 * c.d_ffn, c.d_model, c.vocab};
+  const int ks[5] = {c.d_model, c.n_heads * c.head_dim, c.d_model, c.d_ffn, c.d_model};
+  L.s_max = 1;
+  for (int i = 0; i < 5; ++i) {
+    L.op[i].out = outs[i];
+    L.op[i].k = ks[i];
+    choose_split(L.op[i], i != 4);
+    if (i != 4) L.s_max = std::max(L.s_max, L.op[i].ksplit);
+  }
+  L.part_ld = (int)align_up(std::max(std::max(qkv_out, 2 * c.d_ffn), c.d_model), 4);
+  L.max_chunks = (c.max_ctx + n) / kChunk + 1;
+  L.pages_per_seq = (c.max_ctx + c.page_size - 1) / c.page_size;
+  L.n_pages = L.pages_per_seq * c.max_seqs;
+  L.ref_tiles = L.op[4].n_tiles * 4;
+  L.dbg_floats = c.debug_taps ? (size_t)kPrefillRows * (std::max(c.d_ffn, c.d_model) + L.part_ld) + c.vocab : 0;
+
+  const size_t kv_pool = (size_t)c.n_layers * L.n_pages * c.page_size * c.n_kv_heads * c.head_dim * 2;
+  const size_t kv_slot = (size_t)c.max_seqs * L.n_slots * c.n_layers * c.n_kv_heads * c.head_dim * 2;
+  const size_t P = c.act_planes, R = L.R_cap;
+  size_t sz[B_COUNT];
+  sz[B_SEQS] = sizeof(SeqState) * c.max_seqs;
+  sz[B_TOKENS] = sizeof(int) * (size_t)c.max_seqs * (c.max_ctx + 1);
+  sz[B_B] = sizeof(int) * (size_t)c.max_seqs * L.n_nodes;
+  sz[B_PT] = sizeof(int) * (size_t)L.n_pages;
+  sz[B_ROWS] = sizeof(RowInfo) * R;
+  sz[B_GNB] = sizeof(int) * kMaxGrp;
+  sz[B_ENB] = sizeof(int) * kMaxGrp;
+  sz[B_KEY] = sizeof(unsigned long long) * R;
+  sz[B_REFT] = sizeof(float2) * (size_t)c.max_seqs * L.ref_tiles;
+  sz[B_CMD] = sizeof(CollapseCmd) * c.max_seqs;
+  sz[B_KPOOL] = kv_pool;
+  sz[B_VPOOL] = kv_pool;
+  sz[B_KSLOT] = kv_slot;
+  sz[B_VSLOT] = kv_slot;
+  sz[B_XCUR] = sizeof(float) * R * c.d_model;
+  sz[B_XFRONT] = sizeof(float) * R * c.d_model;
+  sz[B_ACTA] = 2 * P * R * c.d_model;
+  sz[B_ACTO] = 2 * P * R * c.n_heads * c.head_dim;
+  sz[B_ACTF] = 2 * P * R * c.d_ffn;
+  sz[B_ACTE] = 2 * P * R * c.d_model;
+  sz[B_PART] = sizeof(float) * (size_t)L.s_max * R * L.part_ld;
+  sz[B_QBUF] = sizeof(float) * R * c.n_heads * c.head_dim;
+  sz[B_APART] = sizeof(float) * R * c.n_heads * (size_t)L.max_chunks * (c.head_dim + 2);
+  sz[B_ROPE] = sizeof(float2) * (size_t)(c.max_ctx + kMaxAnc + 1) * (c.head_dim / 2);
+  sz[B_TAPH] = c.debug_taps ? sizeof(float) * R * (size_t)L.max_len * c.d_model : 0;
+  sz[B_DBG] = sizeof(float) * L.dbg_floats;
+  size_t off = 0;
+  for (int i = 0; i < B_COUNT; ++i) {
+    L.off[i] = off;
+    off += align_up(sz[i], 1024);
+  }
+  L.total = off;
+}
+
+RingCfg make_ring(const Plan& p, int planes) {
+  RingCfg r;
+  r.x_cap = 16;
+  for (int g = 0; g < p.n_grp; ++g) r.x_cap = std::max(r.x_cap, p.rows_cap[g]);
+  const size_t stage = 16384 + (size_t)planes * r.x_cap * 128;
+  const size_t budget = 200 * 1024;
+  r.n_stages = (int)std::max<size_t>(2, std::min<size_t>(12, budget / stage));
+  r.acc_cols = 32;
+  while (r.acc_cols < r.x_cap) r.acc_cols *= 2;
+  r.smem = r.n_stages * stage + 1024 + 512;
+  return r;
+}
+
+typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                             const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                             CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+int encode_3d(dex_ctx* c, EncodeFn fn, CUtensorMap* tm, const void* base, uint64_t d0, uint64_t d1, uint64_t d2,
+              uint32_t box1) {
+  cuuint64_t dims[3] = {d0, d1, d2};
+  cuuint64_t strides[2] = {d0 * 2, d0 * d1 * 2};
+  cuuint32_t box[3] = {(cuuint32_t)kTileK, box1, 1};
+  cuuint32_t es[3] = {1, 1, 1};
+  CUresult r = fn(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(base), dims, strides, box, es,
+                  CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                  CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return fail(c, DEX_ECUDA, "cuTensorMapEncodeTiled failed (%d)", (int)r);
+  return DEX_OK;
+}
+
+// ---- phase timing (taps only) ----
+void ph_begin(dex_ctx* c, Phase p) {
+  if (!c->cfg.debug_taps) return;
+  if (c->ev_used[p] == c->ev[p].size()) {
+    cudaEvent_t a, b;
+    cudaEventCreate(&a);
+    cudaEventCreate(&b);
+    c->ev[p].push_back({a, b});
+  }
+  cudaEventRecord(c->ev[p][c->ev_used[p]].first, c->stream);
+}
+void ph_end(dex_ctx* c, Phase p) {
+  if (!c->cfg.debug_taps) return;
+  cudaEventRecord(c->ev[p][c->ev_used[p]].second, c->stream);
+  c->ev_used[p]++;
+}
+
+int run_gemm(dex_ctx* c, int which, const CUtensorMap& tmX, const Plan& plan, const RingCfg& ring, int step, int mode,
+             const int* grp_nb) {
+  const OpCfg& o = c->op[which];
+  GemmArgs a;
+  memset(&a, 0, sizeof a);
+  a.plan = plan;
+  a.step = step;
+  a.out_dim = o.out;
+  a.k_dim = o.k;
+  a.n_tiles = o.n_tiles;
+  a.ksplit = o.ksplit;
+  a.kb_per_split = o.kbps;
+  a.kb_total = o.kb_total;
+  a.planes = c->cfg.act_planes;
+  a.mode = mode;
+  a.x_cap = ring.x_cap;
+  a.n_stages = ring.n_stages;
+  a.acc_cols = ring.acc_cols;
+  a.grp_nb = grp_nb;
+  a.rows = c->D.rows;
+  a.part = c->D.part;
+  a.part_ld = c->D.part_ld;
+  a.part_split_stride = c->part_split_stride;
+  a.best_key = c->D.best_key;
+  a.ref_tile = c->D.ref_tile;
+  a.ref_tiles = c->D.ref_tiles;
+  a.vocab = c->D.vocab;
+  if (which == 4) {   // the LM head is one [V, d] matrix: every exit chunk streams "layer" 0
+    for (int g = 0; g < kMaxGrp; ++g) a.plan.layer_lo[g] = 0;
+  }
+  CU(c, launch_gemm(o.tmW, tmX, a, c->n_sms, ring.smem, c->stream));
+  return DEX_OK;
+}
+
+// Layers of one plan: for j = 0 .. max_len-1, every live group runs its layer lo+j (a2 + a3).
+int enqueue_layers(dex_ctx* c, const Plan& plan, const RingCfg& ring, int rows, int n_chunks, int max_len) {
+  const Dev& D = c->D;
+  const size_t ss = c->part_split_stride;
+  for (int j = 0; j < max_len; ++j) {
+    int rc;
+    ph_begin(c, PH_GEMM);
+    rc = run_gemm(c, 0, c->tmX[0], plan, ring, j, 0, D.grp_nb);
+    ph_end(c, PH_GEMM);
+    if (rc) return rc;
+    ph_begin(c, PH_GLUE);
+    CU(c, launch_rope_kv(D, plan, rows, j, c->op[0].ksplit, ss, c->stream));
+    ph_end(c, PH_GLUE);
+    ph_begin(c, PH_ATTN);
+    CU(c, launch_attn(D, plan, rows, j, n_chunks, c->stream));
+    ph_end(c, PH_ATTN);
+    ph_begin(c, PH_GEMM);
+    rc = run_gemm(c, 1, c->tmX[1], plan, ring, j, 0, D.grp_nb);
+    ph_end(c, PH_GEMM);
+    if (rc) return rc;
+    ph_begin(c, PH_GLUE);
+    CU(c, launch_add_norm(D, plan, rows, j, 0, c->op[1].ksplit, ss, c->stream));
+    ph_end(c, PH_GLUE);
+    ph_begin(c, PH_GEMM);
+    rc = run_gemm(c, 2, c->tmX[0], plan, ring, j, 0, D.grp_nb);
+    ph_end(c, PH_GEMM);
+    if (rc) return rc;
+    ph_begin(c, PH_GLUE);
+    CU(c, launch_silu_mul(D, plan, rows, j, c->op[2].ksplit, ss, c->stream));
+    ph_end(c, PH_GLUE);
+    ph_begin(c, PH_GEMM);
+    rc = run_gemm(c, 3, c->tmX[2], plan, ring, j, 0, D.grp_nb);
+    ph_end(c, PH_GEMM);
+    if (rc) return rc;
+    ph_begin(c, PH_GLUE);
+    CU(c, launch_add_norm(D, plan, rows, j, 1, c->op[3].ksplit, ss, c->stream));
+    ph_end(c, PH_GLUE);
+  }
+  return DEX_OK;
+}
+
+int enqueue_collapse(dex_ctx* c) {
+  ph_begin(c, PH_COMMIT);
+  CU(c, launch_collapse(c->D, c->dec_plan, c->cfg.eos_id, c->stream));
+  ph_end(c, PH_COMMIT);
+  return DEX_OK;
+}
+
+int enqueue_step(dex_ctx* c, uint32_t flags, int n_chunks) {
+  const Dev& D = c->D;
+  ph_begin(c, PH_BOOK);
+  CU(c, launch_rows_decode(D, c->dec_plan, c->stream));
+  CU(c, launch_gather_norm(D, c->dec_plan, D.R_dec, c->stream));
+  ph_end(c, PH_BOOK);
+  int rc = enqueue_layers(c, c->dec_plan, c->dec_ring, D.R_dec, n_chunks, D.max_len);
+  if (rc) return rc;
+  ph_begin(c, PH_EXIT);
+  rc = run_gemm(c, 4, c->tmX[3], c->exit_plan, c->exit_ring, 0, 1, D.exit_nb);
+  ph_end(c, PH_EXIT);
+  if (rc) return rc;
+  ph_begin(c, PH_COMMIT);
+  CU(c, launch_decide(D, c->dec_plan, (flags & DEX_STEP_AUTOCOLLAPSE) ? 1 : 0, c->stream));
+  ph_end(c, PH_COMMIT);
+  return enqueue_collapse(c);
+}
+
+int ensure_pages(dex_ctx* c, int s, int n_positions) {
+  HostSeq& hs = c->seqs[s];
+  const int need = (n_positions + c->cfg.page_size - 1) / c->cfg.page_size;
+  if (need > c->D.pages_per_seq) return fail(c, DEX_ECAPACITY, "sequence %d exceeds max_ctx", s);
+  bool changed = false;
+  while ((int)hs.pages.size() < need) {
+    if (c->free_pages.empty()) return fail(c, DEX_ECAPACITY, "out of KV pages");
+    int pg = c->free_pages.back();
+    c->free_pages.pop_back();
+    c->page_table_host[s * c->D.pages_per_seq + hs.pages.size()] = pg;
+    hs.pages.push_back(pg);
+    changed = true;
+  }
+  if (changed)
+    CU(c, cudaMemcpyAsync(c->D.page_table + s * c->D.pages_per_seq, &c->page_table_host[s * c->D.pages_per_seq],
+                          sizeof(int) * c->D.pages_per_seq, cudaMemcpyHostToDevice, c->stream));
+  return DEX_OK;
+}
+
+void collect_phase_times(dex_ctx* c) {
+  if (!c->cfg.debug_taps) return;
+  float total = 0.f;
+  for (int p = 0; p < PH_N; ++p) {
+    float us = 0.f;
+    for (size_t i = 0; i < c->ev_used[p]; ++i) {
+      float ms = 0.f;
+      cudaEventElapsedTime(&ms, c->ev[p][i].first, c->ev[p][i].second);
+      us += ms * 1000.f;
+    }
+    // bookkeeping, gemm, glue, attention, exit, commit+collapse
+    c->phase_us[p] = us;
+    total += us;
+    c->ev_used[p] = 0;
+  }
+  c->phase_us[6] = 0.f;
+  c->phase_us[7] = total;
+}
+
+}  // namespace
+
+// =============================================================================================
+extern "C" {
+
+const char* dex_last_error(const dex_ctx* ctx) { return ctx ? ctx->err.c_str() : g_last_error.c_str(); }
+
+int32_t dex_workspace_bytes(const dex_config* cfg, const int32_t* depths, int32_t n_depths, size_t* out_bytes) {
+  int rc = validate(cfg, depths, n_depths);
+  if (rc) return rc;
+  if (!out_bytes) return fail(nullptr, DEX_EINVAL, "null out_bytes");
+  Layout* L = new Layout;
+  make_layout(*cfg, depths, n_depths, *L);
+  *out_bytes = L->total;
+  delete L;
+  return DEX_OK;
+}
+
+int32_t dex_init(dex_ctx** out, const dex_config* cfg, const dex_weights* w, const int32_t* depths, int32_t n_depths,
+                 void* workspace, size_t workspace_bytes, void* cuda_stream) {
+  if (!out) return fail(nullptr, DEX_EINVAL, "null out");
+  *out = nullptr;
+  int rc = validate(cfg, depths, n_depths);
+  if (rc) return rc;
+  if (!w || !w->embed || !w->lm_head || !w->wqkv || !w->wo || !w->wgu || !w->wdn || !w->norm_attn || !w->norm_ffn ||
+      !w->norm_final)
+    return fail(nullptr, DEX_EINVAL, "null weight pointer");
+  if (!workspace || (reinterpret_cast<uintptr_t>(workspace) & 1023)) return fail(nullptr, DEX_EINVAL, "workspace must be 1024-byte aligned");
+  std::unique_ptr<Layout> Lp(new Layout);
+  Layout& L = *Lp;
+  make_layout(*cfg, depths, n_depths, L);
+  if (workspace_bytes < L.total) return fail(nullptr, DEX_ECAPACITY, "workspace too small: need %zu bytes", L.total);
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0)
+    return fail(nullptr, DEX_ECUDA, "no CUDA device: this library has no CPU fallback");
+  dex_ctx* c = new dex_ctx;
+  c->cfg = *cfg;
+  c->stream = static_cast<cudaStream_t>(cuda_stream);
+  c->dec_plan = L.dec;
+  c->pre_plan = L.pre;
+  c->exit_plan = L.ext;
+  c->result_host = nullptr;
+  memset(c->ev_used, 0, sizeof c->ev_used);
+  memset(c->phase_us, 0, sizeof c->phase_us);
+  int dev = 0;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&c->n_sms, cudaDevAttrMultiProcessorCount, dev);
+
+  Dev& D = c->D;
+  memset(&D, 0, sizeof D);
+  D.L = cfg->n_layers; D.d = cfg->d_model; D.nh = cfg->n_heads; D.nkv = cfg->n_kv_heads; D.hd = cfg->head_dim;
+  D.ffn = cfg->d_ffn; D.vocab = cfg->vocab; D.qkv_out = (cfg->n_heads + 2 * cfg->n_kv_heads) * cfg->head_dim;
+  D.eps = cfg->rms_eps; D.N = n_depths;
+  for (int i = 0; i < n_depths; ++i) D.depths[i] = depths[i];
+  D.max_seqs = cfg->max_seqs; D.max_ctx = cfg->max_ctx; D.page_size = cfg->page_size;
+  D.pages_per_seq = L.pages_per_seq; D.n_pages = L.n_pages; D.n_slots = L.n_slots; D.n_nodes = L.n_nodes;
+  D.R_cap = L.R_cap; D.R_dec = L.R_dec; D.decs = cfg->decs; D.planes = cfg->act_planes; D.taps = cfg->debug_taps;
+  D.max_len = L.max_len; D.part_ld = L.part_ld; D.max_chunks = L.max_chunks; D.ref_tiles = L.ref_tiles;
+  D.embed = static_cast<const __nv_bfloat16*>(w->embed);
+  D.lm_head = static_cast<const __nv_bfloat16*>(w->lm_head);
+  D.norm_attn = w->norm_attn; D.norm_ffn = w->norm_ffn; D.norm_final = w->norm_final;
+  uint8_t* ws = static_cast<uint8_t*>(workspace);
+#define WSP(T, b) reinterpret_cast<T*>(ws + L.off[b])
+  D.seqs = WSP(SeqState, B_SEQS); D.tokens = WSP(int, B_TOKENS); D.B = WSP(int, B_B); D.page_table = WSP(int, B_PT);
+  D.rows = WSP(RowInfo, B_ROWS); D.grp_nb = WSP(int, B_GNB); D.exit_nb = WSP(int, B_ENB);
+  D.best_key = WSP(unsigned long long, B_KEY); D.ref_tile = WSP(float2, B_REFT); D.cmd = WSP(CollapseCmd, B_CMD);
+  D.kpool = WSP(__nv_bfloat16, B_KPOOL); D.vpool = WSP(__nv_bfloat16, B_VPOOL);
+  D.kslot = WSP(__nv_bfloat16, B_KSLOT); D.vslot = WSP(__nv_bfloat16, B_VSLOT);
+  D.x_cur = WSP(float, B_XCUR); D.x_front = WSP(float, B_XFRONT);
+  D.act_a = WSP(__nv_bfloat16, B_ACTA); D.act_o = WSP(__nv_bfloat16, B_ACTO);
+  D.act_f = WSP(__nv_bfloat16, B_ACTF); D.act_e = WSP(__nv_bfloat16, B_ACTE);
+  D.part = WSP(float, B_PART); D.qbuf = WSP(float, B_QBUF); D.attn_part = WSP(float, B_APART);
+  D.rope = WSP(float2, B_ROPE); D.tap_hidden = cfg->debug_taps ? WSP(float, B_TAPH) : nullptr;
+  c->dbg_stage = cfg->debug_taps ? WSP(float, B_DBG) : nullptr;
+  c->dbg_floats = L.dbg_floats;
+#undef WSP
+  c->part_split_stride = (size_t)L.R_cap * L.part_ld;
+  for (int i = 0; i < 5; ++i) c->op[i] = L.op[i];
+  c->dec_ring = make_ring(c->dec_plan, cfg->act_planes);
+  c->pre_ring = make_ring(c->pre_plan, cfg->act_planes);
+  c->exit_ring = make_ring(c->exit_plan, cfg->act_planes);
+
+#define INIT_FAIL(expr)          \
+  do {                           \
+    int rc_ = (expr);            \
+    if (rc_) {                   \
+      g_last_error = c->err;     \
+      delete c;                  \
+      return rc_;                \
+    }                            \
+  } while (0)
+
+  // TMA descriptors (driver entry point fetched at run time: no link-time libcuda dependency)
+  void* fnp = nullptr;
+  cudaDriverEntryPointQueryResult qres;
+  if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fnp, cudaEnableDefault, &qres) != cudaSuccess || !fnp) {
+    delete c;
+    return fail(nullptr, DEX_ECUDA, "cuTensorMapEncodeTiled entry point not found");
+  }
+  EncodeFn enc = reinterpret_cast<EncodeFn>(fnp);
+  if (gemm_init() != cudaSuccess) {
+    delete c;
+    return fail(nullptr, DEX_ECUDA, "cannot raise the GEMM kernel's dynamic shared memory limit");
+  }
+  const void* wptr[5] = {w->wqkv, w->wo, w->wgu, w->wdn, w->lm_head};
+  for (int i = 0; i < 5; ++i)
+    INIT_FAIL(encode_3d(c, enc, &c->op[i].tmW, wptr[i], c->op[i].k, c->op[i].out, i == 4 ? 1 : D.L, kTileM));
+  const void* xptr[4] = {D.act_a, D.act_o, D.act_f, D.act_e};
+  const int xk[4] = {D.d, D.nh * D.hd, D.ffn, D.d};
+  for (int i = 0; i < 4; ++i)
+    INIT_FAIL(encode_3d(c, enc, &c->tmX[i], xptr[i], xk[i], D.R_cap, cfg->act_planes, kBoxRows));
+
+  // state: FSM zeroed, free pages, result buffer, RoPE table
+  auto cu_or_fail = [&](cudaError_t e, const char* what) -> int {
+    if (e != cudaSuccess) return fail(c, DEX_ECUDA, "%s: %s", what, cudaGetErrorString(e));
+    return DEX_OK;
+  };
+  INIT_FAIL(cu_or_fail(cudaMemsetAsync(ws, 0, L.off[B_KPOOL], c->stream), "memset state"));
+  INIT_FAIL(cu_or_fail(cudaMemsetAsync(D.rows, 0, sizeof(RowInfo) * D.R_cap, c->stream), "memset rows"));
+  INIT_FAIL(cu_or_fail(cudaHostAlloc(reinterpret_cast<void**>(&c->result_host), sizeof(dex_step_result) * cfg->max_seqs,
+                                     cudaHostAllocMapped),
+                       "cudaHostAlloc"));
+  memset(c->result_host, 0, sizeof(dex_step_result) * cfg->max_seqs);
+  INIT_FAIL(cu_or_fail(cudaHostGetDevicePointer(reinterpret_cast<void**>(&D.result_dev), c->result_host, 0),
+                       "cudaHostGetDevicePointer"));
+  c->seqs.resize(cfg->max_seqs);
+  c->page_table_host.assign((size_t)D.n_pages, 0);
+  for (int p = D.n_pages - 1; p >= 0; --p) c->free_pages.push_back(p);
+  INIT_FAIL(cu_or_fail(launch_rope_table(D, (double)cfg->rope_theta, cfg->max_ctx + kMaxAnc + 1, c->stream), "rope table"));
+  INIT_FAIL(cu_or_fail(cudaStreamSynchronize(c->stream), "init sync"));
+#undef INIT_FAIL
+  *out = c;
+  return DEX_OK;
+}
+
+int32_t dex_destroy(dex_ctx* c) {
+  if (!c) return DEX_OK;
+  cudaStreamSynchronize(c->stream);
+  for (auto& kv : c->graphs) cudaGraphExecDestroy(kv.second);
+  for (int p = 0; p < PH_N; ++p)
+    for (auto& e : c->ev[p]) {
+      cudaEventDestroy(e.first);
+      cudaEventDestroy(e.second);
+    }
+  if (c->result_host) cudaFreeHost(c->result_host);
+  delete c;
+  return DEX_OK;
+}
+
+int32_t dex_prefill(dex_ctx* c, int32_t seq, const int32_t* prompt, int32_t n) {
+  if (!c) return fail(nullptr, DEX_EINVAL, "null ctx");
+  if (seq < 0 || seq >= c->cfg.max_seqs) return fail(c, DEX_EINVAL, "seq out of range");
+  if (!prompt || n < 1) return fail(c, DEX_EINVAL, "empty prompt");
+  if (n > c->cfg.max_ctx) return fail(c, DEX_ECAPACITY, "prompt longer than max_ctx");
+  for (int i = 0; i < n; ++i)
+    if (prompt[i] < 0 || prompt[i] >= c->cfg.vocab) return fail(c, DEX_EINVAL, "prompt token out of range");
+  HostSeq& hs = c->seqs[seq];
+  for (int pg : hs.pages) c->free_pages.push_back(pg);   // reset the sequence
+  hs = HostSeq();
+  const Dev& D = c->D;
+  int rc = ensure_pages(c, seq, n);
+  if (rc) return rc;
+  CU(c, cudaMemcpyAsync(D.tokens + (size_t)seq * (D.max_ctx + 1), prompt, sizeof(int) * n, cudaMemcpyHostToDevice, c->stream));
+  for (int p0 = 0; p0 < n - 1; p0 += kPrefillRows) {
+    const int R = std::min(kPrefillRows, n - 1 - p0);
+    CU(c, launch_rows_prefill(D, seq, p0, R, c->stream));
+    CU(c, launch_gather_norm(D, c->pre_plan, R, c->stream));
+    const int n_chunks = (p0 + R - 1) / kChunk + 1;
+    rc = enqueue_layers(c, c->pre_plan, c->pre_ring, R, n_chunks, D.L);
+    if (rc) return rc;
+  }
+  CU(c, launch_seq_init(D, seq, n, c->stream));
+  CU(c, cudaStreamSynchronize(c->stream));   // prompt is a caller buffer: copies must have completed
+  for (int p = 0; p < PH_N; ++p) c->ev_used[p] = 0;
+  hs.active = 1; hs.q = 0; hs.ctx_len = n - 1; hs.n_tok = n; hs.pending = 0; hs.done = (n >= c->cfg.max_ctx);
+  return DEX_OK;
+}
+
+int32_t dex_step(dex_ctx* c, uint32_t flags, dex_step_result* out) {
+  if (!c || !out) return fail(c, DEX_EINVAL, "null argument");
+  const Dev& D = c->D;
+  int n_live = 0, max_pos = 0;
+  for (int s = 0; s < c->cfg.max_seqs; ++s) {
+    HostSeq& hs = c->seqs[s];
+    if (hs.active && hs.pending) return fail(c, DEX_ESTATE, "sequence %d has a pending commit: call dex_collapse", s);
+    if (!hs.active || hs.done) continue;
+    int rc = ensure_pages(c, s, hs.ctx_len + 1);
+    if (rc) return rc;
+    ++n_live;
+    max_pos = std::max(max_pos, hs.ctx_len + D.N - 1);
+  }
+  if (n_live > 0) {
+    const int n_chunks = max_pos / kChunk + 1;
+    if (c->cfg.use_graph && !c->cfg.debug_taps) {
+      const long long key = ((long long)n_chunks << 8) | (flags & 0xff);
+      auto it = c->graphs.find(key);
+      if (it == c->graphs.end()) {
+        cudaGraph_t g;
+        CU(c, cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal));
+        int rc = enqueue_step(c, flags, n_chunks);
+        cudaError_t e = cudaStreamEndCapture(c->stream, &g);
+        if (rc) return rc;
+        CU(c, e);
+        cudaGraphExec_t ge;
+        CU(c, cudaGraphInstantiate(&ge, g, 0));
+        cudaGraphDestroy(g);
+        it = c->graphs.emplace(key, ge).first;
+      }
+      CU(c, cudaGraphLaunch(it->second, c->stream));
+    } else {
+      int rc = enqueue_step(c, flags, n_chunks);
+      if (rc) return rc;
+    }
+    CU(c, cudaStreamSynchronize(c->stream));
+    collect_phase_times(c);
+  }
+  for (int s = 0; s < c->cfg.max_seqs; ++s) {
+    HostSeq& hs = c->seqs[s];
+    if (n_live == 0 || !hs.active || hs.done) {
+      memset(&out[s], 0, sizeof(dex_step_result));
+      out[s].token = -1; out[s].match_k = -1;
+      out[s].q_before = out[s].q_after = hs.q; out[s].n_tokens = hs.n_tok; out[s].done = hs.done;
+      for (int i = 0; i < DEX_MAX_DEPTHS; ++i) out[s].anchor_tokens[i] = -1;
+      continue;
+    }
+    out[s] = c->result_host[s];
+    hs.last_q_before = out[s].q_before;
+    hs.q = out[s].q_after;
+    hs.n_tok = out[s].n_tokens;
+    hs.ctx_len = hs.n_tok - 1;
+    hs.done = out[s].done;
+    hs.pending = (!out[s].committed && out[s].q_before == D.N - 1) ? 1 : 0;
+    memcpy(hs.anchor_tokens, out[s].anchor_tokens, sizeof hs.anchor_tokens);
+  }
+  return DEX_OK;
+}
+
+int32_t dex_collapse(dex_ctx* c, int32_t seq, int32_t branch_k, int32_t token) {
+  if (!c) return fail(nullptr, DEX_EINVAL, "null ctx");
+  if (seq < 0 || seq >= c->cfg.max_seqs) return fail(c, DEX_EINVAL, "seq out of range");
+  HostSeq& hs = c->seqs[seq];
+  const int N = c->D.N;
+  if (!hs.active || !hs.pending) return fail(c, DEX_ESTATE, "no pending commit: the anchor is not at final depth");
+  if (branch_k < 0 || branch_k > N - 1) return fail(c, DEX_EINVAL, "branch_k out of range");
+  if (token < 0 || token >= c->cfg.vocab) return fail(c, DEX_EINVAL, "token out of range");
+  if (branch_k < N - 1 && hs.anchor_tokens[branch_k] != token)
+    return fail(c, DEX_EINVAL, "B[anchor(%d)] = %d != token %d", branch_k, hs.anchor_tokens[branch_k], token);
+  CU(c, launch_set_cmd(c->D, seq, branch_k, token, c->stream));
+  int rc = enqueue_collapse(c);
+  if (rc) return rc;
+  CU(c, cudaStreamSynchronize(c->stream));
+  for (int p = 0; p < PH_N; ++p) c->ev_used[p] = 0;
+  hs.pending = 0;
+  hs.q = (branch_k < N - 1) ? (N - 1 - branch_k) : 0;
+  hs.n_tok += 1;
+  hs.ctx_len += 1;
+  hs.done = (hs.n_tok >= c->cfg.max_ctx || token == c->cfg.eos_id) ? 1 : 0;
+  return DEX_OK;
+}
+
+int32_t dex_get_tokens(dex_ctx* c, int32_t seq, int32_t* out, int32_t cap, int32_t* n_out) {
+  if (!c || !out || !n_out) return fail(c, DEX_EINVAL, "null argument");
+  if (seq < 0 || seq >= c->cfg.max_seqs) return fail(c, DEX_EINVAL, "seq out of range");
+  const int n = std::min(cap, c->seqs[seq].n_tok);
+  *n_out = c->seqs[seq].n_tok;
+  if (n > 0) {
+    CU(c, cudaMemcpyAsync(out, c->D.tokens + (size_t)seq * (c->D.max_ctx + 1), sizeof(int) * n, cudaMemcpyDeviceToHost, c->stream));
+    CU(c, cudaStreamSynchronize(c->stream));
+  }
+  return DEX_OK;
+}
+
+int32_t dex_debug_read(dex_ctx* c, int32_t what, int32_t seq, int32_t a, void* dst, size_t dst_bytes) {
+  if (!c || !dst) return fail(c, DEX_EINVAL, "null argument");
+  if (seq < 0 || seq >= c->cfg.max_seqs) return fail(c, DEX_EINVAL, "seq out of range");
+  const Dev& D = c->D;
+  const HostSeq& hs = c->seqs[seq];
+  if (what == DEX_TAP_FSM) {
+    if (dst_bytes < 4 * sizeof(int)) return fail(c, DEX_EINVAL, "dst too small");
+    SeqState st;
+    CU(c, cudaMemcpyAsync(&st, D.seqs + seq, sizeof st, cudaMemcpyDeviceToHost, c->stream));
+    CU(c, cudaStreamSynchronize(c->stream));
+    int* o = static_cast<int*>(dst);
+    o[0] = st.q; o[1] = st.ctx_len; o[2] = st.n_tok; o[3] = st.pending;
+    return DEX_OK;
+  }
+  if (what == DEX_TAP_B) {
+    if (dst_bytes < sizeof(int) * D.n_nodes) return fail(c, DEX_EINVAL, "dst too small");
+    CU(c, cudaMemcpyAsync(dst, D.B + (size_t)seq * D.n_nodes, sizeof(int) * D.n_nodes, cudaMemcpyDeviceToHost, c->stream));
+    CU(c, cudaStreamSynchronize(c->stream));
+    return DEX_OK;
+  }
+  if (!c->cfg.debug_taps) return fail(c, DEX_ESTATE, "debug_taps is off");
+  if (what == DEX_TAP_HIDDEN) {
+    const int q = hs.last_q_before;
+    const int o = a - ((1 << q) - 1);
+    if (o < 0 || o >= (1 << q)) return fail(c, DEX_EINVAL, "node %d is not on the last round's level %d", a, q);
+    const int m = stage_of(q, o);
+    const int row = c->dec_plan.row_base[m] + seq * cap_of(D.N, m) + idx_in_stage(q, o, m);
+    const size_t bytes = sizeof(float) * (size_t)c->dec_plan.layer_len[m] * D.d;
+    if (dst_bytes < bytes) return fail(c, DEX_EINVAL, "dst too small");
+    CU(c, cudaMemcpyAsync(dst, D.tap_hidden + (size_t)row * D.max_len * D.d, bytes, cudaMemcpyDeviceToHost, c->stream));
+    CU(c, cudaStreamSynchronize(c->stream));
+    return DEX_OK;
+  }
+  if (what == DEX_TAP_LOGITS) {
+    if (hs.last_q_before != D.N - 1) return fail(c, DEX_ESTATE, "the last round did not reach final depth");
+    if (dst_bytes < sizeof(float) * D.vocab) return fail(c, DEX_EINVAL, "dst too small");
+    const int row = c->dec_plan.row_base[D.N - 1] + seq * cap_of(D.N, D.N - 1);
+    float* tmp = c->dbg_stage + (c->dbg_floats - D.vocab);
+    CU(c, launch_tap_logits(D, row, tmp, c->stream));
+    CU(c, cudaMemcpyAsync(dst, tmp, sizeof(float) * D.vocab, cudaMemcpyDeviceToHost, c->stream));
+    CU(c, cudaStreamSynchronize(c->stream));
+    return DEX_OK;
+  }
+  return fail(c, DEX_EINVAL, "unknown tap %d", what);
+}
+
+int32_t dex_debug_gemm(dex_ctx* c, int32_t which, int32_t layer, const float* x, int32_t rows, float* y) {
+  if (!c || !x || !y) return fail(c, DEX_EINVAL, "null argument");
+  if (!c->cfg.debug_taps) return fail(c, DEX_ESTATE, "debug_taps is off");
+  if (which < 0 || which > 3) return fail(c, DEX_EINVAL, "which must be 0..3");
+  if (layer < 0 || layer >= c->D.L) return fail(c, DEX_EINVAL, "layer out of range");
+  if (rows < 1 || rows > kPrefillRows) return fail(c, DEX_EINVAL, "rows must be in [1,128]");
+  const Dev& D = c->D;
+  const OpCfg& o = c->op[which];
+  __nv_bfloat16* act[4] = {D.act_a, D.act_o, D.act_a, D.act_f};
+  const int xm[4] = {0, 1, 0, 2};
+  float* xs = c->dbg_stage;
+  float* ys = c->dbg_stage + (size_t)kPrefillRows * std::max(D.ffn, D.d);
+  CU(c, cudaMemcpyAsync(xs, x, sizeof(float) * (size_t)rows * o.k, cudaMemcpyHostToDevice, c->stream));
+  CU(c, launch_debug_rows(D, rows, c->stream));
+  CU(c, launch_debug_split(xs, act[which], rows, o.k, (size_t)D.R_cap * o.k, D.planes, c->stream));
+  Plan p = c->pre_plan;
+  p.layer_lo[0] = layer;
+  p.layer_len[0] = 1;
+  int rc = run_gemm(c, which, c->tmX[xm[which]], p, c->pre_ring, 0, 0, D.grp_nb);
+  if (rc) return rc;
+  CU(c, launch_debug_sum(D.part, ys, rows, o.out, D.part_ld, o.ksplit, c->part_split_stride, c->stream));
+  CU(c, cudaMemcpyAsync(y, ys, sizeof(float) * (size_t)rows * o.out, cudaMemcpyDeviceToHost, c->stream));
+  CU(c, cudaStreamSynchronize(c->stream));
+  for (int ph = 0; ph < PH_N; ++ph) c->ev_used[ph] = 0;
+  return DEX_OK;
+}
+
+int32_t dex_debug_phase_us(dex_ctx* c, float* out8) {
+  if (!c || !out8) return fail(c, DEX_EINVAL, "null argument");
+  if (!c->cfg.debug_taps) return fail(c, DEX_ESTATE, "debug_taps is off");
+  memcpy(out8, c->phase_us, sizeof(float) * 8);
+  return DEX_OK;
+}
+
+}  // extern "C"

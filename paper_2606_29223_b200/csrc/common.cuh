@@ -1,0 +1,190 @@
+// common.cuh — device-side state layout shared by the DEX kernels (HBM layout: DESIGN.md "Data layout").
+#pragma once
+#include <cstdint>
+#include <cuda.h>
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+
+#include "../../include/dex.h"
+
+namespace dexk {
+
+constexpr int kMaxGrp = DEX_MAX_DEPTHS;
+constexpr int kMaxAnc = DEX_MAX_DEPTHS;
+constexpr int kChunk = 64;          // attention reduces over absolute positions in chunks of 64 (H3)
+constexpr int kTileM = 128;         // GEMM: weight rows (out features) per MMA tile
+constexpr int kTileK = 64;          // GEMM: bf16 K elements per pipeline stage (128 B rows, SW128)
+constexpr int kBoxRows = 16;        // activation rows per TMA box
+constexpr int kPrefillRows = 128;   // rows per prefill chunk
+
+// A "plan" = groups of stacked rows, each streaming its own layer segment.  Decode: group m =
+// explorer E_m with stage Pi_m = Layers(d_{m-1}, d_m].  Prefill: one group
+// over all L layers.  Exit: groups are <=256-row chunks of all rows, "layer" 0 of the LM head.
+struct Plan {
+  int n_grp;
+  int row_base[kMaxGrp];   // first row of the group (multiple of 16)
+  int rows_cap[kMaxGrp];   // row capacity (multiple of 16, <= 256)
+  int layer_lo[kMaxGrp];   // d_{m-1}
+  int layer_len[kMaxGrp];  // |Pi_m|
+};
+
+// One lattice row of the current round (an exploration token).
+struct RowInfo {
+  int valid;               // 0: dead row
+  int seq;
+  int node;                // heap id in the binary expansion tree (reading R2); prefill: -1
+  int pos;                 // absolute token position (RoPE, causal limit)
+  int grp;                 // plan group (= stage m for decode rows)
+  int slot;                // compact slot id whose K/V this row writes; -1: write committed pages
+  int n_paged;             // positions [0, n_paged) are read from committed pages
+  int n_anc;               // positions n_paged + i, i < n_anc, are read from slot anc[i]; then own slot
+  int anc[kMaxAnc];
+  int parent_row;          // >= 0: h_in = frontier hidden of that row; -1: h_in = Embed[tok_in]
+  int tok_in;
+  int is_ref;              // final-depth anchor node 2^{N-1}-1: never masked (Alg. 2 lines 1-4)
+  int n_mask;              // DECS: tokens proposed by shallower nodes of the same slot chain
+  int mask_tok[kMaxAnc];
+  int pad[4];
+};
+static_assert(sizeof(RowInfo) == 32 * 4, "RowInfo is 128 bytes");
+
+// Per-sequence FSM and committed-prefix bookkeeping.
+struct SeqState {
+  int active;
+  int q;                   // rounds completed since the last commit
+  int ctx_len;             // committed K/V positions (= n_tok - 1)
+  int n_tok;               // committed tokens incl. prompt
+  int last_tok;            // x[n-1]: the next root-slot input
+  int pending;             // anchor at final depth, commit not yet applied
+  int done;
+  int pad;
+};
+
+// What the apply/collapse kernels do for a sequence after a round.
+struct CollapseCmd {
+  int op;                  // 0 none, 1 advance (q+1), 2 commit+collapse, 3 hold (pending)
+  int k_sel;
+  int token;
+  int q_old;
+};
+
+// All device pointers + shape; passed by value to kernels.
+struct Dev {
+  // shape
+  int L, d, nh, nkv, hd, ffn, vocab, qkv_out;
+  float eps;
+  int N;                   // |X|
+  int depths[kMaxGrp];     // X
+  int max_seqs, max_ctx, page_size, pages_per_seq, n_slots;  // n_slots = 2^{N-1} compact slots / seq
+  int n_nodes;             // 2^N - 1
+  int R_cap;               // rows of every row-indexed buffer
+  int R_dec;               // rows used by the decode plan
+  int decs, planes, taps;
+  int max_len;             // max_m |Pi_m|
+  // weights
+  const __nv_bfloat16 *embed, *lm_head;
+  const float *norm_attn, *norm_ffn, *norm_final;
+  // state
+  SeqState* seqs;          // [max_seqs]
+  int* tokens;             // [max_seqs][max_ctx + 1]
+  int* B;                  // [max_seqs][n_nodes] explore buffer
+  int* page_table;         // [max_seqs][pages_per_seq]
+  __nv_bfloat16 *kpool, *vpool;   // [L][n_pages][page_size][nkv][hd]
+  __nv_bfloat16 *kslot, *vslot;   // [max_seqs][n_slots][L][nkv][hd]
+  float* x_cur;            // [R_cap][d] residual stream of this round's rows
+  float* x_front;          // [R_cap][d] frontier hidden (h_out of the previous level)
+  RowInfo* rows;           // [R_cap]
+  int* grp_nb;             // [kMaxGrp] live row extent per decode/prefill group (multiple of 16)
+  int* exit_nb;            // [kMaxGrp] live row extent per exit chunk
+  __nv_bfloat16 *act_a, *act_o, *act_f, *act_e;   // [planes][R_cap][K] MMA operands
+  float* part;             // [S][R_cap][part_ld] split-K partial sums
+  int part_ld;
+  float* qbuf;             // [R_cap][nh*hd]
+  float* attn_part;        // [R_cap][nh][max_chunks][hd + 2]
+  int max_chunks;
+  float2* rope;            // [max_ctx + kMaxAnc + 1][hd/2] (cos, sin)
+  unsigned long long* best_key;   // [R_cap]
+  float2* ref_tile;        // [max_seqs][ref_tiles] per (tile, lane-quarter) top-2 of the anchor row
+  int ref_tiles;
+  CollapseCmd* cmd;        // [max_seqs]
+  dex_step_result* result_dev;    // [max_seqs] (mapped pinned host memory)
+  float* tap_hidden;       // [R_cap][max_len][d] (taps only)
+  int n_pages;
+};
+
+__host__ __device__ inline size_t kv_page_elems(const Dev& D) { return (size_t)D.page_size * D.nkv * D.hd; }
+__host__ __device__ inline size_t kv_layer_elems(const Dev& D) { return (size_t)D.n_pages * kv_page_elems(D); }
+
+// Address of K (or V) of committed position p of sequence s at layer l: [nkv][hd].
+__device__ __forceinline__ size_t page_off(const Dev& D, int s, int l, int p) {
+  int pg = D.page_table[s * D.pages_per_seq + p / D.page_size];
+  return (size_t)l * kv_layer_elems(D) + (size_t)pg * kv_page_elems(D) + (size_t)(p % D.page_size) * D.nkv * D.hd;
+}
+__device__ __forceinline__ size_t slot_off(const Dev& D, int s, int slot, int l) {
+  return (((size_t)s * D.n_slots + slot) * D.L + l) * D.nkv * D.hd;
+}
+
+// Order-preserving float -> uint32 (larger float <=> larger key).
+__device__ __forceinline__ uint32_t f2key(float f) {
+  uint32_t u = __float_as_uint(f);
+  return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
+}
+__device__ __forceinline__ float key2f(uint32_t k) {
+  uint32_t u = (k & 0x80000000u) ? (k & 0x7FFFFFFFu) : ~k;
+  return __uint_as_float(u);
+}
+
+// fp32 -> bf16 hi (+ lo residual) planes.
+__device__ __forceinline__ void split_store(__nv_bfloat16* base, size_t plane_stride, size_t idx, float v, int planes) {
+  __nv_bfloat16 hi = __float2bfloat16_rn(v);
+  base[idx] = hi;
+  if (planes > 1) base[plane_stride + idx] = __float2bfloat16_rn(v - __bfloat162float(hi));
+}
+
+// ---------------------------------------------------------------------------------------
+// Tree arithmetic (heap reading R2: depth child 2i+1, position child 2i+2).  A node of
+// level q is (q, o) with o in [0, 2^q): the bits of o, MSB first, are the moves from the
+// root (0 = depth move, 1 = position move).
+__host__ __device__ inline int node_id(int level, int o) { return (1 << level) - 1 + o; }
+__host__ __device__ inline int node_level(int node) {
+  int l = 0;
+  while ((2 << l) - 1 <= node) ++l;
+  return l;
+}
+__host__ __device__ inline int stage_of(int level, int o) {  // trailing depth moves
+  if (o == 0) return level;
+  int m = 0;
+  while (((o >> m) & 1) == 0) ++m;
+  return m;
+}
+__host__ __device__ inline int cap_of(int N, int m) {  // max rows of stage m per sequence
+  int e = N - 2 - m;
+  return e > 0 ? (1 << e) : 1;
+}
+// index of (level q, offset o) among the level's rows of its stage, ascending o
+__host__ __device__ inline int idx_in_stage(int level, int o, int m) { return (m == level) ? 0 : (o >> (m + 1)); }
+__host__ __device__ inline int compact_slot(int root_node) { return (root_node + 1) >> 1; }
+
+struct GemmArgs {
+  Plan plan;
+  int step;                // layer-step j (layer = layer_lo[g] + j); groups with j >= layer_len are idle
+  int out_dim, k_dim;
+  int n_tiles;             // ceil(out / 128)
+  int ksplit, kb_per_split, kb_total;
+  int planes;
+  int mode;                // 0: store split-K partials, 1: fused argmax (exit head)
+  int x_cap;               // activation rows per ring stage (multiple of 16)
+  int n_stages;            // ring depth
+  int acc_cols;            // TMEM columns per accumulator stage (power of two >= 32)
+  const int* grp_nb;
+  const RowInfo* rows;
+  float* part;
+  int part_ld;
+  size_t part_split_stride;
+  unsigned long long* best_key;
+  float2* ref_tile;
+  int ref_tiles;
+  int vocab;
+};
+
+}  // namespace dexk
