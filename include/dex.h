@@ -158,9 +158,18 @@ int32_t dex_debug_read(dex_ctx* ctx, int32_t what, int32_t seq, int32_t a, void*
 int32_t dex_debug_gemm(dex_ctx* ctx, int32_t which, int32_t layer, const float* x, int32_t rows, float* y);
 
 /* Per-kernel-class device time of the last dex_step in microseconds (CUDA events around each
- * phase; only when cfg.debug_taps = 1, which disables graph replay): float[8] =
- * {bookkeeping, gemm, glue(norm/rope/silu), attention, exit, commit+collapse, 0, total}. */
+ * launch on the context's stream; only while profiling is on, which bypasses graph replay):
+ * host float[8] = {bookkeeping, segment GEMMs, glue (norm/rope/silu), attention, exit GEMM,
+ * commit+collapse, 0, total}. */
 int32_t dex_debug_phase_us(dex_ctx* ctx, float* out8);
+
+/* Measurement hook used by bench.py.  Copies out (host double[8] each, may be NULL) the
+ * per-class device microseconds accumulated over the dex_step calls since the last reset
+ * (same classes as dex_debug_phase_us; zeros unless profiling was on) and the counters
+ * {rounds, kernel launches, segment-GEMM launches, segment-GEMM algorithmic weight bytes,
+ *  exit-GEMM LM-head bytes, committed-KV bytes attended, 0, 0}; then, if on >= 0, resets both
+ * and switches profiling on (1) or off (0).  on < 0: read only. */
+int32_t dex_profile(dex_ctx* ctx, int32_t on, double* phase_us_acc8, double* counters8);
 
 int32_t dex_destroy(dex_ctx* ctx);
 const char* dex_last_error(const dex_ctx* ctx);   /* ctx may be NULL: last global error */

@@ -51,6 +51,7 @@ _SIGNATURES = {
     "dex_debug_read": (C.c_int32, [C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_void_p, C.c_size_t]),
     "dex_debug_gemm": (C.c_int32, [C.c_void_p, C.c_int32, C.c_int32, C.POINTER(C.c_float), C.c_int32, C.POINTER(C.c_float)]),
     "dex_debug_phase_us": (C.c_int32, [C.c_void_p, C.POINTER(C.c_float)]),
+    "dex_profile": (C.c_int32, [C.c_void_p, C.c_int32, C.POINTER(C.c_double), C.POINTER(C.c_double)]),
     "dex_destroy": (C.c_int32, [C.c_void_p]),
     "dex_last_error": (C.c_char_p, [C.c_void_p]),
 }
@@ -141,6 +142,12 @@ def dex_debug_phase_us(ctx):
     return out
 
 
+def dex_profile(ctx, on):
+    ph, ct = np.zeros(8, dtype=np.float64), np.zeros(8, dtype=np.float64)
+    _check(lib().dex_profile(ctx, on, ph.ctypes.data_as(C.POINTER(C.c_double)), ct.ctypes.data_as(C.POINTER(C.c_double))), ctx)
+    return ph, ct
+
+
 def dex_destroy(ctx):
     _check(lib().dex_destroy(ctx))
 
@@ -223,6 +230,9 @@ class Dex:
     def gemm(self, which, layer, x):
         outs = (self.shape.qkv_out, self.shape.d_model, 2 * self.shape.d_ffn, self.shape.d_model)
         return dex_debug_gemm(self.ctx, which, layer, x, outs[which])
+
+    def profile(self, on):
+        return dex_profile(self.ctx, on)
 
     def phase_us(self):
         return dex_debug_phase_us(self.ctx)

@@ -23,7 +23,7 @@ cudaError_t launch_gather_norm(const Dev&, const Plan&, int, cudaStream_t);
 cudaError_t launch_add_norm(const Dev&, const Plan&, int, int, int, int, size_t, cudaStream_t);
 cudaError_t launch_rope_kv(const Dev&, const Plan&, int, int, int, size_t, cudaStream_t);
 cudaError_t launch_silu_mul(const Dev&, const Plan&, int, int, int, size_t, cudaStream_t);
-cudaError_t launch_attn(const Dev&, const Plan&, int, int, int, cudaStream_t);
+cudaError_t launch_attn(const Dev&, const Plan&, int, int, int, int, cudaStream_t);
 cudaError_t launch_decide(const Dev&, const Plan&, int, cudaStream_t);
 cudaError_t launch_set_cmd(const Dev&, int, int, int, cudaStream_t);
 cudaError_t launch_collapse(const Dev&, const Plan&, int, cudaStream_t);
@@ -79,6 +79,9 @@ struct dex_ctx {
   std::vector<std::pair<cudaEvent_t, cudaEvent_t>> ev[PH_N];
   size_t ev_used[PH_N];
   float phase_us[8];
+  double phase_us_acc[8];
+  int profiling;
+  double counters[8];                 // rounds, kernel launches, gemm launches, gemm weight bytes, exit bytes, kv bytes
 };
 
 namespace {
@@ -118,6 +121,7 @@ int validate(const dex_config* cfg, const int32_t* depths, int32_t n) {
   if (cfg->max_ctx < 2) return fail(nullptr, DEX_EINVAL, "max_ctx too small");
   if (cfg->act_planes != 1 && cfg->act_planes != 2) return fail(nullptr, DEX_EINVAL, "act_planes must be 1 or 2");
   if (cfg->vocab < 2) return fail(nullptr, DEX_EINVAL, "vocab too small");
+  if (cfg->d_model > 8192) return fail(nullptr, DEX_ECAPACITY, "d_model > 8192 not supported");
   if (cfg->max_seqs * cap_of(n, 0) > 256) return fail(nullptr, DEX_ECAPACITY, "max_seqs * 2^(N-2) rows exceed 256 per stage");
   return DEX_OK;
 }
@@ -263,7 +267,7 @@ int encode_3d(dex_ctx* c, EncodeFn fn, CUtensorMap* tm, const void* base, uint64
 
 // ---- phase timing (taps only) ----
 void ph_begin(dex_ctx* c, Phase p) {
-  if (!c->cfg.debug_taps) return;
+  if (!c->profiling) return;
   if (c->ev_used[p] == c->ev[p].size()) {
     cudaEvent_t a, b;
     cudaEventCreate(&a);
@@ -273,7 +277,7 @@ void ph_begin(dex_ctx* c, Phase p) {
   cudaEventRecord(c->ev[p][c->ev_used[p]].first, c->stream);
 }
 void ph_end(dex_ctx* c, Phase p) {
-  if (!c->cfg.debug_taps) return;
+  if (!c->profiling) return;
   cudaEventRecord(c->ev[p][c->ev_used[p]].second, c->stream);
   c->ev_used[p]++;
 }
@@ -298,6 +302,7 @@ int run_gemm(dex_ctx* c, int which, const CUtensorMap& tmX, const Plan& plan, co
   a.acc_cols = ring.acc_cols;
   a.grp_nb = grp_nb;
   a.rows = c->D.rows;
+  a.n_rows = c->D.R_cap;
   a.part = c->D.part;
   a.part_ld = c->D.part_ld;
   a.part_split_stride = c->part_split_stride;
@@ -326,7 +331,7 @@ int enqueue_layers(dex_ctx* c, const Plan& plan, const RingCfg& ring, int rows, 
     CU(c, launch_rope_kv(D, plan, rows, j, c->op[0].ksplit, ss, c->stream));
     ph_end(c, PH_GLUE);
     ph_begin(c, PH_ATTN);
-    CU(c, launch_attn(D, plan, rows, j, n_chunks, c->stream));
+    CU(c, launch_attn(D, plan, rows, j, n_chunks, &plan == &c->dec_plan ? 1 : 0, c->stream));
     ph_end(c, PH_ATTN);
     ph_begin(c, PH_GEMM);
     rc = run_gemm(c, 1, c->tmX[1], plan, ring, j, 0, D.grp_nb);
@@ -397,8 +402,42 @@ int ensure_pages(dex_ctx* c, int s, int n_positions) {
   return DEX_OK;
 }
 
+// Algorithmic bytes and launch counts of one round, from the host mirror of the FSM
+// (DESIGN.md "Roofline accounting"): a live stage streams its layer's weights once per layer-step.
+void account_round(dex_ctx* c) {
+  const Dev& D = c->D;
+  bool live[kMaxGrp] = {false};
+  double kv = 0;
+  for (int s = 0; s < c->cfg.max_seqs; ++s) {
+    const HostSeq& hs = c->seqs[s];
+    if (!hs.active || hs.done) continue;
+    for (int m = 0; m <= hs.q && m < D.N; ++m) {
+      live[m] = true;
+      kv += (double)c->dec_plan.layer_len[m] * hs.ctx_len * 2.0 * D.nkv * D.hd * 2.0;   // committed K+V read once per stage layer
+    }
+  }
+  double wbytes = 0;
+  int gemm_launches = 0;
+  for (int j = 0; j < D.max_len; ++j) {
+    bool any = false;
+    for (int m = 0; m < D.N; ++m)
+      if (live[m] && j < c->dec_plan.layer_len[m]) {
+        any = true;
+        for (int i = 0; i < 4; ++i) wbytes += 2.0 * c->op[i].out * c->op[i].k;
+      }
+    (void)any;
+    gemm_launches += 4;
+  }
+  c->counters[0] += 1;
+  c->counters[1] += 2 + 10.0 * D.max_len + 1 + 1 + 3;
+  c->counters[2] += gemm_launches;
+  c->counters[3] += wbytes;
+  c->counters[4] += 2.0 * c->op[4].out * c->op[4].k * c->exit_plan.n_grp;
+  c->counters[5] += kv;
+}
+
 void collect_phase_times(dex_ctx* c) {
-  if (!c->cfg.debug_taps) return;
+  if (!c->profiling) return;
   float total = 0.f;
   for (int p = 0; p < PH_N; ++p) {
     float us = 0.f;
@@ -409,6 +448,7 @@ void collect_phase_times(dex_ctx* c) {
     }
     // bookkeeping, gemm, glue, attention, exit, commit+collapse
     c->phase_us[p] = us;
+    c->phase_us_acc[p] += us;
     total += us;
     c->ev_used[p] = 0;
   }
@@ -460,6 +500,9 @@ int32_t dex_init(dex_ctx** out, const dex_config* cfg, const dex_weights* w, con
   c->result_host = nullptr;
   memset(c->ev_used, 0, sizeof c->ev_used);
   memset(c->phase_us, 0, sizeof c->phase_us);
+  memset(c->phase_us_acc, 0, sizeof c->phase_us_acc);
+  memset(c->counters, 0, sizeof c->counters);
+  c->profiling = cfg->debug_taps ? 1 : 0;
   int dev = 0;
   cudaGetDevice(&dev);
   cudaDeviceGetAttribute(&c->n_sms, cudaDevAttrMultiProcessorCount, dev);
@@ -609,7 +652,8 @@ int32_t dex_step(dex_ctx* c, uint32_t flags, dex_step_result* out) {
   }
   if (n_live > 0) {
     const int n_chunks = max_pos / kChunk + 1;
-    if (c->cfg.use_graph && !c->cfg.debug_taps) {
+    account_round(c);
+    if (c->cfg.use_graph && !c->profiling) {
       const long long key = ((long long)n_chunks << 8) | (flags & 0xff);
       auto it = c->graphs.find(key);
       if (it == c->graphs.end()) {
@@ -763,8 +807,20 @@ int32_t dex_debug_gemm(dex_ctx* c, int32_t which, int32_t layer, const float* x,
 
 int32_t dex_debug_phase_us(dex_ctx* c, float* out8) {
   if (!c || !out8) return fail(c, DEX_EINVAL, "null argument");
-  if (!c->cfg.debug_taps) return fail(c, DEX_ESTATE, "debug_taps is off");
+  if (!c->profiling) return fail(c, DEX_ESTATE, "profiling is off");
   memcpy(out8, c->phase_us, sizeof(float) * 8);
+  return DEX_OK;
+}
+
+int32_t dex_profile(dex_ctx* c, int32_t on, double* phase_us_acc8, double* counters8) {
+  if (!c) return fail(c, DEX_EINVAL, "null ctx");
+  if (phase_us_acc8) memcpy(phase_us_acc8, c->phase_us_acc, sizeof(double) * 8);
+  if (counters8) memcpy(counters8, c->counters, sizeof(double) * 8);
+  if (on >= 0) {
+    c->profiling = (on || c->cfg.debug_taps) ? 1 : 0;
+    memset(c->phase_us_acc, 0, sizeof c->phase_us_acc);
+    memset(c->counters, 0, sizeof c->counters);
+  }
   return DEX_OK;
 }
 

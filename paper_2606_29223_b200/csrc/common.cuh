@@ -178,6 +178,7 @@ struct GemmArgs {
   int acc_cols;            // TMEM columns per accumulator stage (power of two >= 32)
   const int* grp_nb;
   const RowInfo* rows;
+  int n_rows;              // R_cap
   float* part;
   int part_ld;
   size_t part_split_stride;

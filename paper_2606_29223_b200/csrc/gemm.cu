@@ -71,9 +71,15 @@ k_gemm(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CUtensor
 
   const int warp = threadIdx.x >> 5;
   const int lane = threadIdx.x & 31;
+  asm volatile("griddepcontrol.launch_dependents;\n" ::: "memory");
 
   __shared__ int live_g[kMaxGrp], live_nb[kMaxGrp];
   __shared__ int n_live_s;
+  __shared__ uint32_t s_valid[32];                 // live-row bitmap (R_cap <= 1024)
+  if (threadIdx.x < 32) s_valid[threadIdx.x] = 0;
+  __syncthreads();
+  for (int r = threadIdx.x; r < a.n_rows; r += kGemmThreads)
+    if (a.rows[r].valid) atomicOr(&s_valid[r >> 5], 1u << (r & 31));
   if (threadIdx.x == 0) {
     n_live_s = build_live(a, live_g, live_nb);
     for (int i = 0; i < a.n_stages; ++i) {
@@ -101,18 +107,32 @@ k_gemm(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CUtensor
   if (warp == 0) {
     // ===================== TMA producer =====================
     if (lane == 0) {
-      int stage = 0;
+      // Weights do not depend on the preceding kernel: the first ring-full of weight tiles is
+      // requested BEFORE waiting on the programmatic dependency, the activation boxes after it.
+      int pre = 0;
+      for (int item = blockIdx.x; item < n_items && pre < a.n_stages; item += gridDim.x) {
+        Item it = decode_item(a, item, live_g, live_nb);
+        const uint32_t tx = kABytes + a.planes * it.nb * 128;
+        for (int kb = it.kb0; kb < it.kb1 && pre < a.n_stages; ++kb, ++pre) {
+          mbar_expect_tx(&full[pre], tx);
+          tma_load_3d(smem + (size_t)pre * stage_bytes, &tmW, &full[pre], kb * kTileK, it.tile * kTileM, it.layer, kEvictFirst);
+        }
+      }
+      asm volatile("griddepcontrol.wait;\n" ::: "memory");
+      int stage = 0, issued = 0;
       uint32_t phase = 0;
       for (int item = blockIdx.x; item < n_items; item += gridDim.x) {
         Item it = decode_item(a, item, live_g, live_nb);
         const int row0 = a.plan.row_base[it.g];
         const uint32_t tx = kABytes + a.planes * it.nb * 128;
-        for (int kb = it.kb0; kb < it.kb1; ++kb) {
-          mbar_wait(&empty[stage], phase ^ 1);
+        for (int kb = it.kb0; kb < it.kb1; ++kb, ++issued) {
           uint8_t* sA = smem + (size_t)stage * stage_bytes;
           uint8_t* sB = sA + kABytes;
-          mbar_expect_tx(&full[stage], tx);
-          tma_load_3d(sA, &tmW, &full[stage], kb * kTileK, it.tile * kTileM, it.layer, kEvictFirst);
+          if (issued >= pre) {
+            mbar_wait(&empty[stage], phase ^ 1);
+            mbar_expect_tx(&full[stage], tx);
+            tma_load_3d(sA, &tmW, &full[stage], kb * kTileK, it.tile * kTileM, it.layer, kEvictFirst);
+          }
           for (int p = 0; p < a.planes; ++p)
             for (int r = 0; r < it.nb; r += kBoxRows)
               tma_load_3d(sB + p * plane_bytes + r * 128, &tmX, &full[stage], kb * kTileK, row0 + r, p, kEvictLast);
@@ -183,13 +203,15 @@ k_gemm(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CUtensor
           float* dst = a.part + (size_t)it.split * a.part_split_stride + (size_t)(row0 + c0) * a.part_ld + col;
 #pragma unroll
           for (int i = 0; i < 16; ++i) {
-            if (a.rows[row0 + c0 + i].valid && col < a.out_dim) dst[(size_t)i * a.part_ld] = __uint_as_float(v[i]);
+            const int rr = row0 + c0 + i;
+            if (((s_valid[rr >> 5] >> (rr & 31)) & 1u) && col < a.out_dim) dst[(size_t)i * a.part_ld] = __uint_as_float(v[i]);
           }
         } else {
 #pragma unroll
           for (int i = 0; i < 16; ++i) {
-            const RowInfo* ri = &a.rows[row0 + c0 + i];
-            if (!ri->valid) continue;                       // warp-uniform
+            const int rr = row0 + c0 + i;
+            if (!((s_valid[rr >> 5] >> (rr & 31)) & 1u)) continue;   // warp-uniform
+            const RowInfo* ri = &a.rows[rr];
             float val = __uint_as_float(v[i]);
             bool dead = col >= a.vocab;
             const int nm = ri->n_mask;                      // Alg. 2 lines 5-7: mask prior proposals
@@ -230,8 +252,17 @@ cudaError_t gemm_init() {
 // Host-side launcher (called from api.cu).
 cudaError_t launch_gemm(const CUtensorMap& tmW, const CUtensorMap& tmX, const GemmArgs& a, int grid, size_t smem_bytes,
                         cudaStream_t stream) {
-  k_gemm<<<grid, kGemmThreads, smem_bytes, stream>>>(tmW, tmX, a);
-  return cudaGetLastError();
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(grid);
+  cfg.blockDim = dim3(kGemmThreads);
+  cfg.dynamicSmemBytes = smem_bytes;
+  cfg.stream = stream;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at;
+  cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, k_gemm, tmW, tmX, a);
 }
 
 }  // namespace dexk

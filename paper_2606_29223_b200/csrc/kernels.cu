@@ -33,6 +33,43 @@ __device__ __forceinline__ float block_sum(float v, float* red /*[33]*/) {
   __syncthreads();
   return red[32];
 }
+// Programmatic dependent launch: every kernel between the first segment GEMM and the exit GEMM
+// is launched with programmatic stream serialization; it lets its dependents start early
+// (pdl_trigger) and waits for its own predecessor before touching anything that predecessor
+// wrote (pdl_wait).  Row tables / grp_nb are written before k_gather_norm, which is a normal
+// launch, so they are complete for every later kernel of the round.
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;\n" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;\n" ::: "memory"); }
+
+__device__ __forceinline__ float4 ld4(const float* p) { return *reinterpret_cast<const float4*>(p); }
+__device__ __forceinline__ float4 add4(float4 a, float4 b) { return make_float4(a.x + b.x, a.y + b.y, a.z + b.z, a.w + b.w); }
+// sum of up to 8 split-K partials, loads issued together, added in split order (fixed order: H3)
+__device__ __forceinline__ float4 sum_splits4(const float* p, int ksplit, size_t split_stride) {
+  float4 v[8];
+#pragma unroll
+  for (int s = 0; s < 8; ++s)
+    if (s < ksplit) v[s] = ld4(p + (size_t)s * split_stride);
+  float4 acc = v[0];
+#pragma unroll
+  for (int s = 1; s < 8; ++s)
+    if (s < ksplit) acc = add4(acc, v[s]);
+  return acc;
+}
+__device__ __forceinline__ void split_store4(__nv_bfloat16* base, size_t plane_stride, size_t idx, float4 v, int planes) {
+  __nv_bfloat162 h0 = __floats2bfloat162_rn(v.x, v.y), h1 = __floats2bfloat162_rn(v.z, v.w);
+  uint2 pk;
+  pk.x = *reinterpret_cast<uint32_t*>(&h0);
+  pk.y = *reinterpret_cast<uint32_t*>(&h1);
+  *reinterpret_cast<uint2*>(base + idx) = pk;
+  if (planes > 1) {
+    const float2 f0 = __bfloat1622float2(h0), f1 = __bfloat1622float2(h1);
+    __nv_bfloat162 l0 = __floats2bfloat162_rn(v.x - f0.x, v.y - f0.y), l1 = __floats2bfloat162_rn(v.z - f1.x, v.w - f1.y);
+    pk.x = *reinterpret_cast<uint32_t*>(&l0);
+    pk.y = *reinterpret_cast<uint32_t*>(&l1);
+    *reinterpret_cast<uint2*>(base + plane_stride + idx) = pk;
+  }
+}
+
 __device__ __forceinline__ bool seq_live(const SeqState& s) { return s.active && !s.done && !s.pending; }
 __device__ __forceinline__ int round16(int v) { return (v + 15) & ~15; }
 
@@ -184,56 +221,77 @@ __global__ void k_rope_table(Dev D, double theta, int n_pos) {
 // ------------------------------------------------------------------------------------------
 // a1 + first RMSNorm: h_in = parent's frontier hidden (depth expansion) or Embed[tok]
 // (position expansion), then a = RMSNorm(h_in; w_attn[first layer of the stage]).
-__global__ void __launch_bounds__(256) k_gather_norm(Dev D, Plan plan) {
+__global__ void __launch_bounds__(1024) k_gather_norm(Dev D, Plan plan) {
   __shared__ float red[33];
   const int r = blockIdx.x;
   const RowInfo ri = D.rows[r];
   if (!ri.valid) return;
   float* x = D.x_cur + (size_t)r * D.d;
+  const int nv = D.d >> 2;
+  float4 xv[2];
   float ss = 0.f;
-  if (ri.parent_row >= 0) {
-    const float* src = D.x_front + (size_t)ri.parent_row * D.d;
-    for (int i = threadIdx.x; i < D.d; i += blockDim.x) {
-      float v = src[i];
-      x[i] = v;
-      ss += v * v;
-    }
-  } else {
-    const __nv_bfloat16* src = D.embed + (size_t)ri.tok_in * D.d;
-    for (int i = threadIdx.x; i < D.d; i += blockDim.x) {
-      float v = __bfloat162float(src[i]);
-      x[i] = v;
-      ss += v * v;
+#pragma unroll
+  for (int it = 0; it < 2; ++it) {
+    const int i = threadIdx.x + it * blockDim.x;
+    if (i < nv) {
+      float4 v;
+      if (ri.parent_row >= 0) {
+        v = ld4(D.x_front + (size_t)ri.parent_row * D.d + 4 * i);
+      } else {
+        const uint2 pk = *reinterpret_cast<const uint2*>(D.embed + (size_t)ri.tok_in * D.d + 4 * i);
+        const float2 a = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(&pk.x));
+        const float2 b = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(&pk.y));
+        v = make_float4(a.x, a.y, b.x, b.y);
+      }
+      xv[it] = v;
+      *reinterpret_cast<float4*>(x + 4 * i) = v;
+      ss += v.x * v.x + v.y * v.y + v.z * v.z + v.w * v.w;
     }
   }
   ss = block_sum(ss, red);
   const float inv = 1.0f / sqrtf(ss / (float)D.d + D.eps);
   const float* w = D.norm_attn + (size_t)plan.layer_lo[ri.grp] * D.d;
   const size_t ps = (size_t)D.R_cap * D.d;
-  for (int i = threadIdx.x; i < D.d; i += blockDim.x)
-    split_store(D.act_a, ps, (size_t)r * D.d + i, x[i] * inv * w[i], D.planes);
+#pragma unroll
+  for (int it = 0; it < 2; ++it) {
+    const int i = threadIdx.x + it * blockDim.x;
+    if (i < nv) {
+      const float4 wv = ld4(w + 4 * i), v = xv[it];
+      split_store4(D.act_a, ps, (size_t)r * D.d + 4 * i,
+                   make_float4(v.x * inv * wv.x, v.y * inv * wv.y, v.z * inv * wv.z, v.w * inv * wv.w), D.planes);
+    }
+  }
 }
 
 // x += sum_s part[s]; then RMSNorm into the next GEMM's operand planes.
 //   mode 0 (after o_proj):    w = norm_ffn[l]                      -> act_a
 //   mode 1 (after down_proj): w = norm_attn[l+1] if the stage continues -> act_a,
 //                             else the shared final norm (exit) -> act_e
-__global__ void __launch_bounds__(256) k_add_norm(Dev D, Plan plan, int step, int mode, int ksplit, size_t split_stride) {
+// One CTA per row, one float4 per thread and pass (d <= 8192), all split loads in flight at once.
+__global__ void __launch_bounds__(1024) k_add_norm(Dev D, Plan plan, int step, int mode, int ksplit, size_t split_stride) {
   __shared__ float red[33];
+  pdl_trigger();
   const int r = blockIdx.x;
   const RowInfo ri = D.rows[r];
   if (!ri.valid || step >= plan.layer_len[ri.grp]) return;
   const int layer = plan.layer_lo[ri.grp] + step;
   float* x = D.x_cur + (size_t)r * D.d;
   const float* p = D.part + (size_t)r * D.part_ld;
+  const int nv = D.d >> 2;
+  pdl_wait();
+  float4 xv[2];
   float ss = 0.f;
-  for (int i = threadIdx.x; i < D.d; i += blockDim.x) {
-    float acc = p[i];
-    for (int s = 1; s < ksplit; ++s) acc += p[(size_t)s * split_stride + i];
-    float v = x[i] + acc;
-    x[i] = v;
-    ss += v * v;
-    if (mode == 1 && D.taps) D.tap_hidden[((size_t)r * D.max_len + step) * D.d + i] = v;
+#pragma unroll
+  for (int it = 0; it < 2; ++it) {
+    const int i = threadIdx.x + it * blockDim.x;
+    if (i < nv) {
+      float4 a = sum_splits4(p + 4 * i, ksplit, split_stride);
+      float4 v = add4(ld4(x + 4 * i), a);
+      xv[it] = v;
+      *reinterpret_cast<float4*>(x + 4 * i) = v;
+      ss += v.x * v.x + v.y * v.y + v.z * v.z + v.w * v.w;
+      if (mode == 1 && D.taps) *reinterpret_cast<float4*>(D.tap_hidden + ((size_t)r * D.max_len + step) * D.d + 4 * i) = v;
+    }
   }
   ss = block_sum(ss, red);
   const float inv = 1.0f / sqrtf(ss / (float)D.d + D.eps);
@@ -248,68 +306,83 @@ __global__ void __launch_bounds__(256) k_add_norm(Dev D, Plan plan, int step, in
     dst = D.act_e;
   }
   const size_t ps = (size_t)D.R_cap * D.d;
-  for (int i = threadIdx.x; i < D.d; i += blockDim.x)
-    split_store(dst, ps, (size_t)r * D.d + i, x[i] * inv * w[i], D.planes);
+#pragma unroll
+  for (int it = 0; it < 2; ++it) {
+    const int i = threadIdx.x + it * blockDim.x;
+    if (i < nv) {
+      const float4 wv = ld4(w + 4 * i), v = xv[it];
+      split_store4(dst, ps, (size_t)r * D.d + 4 * i,
+                   make_float4(v.x * inv * wv.x, v.y * inv * wv.y, v.z * inv * wv.z, v.w * inv * wv.w), D.planes);
+    }
+  }
 }
 
 // q,k,v = sum of split-K partials; RoPE (rotate-half, R13) on q,k; q -> fp32 buffer; k,v -> bf16
 // into the row's slot K/V (branch-private) or, for prefill rows, straight into committed pages.
+// grid (rows, blocks): a thread owns 4 consecutive dims of one head (and their rotate-half partners).
 __global__ void __launch_bounds__(256) k_rope_kv(Dev D, Plan plan, int step, int ksplit, size_t split_stride) {
+  pdl_trigger();
   const int r = blockIdx.x;
   const RowInfo ri = D.rows[r];
   if (!ri.valid || step >= plan.layer_len[ri.grp]) return;
   const int layer = plan.layer_lo[ri.grp] + step;
-  const int hd = D.hd, half = hd / 2;
+  const int hd = D.hd, half = hd / 2, qd = half / 4;     // qd: float4 groups per half head
   const float* p = D.part + (size_t)r * D.part_ld;
   const float2* rt = D.rope + (size_t)ri.pos * half;
   const size_t kvo = (ri.slot >= 0) ? slot_off(D, ri.seq, ri.slot, layer) : page_off(D, ri.seq, layer, ri.pos);
   __nv_bfloat16* kd = ((ri.slot >= 0) ? D.kslot : D.kpool) + kvo;
   __nv_bfloat16* vd = ((ri.slot >= 0) ? D.vslot : D.vpool) + kvo;
   const int nq = D.nh * hd, nk = D.nkv * hd;
-  const int n_pairs = (D.nh + D.nkv) * half;
-  for (int t = threadIdx.x; t < n_pairs + nk; t += blockDim.x) {
-    if (t < n_pairs) {
-      const int h = t / half, i = t % half;
+  const int n_rot = (D.nh + D.nkv) * qd;                 // rotated float4 pair groups
+  const int n_v = nk / 4;
+  pdl_wait();
+  for (int t = blockIdx.y * blockDim.x + threadIdx.x; t < n_rot + n_v; t += gridDim.y * blockDim.x) {
+    if (t < n_rot) {
+      const int h = t / qd, i = (t % qd) * 4;
       const int i1 = h * hd + i, i2 = i1 + half;
-      float a = p[i1], b = p[i2];
-      for (int s = 1; s < ksplit; ++s) {
-        a += p[(size_t)s * split_stride + i1];
-        b += p[(size_t)s * split_stride + i2];
-      }
-      const float2 cs = rt[i];
-      const float o1 = a * cs.x - b * cs.y;
-      const float o2 = b * cs.x + a * cs.y;
+      const float4 a = sum_splits4(p + i1, ksplit, split_stride);
+      const float4 b = sum_splits4(p + i2, ksplit, split_stride);
+      const float2 c0 = rt[i], c1 = rt[i + 1], c2 = rt[i + 2], c3 = rt[i + 3];
+      const float4 o1 = make_float4(a.x * c0.x - b.x * c0.y, a.y * c1.x - b.y * c1.y, a.z * c2.x - b.z * c2.y, a.w * c3.x - b.w * c3.y);
+      const float4 o2 = make_float4(b.x * c0.x + a.x * c0.y, b.y * c1.x + a.y * c1.y, b.z * c2.x + a.z * c2.y, b.w * c3.x + a.w * c3.y);
       if (h < D.nh) {
-        D.qbuf[(size_t)r * nq + i1] = o1;
-        D.qbuf[(size_t)r * nq + i2] = o2;
+        *reinterpret_cast<float4*>(D.qbuf + (size_t)r * nq + i1) = o1;
+        *reinterpret_cast<float4*>(D.qbuf + (size_t)r * nq + i2) = o2;
       } else {
-        kd[i1 - nq] = __float2bfloat16_rn(o1);
-        kd[i2 - nq] = __float2bfloat16_rn(o2);
+        __nv_bfloat162 x0 = __floats2bfloat162_rn(o1.x, o1.y), x1 = __floats2bfloat162_rn(o1.z, o1.w);
+        __nv_bfloat162 y0 = __floats2bfloat162_rn(o2.x, o2.y), y1 = __floats2bfloat162_rn(o2.z, o2.w);
+        *reinterpret_cast<__nv_bfloat162*>(kd + i1 - nq) = x0;
+        *reinterpret_cast<__nv_bfloat162*>(kd + i1 - nq + 2) = x1;
+        *reinterpret_cast<__nv_bfloat162*>(kd + i2 - nq) = y0;
+        *reinterpret_cast<__nv_bfloat162*>(kd + i2 - nq + 2) = y1;
       }
     } else {
-      const int i = t - n_pairs;
-      float a = p[nq + nk + i];
-      for (int s = 1; s < ksplit; ++s) a += p[(size_t)s * split_stride + nq + nk + i];
-      vd[i] = __float2bfloat16_rn(a);
+      const int i = (t - n_rot) * 4;
+      const float4 a = sum_splits4(p + nq + nk + i, ksplit, split_stride);
+      *reinterpret_cast<__nv_bfloat162*>(vd + i) = __floats2bfloat162_rn(a.x, a.y);
+      *reinterpret_cast<__nv_bfloat162*>(vd + i + 2) = __floats2bfloat162_rn(a.z, a.w);
     }
   }
 }
 
 // act = SiLU(gate) * up  (SwiGLU), from the split-K partials of the fused gate/up projection.
 __global__ void __launch_bounds__(256) k_silu_mul(Dev D, Plan plan, int step, int ksplit, size_t split_stride) {
+  pdl_trigger();
   const int r = blockIdx.x;
   const RowInfo ri = D.rows[r];
   if (!ri.valid || step >= plan.layer_len[ri.grp]) return;
   const float* p = D.part + (size_t)r * D.part_ld;
   const size_t ps = (size_t)D.R_cap * D.ffn;
-  for (int i = blockIdx.y * blockDim.x + threadIdx.x; i < D.ffn; i += gridDim.y * blockDim.x) {
-    float g = p[i], u = p[D.ffn + i];
-    for (int s = 1; s < ksplit; ++s) {
-      g += p[(size_t)s * split_stride + i];
-      u += p[(size_t)s * split_stride + D.ffn + i];
-    }
-    const float a = g / (1.0f + expf(-g)) * u;
-    split_store(D.act_f, ps, (size_t)r * D.ffn + i, a, D.planes);
+  pdl_wait();
+  for (int i = (blockIdx.y * blockDim.x + threadIdx.x) * 4; i < D.ffn; i += gridDim.y * blockDim.x * 4) {
+    const float4 g = sum_splits4(p + i, ksplit, split_stride);
+    const float4 u = sum_splits4(p + D.ffn + i, ksplit, split_stride);
+    float4 a;
+    a.x = g.x / (1.0f + expf(-g.x)) * u.x;
+    a.y = g.y / (1.0f + expf(-g.y)) * u.y;
+    a.z = g.z / (1.0f + expf(-g.z)) * u.z;
+    a.w = g.w / (1.0f + expf(-g.w)) * u.w;
+    split_store4(D.act_f, ps, (size_t)r * D.ffn + i, a, D.planes);
   }
 }
 
@@ -323,7 +396,7 @@ __global__ void __launch_bounds__(256) k_silu_mul(Dev D, Plan plan, int step, in
 // arithmetic is identical wherever its K/V lives, so a row gives the same bits before and after
 // its ancestors are committed.
 template <int HD>
-__global__ void __launch_bounds__(128) k_attn(Dev D, Plan plan, int step) {
+__global__ void __launch_bounds__(128) k_attn(Dev D, Plan plan, int step, int kv_static) {
   constexpr int CPR = HD / 8;                       // 16-byte chunks per K/V row
   __shared__ __align__(16) __nv_bfloat16 sK[kChunk * HD];
   __shared__ __align__(16) __nv_bfloat16 sV[kChunk * HD];
@@ -332,6 +405,7 @@ __global__ void __launch_bounds__(128) k_attn(Dev D, Plan plan, int step) {
   __shared__ int row_list[256];
   __shared__ int n_rows_s, max_pos_s, n_paged_s;
 
+  pdl_trigger();
   const int c = blockIdx.x, g = blockIdx.y;
   const int m = blockIdx.z / D.max_seqs, s = blockIdx.z % D.max_seqs;
   if (m >= plan.n_grp || step >= plan.layer_len[m]) return;
@@ -361,7 +435,9 @@ __global__ void __launch_bounds__(128) k_attn(Dev D, Plan plan, int step) {
   const int n_paged = n_paged_s;
   const int n_shared = max(0, min(kChunk, min(n_paged, max_pos_s + 1) - c0));
 
-  // stage the committed part of the chunk (one page: page_size % 64 == 0)
+  // stage the committed part of the chunk (one page: page_size % 64 == 0).  Decode: committed
+  // pages do not change during the round, so they are fetched before the dependency wait.
+  if (!kv_static) pdl_wait();
   if (n_shared > 0) {
     const size_t base = page_off(D, s, layer, c0) + (size_t)g * HD;
     const int stride = D.nkv * HD;
@@ -374,6 +450,7 @@ __global__ void __launch_bounds__(128) k_attn(Dev D, Plan plan, int step) {
       *reinterpret_cast<uint4*>(&sV[pl * HD + dj]) = vv;
     }
   }
+  if (kv_static) pdl_wait();   // q and the slot K/V rows come from the predecessor
   __syncthreads();
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -466,10 +543,12 @@ __global__ void __launch_bounds__(128) k_attn(Dev D, Plan plan, int step) {
 // Merge the per-chunk partials in ascending chunk order (fixed order: H3) -> bf16 operand planes.
 template <int HD>
 __global__ void __launch_bounds__(HD) k_attn_combine(Dev D, Plan plan, int step) {
+  pdl_trigger();
   const int r = blockIdx.x, h = blockIdx.y, dd = threadIdx.x;
   const RowInfo* ri = &D.rows[r];
   if (!ri->valid || step >= plan.layer_len[ri->grp]) return;
   const int nc = ri->pos / kChunk + 1;
+  pdl_wait();
   const float* src = D.attn_part + ((size_t)r * D.nh + h) * D.max_chunks * (HD + 2);
   float M = -INFINITY;
   for (int c = 0; c < nc; ++c) M = fmaxf(M, src[(size_t)c * (HD + 2) + HD]);
@@ -752,6 +831,21 @@ __global__ void k_debug_sum(const float* part, float* y, int rows, int out, int 
 // launch wrappers (called from api.cu)
 #define DEX_LAUNCH_CHECK() return cudaGetLastError()
 
+template <typename... KArgs, typename... Args>
+cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, cudaStream_t st, Args... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid;
+  cfg.blockDim = block;
+  cfg.dynamicSmemBytes = 0;
+  cfg.stream = st;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at;
+  cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
+}
+
 cudaError_t launch_rows_decode(const Dev& D, const Plan& p, cudaStream_t st) {
   k_rows_decode<<<(D.R_cap + 127) / 128, 128, 0, st>>>(D, p);
   DEX_LAUNCH_CHECK();
@@ -769,34 +863,36 @@ cudaError_t launch_rope_table(const Dev& D, double theta, int n_pos, cudaStream_
   k_rope_table<<<(n + 255) / 256, 256, 0, st>>>(D, theta, n_pos);
   DEX_LAUNCH_CHECK();
 }
+static int norm_threads(int d) {
+  int threads = ((d / 4 + 1) / 2 + 31) / 32 * 32;      // two float4 per thread cover d
+  return threads < 64 ? 64 : (threads > 1024 ? 1024 : threads);
+}
 cudaError_t launch_gather_norm(const Dev& D, const Plan& p, int rows, cudaStream_t st) {
-  k_gather_norm<<<rows, 256, 0, st>>>(D, p);
+  k_gather_norm<<<rows, norm_threads(D.d), 0, st>>>(D, p);
   DEX_LAUNCH_CHECK();
 }
 cudaError_t launch_add_norm(const Dev& D, const Plan& p, int rows, int step, int mode, int ksplit, size_t ss, cudaStream_t st) {
-  k_add_norm<<<rows, 256, 0, st>>>(D, p, step, mode, ksplit, ss);
-  DEX_LAUNCH_CHECK();
+  return launch_pdl(k_add_norm, dim3(rows), dim3(norm_threads(D.d)), st, D, p, step, mode, ksplit, ss);
 }
 cudaError_t launch_rope_kv(const Dev& D, const Plan& p, int rows, int step, int ksplit, size_t ss, cudaStream_t st) {
-  k_rope_kv<<<rows, 256, 0, st>>>(D, p, step, ksplit, ss);
-  DEX_LAUNCH_CHECK();
+  const int items = (D.nh + D.nkv) * (D.hd / 8) + D.nkv * D.hd / 4;
+  return launch_pdl(k_rope_kv, dim3(rows, (items + 255) / 256), dim3(256), st, D, p, step, ksplit, ss);
 }
 cudaError_t launch_silu_mul(const Dev& D, const Plan& p, int rows, int step, int ksplit, size_t ss, cudaStream_t st) {
-  dim3 g(rows, (D.ffn + 2047) / 2048);
-  k_silu_mul<<<g, 256, 0, st>>>(D, p, step, ksplit, ss);
-  DEX_LAUNCH_CHECK();
+  return launch_pdl(k_silu_mul, dim3(rows, (D.ffn / 4 + 255) / 256), dim3(256), st, D, p, step, ksplit, ss);
 }
-cudaError_t launch_attn(const Dev& D, const Plan& p, int rows, int step, int n_chunks, cudaStream_t st) {
+cudaError_t launch_attn(const Dev& D, const Plan& p, int rows, int step, int n_chunks, int kv_static, cudaStream_t st) {
   dim3 g(n_chunks, D.nkv, p.n_grp * D.max_seqs);
   dim3 gc(rows, D.nh);
+  cudaError_t e;
   if (D.hd == 128) {
-    k_attn<128><<<g, 128, 0, st>>>(D, p, step);
-    k_attn_combine<128><<<gc, 128, 0, st>>>(D, p, step);
-  } else {
-    k_attn<64><<<g, 128, 0, st>>>(D, p, step);
-    k_attn_combine<64><<<gc, 64, 0, st>>>(D, p, step);
+    e = launch_pdl(k_attn<128>, g, dim3(128), st, D, p, step, kv_static);
+    if (e != cudaSuccess) return e;
+    return launch_pdl(k_attn_combine<128>, gc, dim3(128), st, D, p, step);
   }
-  DEX_LAUNCH_CHECK();
+  e = launch_pdl(k_attn<64>, g, dim3(128), st, D, p, step, kv_static);
+  if (e != cudaSuccess) return e;
+  return launch_pdl(k_attn_combine<64>, gc, dim3(64), st, D, p, step);
 }
 cudaError_t launch_decide(const Dev& D, const Plan& p, int auto_collapse, cudaStream_t st) {
   k_decide<<<1, 32 * D.max_seqs, 0, st>>>(D, p, auto_collapse);
