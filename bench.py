@@ -1,0 +1,389 @@
+#!/usr/bin/env python
+"""bench.py — committed tokens/s of the DEX expand-commit-collapse step on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl dex|reference] [--workload c2]
+
+Metric (BASELINE.json:metric): committed tokens/s at the Llama-2-7B shape, bf16, batch 1,
+X = {8,16,24,32} (config c2), next to the library's own AR baseline (X = {L}, same kernels),
+with the segment GEMM's achieved HBM GB/s against the measured copy peak.
+
+A "step" is one whole run of the workload's hot path: rewind the sequence to its prefilled
+prompt (dex_rewind: the prompt's committed K/V stays resident in HBM) and run DEX rounds
+(dex_step: expand -> exit -> commit -> collapse) until `gen_len` tokens
+are committed.  `value` = committed tokens of all ranks / device time of the K steps (CUDA
+events on the library's stream, max over ranks).  `e2e` repeats the step through the C ABI with
+HOST buffers: dex_prefill from a pinned host prompt, the rounds, dex_get_tokens to the host.
+
+Multi-GPU: the path shards only across independent
+sequences -> "replicas only": every rank runs its own replica of the workload, no collective on
+the data path, scaling = weak.
+
+`--impl reference` times the CPU oracle (oracle/, NumPy fp32, as it stands) on a bounded sample
+of the same workload; rank 0 only.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+METRIC = "committed_tokens_per_s"
+UNIT = "tokens/s"
+NOMINAL_HBM_GBS = 8000.0          # the denominator BASELINE.json:metric names
+FALLBACK_HBM_GBS = 6650.0         # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
+
+
+def measured_hbm_peak():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, burst copy)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+# ------------------------------------------------------------------------------------------------
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for ln in self.proc.stdout:
+            self.lines.append(ln)
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        self.thread.join(timeout=2)
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "power_w_max": float(max(pw)),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------------------------------------
+def dist_env():
+    return int(os.environ.get("RANK", 0)), int(os.environ.get("LOCAL_RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
+
+
+def run_rounds(g, T, flags):
+    """DEX rounds until T tokens are committed.  Returns (#rounds, layer_evals, critical_layers, k histogram)."""
+    n, rounds, evals, crit = 0, 0, 0, 0
+    hist = [0] * 8
+    while n < T:
+        r = g.step(flags)[0]
+        rounds += 1
+        evals += r.layer_evals
+        crit += r.critical_layers
+        if r.committed:
+            n += 1
+            hist[r.match_k] += 1
+        if r.done or not r.active:
+            break
+    return rounds, evals, crit, hist
+
+
+def time_steps(torch, g, n_prompt, T, K, flags):
+    """K steps (rewind + T committed tokens each) between two CUDA events on the library's stream."""
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    stats = None
+    e0.record(g.stream)
+    for _ in range(K):
+        g.rewind(0, n_prompt)
+        stats = run_rounds(g, T, flags)
+    e1.record(g.stream)
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1), stats
+
+
+def bench_dex(args):
+    import torch
+    import dex_synth
+    import paper_2606_29223_b200 as P
+    from paper_2606_29223_b200 import build
+    rank, local_rank, world = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the DEX library has no CPU fallback")
+    build.build()
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    wl = dex_synth.workload(args.workload)
+    T = args.gen_len or wl.gen_len
+    n_prompt = args.prompt_len or wl.prompt_len
+    shape, X = wl.shape, wl.depths
+    N, L = len(X), shape.n_layers
+    w_host = dex_synth.make_weights(shape, wl.weight_seed, threads=16)
+    w_dev = {k: v.to(device=dev, dtype=(torch.float32 if k.startswith("norm") else torch.bfloat16)).contiguous()
+             for k, v in w_host.items()}
+    del w_host
+    # the prompt lives in PINNED host memory: dex_prefill copies it to the device inside the e2e region
+    prompt_pin = torch.empty(n_prompt, dtype=torch.int32).pin_memory()
+    prompt = prompt_pin.numpy()
+    prompt[:] = dex_synth.make_prompt(shape.vocab, n_prompt, wl.prompt_seed, seq=rank)
+    max_ctx = n_prompt + T + 8
+    FL = P.DEX_STEP_AUTOCOLLAPSE
+    g = P.Dex(shape, w_dev, X, max_ctx=max_ctx, device=dev, act_planes=args.act_planes)
+    a = P.Dex(shape, w_dev, (L,), max_ctx=max_ctx, device=dev, act_planes=args.act_planes)
+    g.prefill(0, prompt)
+    a.prefill(0, prompt)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    def max_over_ranks(ms):
+        if world == 1:
+            return ms
+        t = torch.tensor([ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    # ---- warm-up (>= 3 steps), also captures the CUDA graphs ----
+    W = max(3, args.warmup)
+    for _ in range(W):
+        g.rewind(0, n_prompt)
+        run_rounds(g, T, FL)
+    for _ in range(2):
+        a.rewind(0, n_prompt)
+        run_rounds(a, T, FL)
+
+    # ---- timed region: K steps, device time, max over ranks ----
+    g.profile(0)
+    clocks = ClockSampler(local_rank)
+    clocks.start()
+    barrier()
+    ms, (rounds, evals, crit, hist) = time_steps(torch, g, n_prompt, T, args.steps, FL)
+    barrier()
+    clk = clocks.stop()
+    _, counters = g.profile(-1)
+    ms = max_over_ranks(ms)
+    dex_tokens = g.tokens()[n_prompt:n_prompt + T].copy()
+    value = world * args.steps * T / (ms * 1e-3)
+
+    # ---- same-kernel AR baseline (X = {L}) ----
+    a.profile(0)
+    barrier()
+    ms_ar, (rounds_ar, _, _, _) = time_steps(torch, a, n_prompt, T, args.steps, FL)
+    barrier()
+    _, counters_ar = a.profile(-1)
+    ms_ar = max_over_ranks(ms_ar)
+    ar_tokens = a.tokens()[n_prompt:n_prompt + T].copy()
+    ar_value = world * args.steps * T / (ms_ar * 1e-3)
+    lossless = bool(np.array_equal(dex_tokens, ar_tokens))
+
+    # ---- e2e: host prompt -> dex_prefill -> rounds -> dex_get_tokens (host), per step ----
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    t0 = time.perf_counter()
+    e0.record(g.stream)
+    e2e_rounds = 0
+    for _ in range(args.steps):
+        g.prefill(0, prompt)
+        e2e_rounds += run_rounds(g, T, FL)[0]
+        out = g.tokens(0, n_prompt + T)
+    e1.record(g.stream)
+    barrier()
+    wall_ms = (time.perf_counter() - t0) * 1e3
+    ms_e2e = max_over_ranks(max(e0.elapsed_time(e1), 0.0))
+    assert np.array_equal(out[n_prompt:], dex_tokens)
+    res_bytes = __import__("ctypes").sizeof(P.DexStepResult)
+    e2e = {"value": world * args.steps * T / (ms_e2e * 1e-3), "unit": UNIT,
+           "h2d_bytes_per_step": int(4 * n_prompt + 4 * g.cfg.max_ctx // g.cfg.page_size + 4),
+           "d2h_bytes_per_step": int(res_bytes * e2e_rounds // args.steps + 4 * (n_prompt + T)),
+           "wall_ms_per_step": wall_ms / args.steps,
+           "includes": "dex_prefill of the pinned host prompt, all rounds with per-round host results, dex_get_tokens"}
+
+    # ---- roofline of the dominant kernel (segment GEMM k_gemm): one profiled pass of the same
+    #      workload with CUDA events around every launch on the library's stream ----
+    peak, peak_src = measured_hbm_peak()
+    roofline, phases = None, None
+    if rank == 0:
+        g.rewind(0, n_prompt)
+        g.profile(1)
+        run_rounds(g, T, FL)
+        ph, ct = g.profile(0)
+        gemm_us, gemm_launches, gemm_bytes = ph[1], ct[2], ct[3]
+        ach = gemm_bytes / (gemm_us * 1e-6) / 1e9
+        roofline = {"kernel": "k_gemm (segment projections, grouped over live stages)", "bound": "hbm",
+                    "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
+                    "frac_of_8TBs": ach / NOMINAL_HBM_GBS, "peak_source": peak_src, "traffic": None,
+                    "launches": int(gemm_launches), "avg_launch_us": gemm_us / max(1, gemm_launches),
+                    "algorithmic_bytes_per_launch": gemm_bytes / max(1, gemm_launches),
+                    "how": "profiled pass after the timed region: cudaEvent pair around each k_gemm launch on the "
+                           "library stream (graph replay and PDL overlap off), bytes = bf16 weights of the live stages"}
+        names = ("bookkeeping", "segment_gemm", "glue", "attention", "exit_gemm", "commit_collapse")
+        phases = {n: ph[i] / T for i, n in enumerate(names)}
+        phases["unit"] = "us per committed token (profiled pass, kernels serialised)"
+        exit_ach = ct[4] / (ph[4] * 1e-6) / 1e9 if ph[4] > 0 else None
+        phases["exit_gemm_GBs"] = exit_ach
+
+    # whole-step roofline of the timed region (north_star: weight + KV bytes touched per step)
+    step_bytes = (counters[3] + counters[4] + counters[5]) / args.steps
+    step_ach = step_bytes * args.steps / (ms * 1e-3) / 1e9
+    ar_bytes = (counters_ar[3] + counters_ar[4] + counters_ar[5]) / args.steps
+    ar_ach = ar_bytes * args.steps / (ms_ar * 1e-3) / 1e9
+
+    cpu = cpu_baseline(args, wl) if (rank == 0 and world == 1 and not args.no_cpu) else None
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": W,
+            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "bf16", "data": "synthetic",
+            "config": {"workload": f"{wl.key}: {shape.name} L={L} d={shape.d_model} X={list(X)} prompt={n_prompt} "
+                                   f"gen={T} bs=1 greedy decs=1",
+                       "parallelism": "replicas only" if world > 1 else "single GPU",
+                       "act_planes": args.act_planes,
+                       "l2": "inputs larger than L2 (13.5 GB of weights streamed per pass vs 126 MB L2)",
+                       "step": "dex_rewind to the prompt + DEX rounds until gen tokens are committed"},
+            "clocks": clk, "e2e": e2e, "gpu_launches": int(counters[1]),
+            "roofline": roofline, "cpu_baseline": cpu,
+            "ar_baseline": {"value": ar_value, "unit": UNIT, "ms_per_token": ms_ar / (args.steps * T),
+                            "hbm_GBs": ar_ach, "frac_of_measured_peak": ar_ach / peak, "frac_of_8TBs": ar_ach / NOMINAL_HBM_GBS,
+                            "what": "same library and kernels, X = {L}"},
+            "dex_over_ar": value / ar_value,
+            "dex_equals_ar_tokens": lossless,
+            "per_token": {"rounds": rounds / T, "layer_evals": evals / T, "critical_layers": crit / T,
+                          "ms": ms / (args.steps * T), "match_k_hist": hist[:N]},
+            "step_roofline": {"bytes_per_step": step_bytes, "achieved_GBs": step_ach, "frac_of_measured_peak": step_ach / peak,
+                              "frac_of_8TBs": step_ach / NOMINAL_HBM_GBS,
+                              "what": "weights of live stages + LM head per round + committed K/V attended, / timed region"},
+            "phases": phases,
+        }
+        print(json.dumps(line))
+    g.close()
+    a.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+# ------------------------------------------------------------------------------------------------
+def oracle_sample(wl, n_prompt, n_tokens, n_steps):
+    """The CPU oracle (NumPy, fp32 at the 7B-class shapes) on a bounded sample of the workload:
+    the workload's model tensors and exploration set, a prompt shortened to `n_prompt` tokens
+    (prefill untimed), `n_tokens` committed DEX tokens per step.  Returns (seconds per step list,
+    threads)."""
+    import copy
+    import dex_synth
+    import oracle
+    shape, X = wl.shape, wl.depths
+    w = dex_synth.make_weights(shape, wl.weight_seed, threads=16)
+    dt = np.float64 if shape.d_model <= 512 else np.float32
+    om = oracle.OracleModel(shape, w, dtype=dt, kv_round="bf16")
+    del w
+    p = dex_synth.make_prompt(shape.vocab, n_prompt, wl.prompt_seed)
+    from oracle.ar import prefill
+    state = prefill(om, [int(t) for t in p])
+    times = []
+    for _ in range(n_steps):
+        st = ([list(x) for x in state[0]], [list(x) for x in state[1]])
+        t0 = time.perf_counter()
+        oracle.dex_decode(om, p, n_tokens, X, decs=True, state=st)
+        times.append(time.perf_counter() - t0)
+    try:
+        from threadpoolctl import threadpool_info
+        threads = max([i.get("num_threads", 1) for i in threadpool_info()] + [1])
+    except Exception:
+        threads = os.cpu_count()
+    return times, threads
+
+
+def cpu_baseline(args, wl):
+    n_prompt, n_tok = (wl.prompt_len, 16) if wl.key == "c1" else (8, args.cpu_tokens)
+    times, threads = oracle_sample(wl, n_prompt, n_tok, 1)
+    return {"value": n_tok / times[0], "unit": UNIT, "cores": int(threads), "kind": "oracle",
+            "sample": f"{wl.key} tensors and X, prompt shortened to {n_prompt} tokens (prefill untimed), "
+                      f"{n_tok} committed DEX tokens, NumPy {'fp64' if wl.key == 'c1' else 'fp32'}, {times[0]:.1f} s"}
+
+
+def bench_reference(args):
+    rank, _, world = dist_env()
+    if rank != 0:
+        return
+    import dex_synth
+    wl = dex_synth.workload(args.workload)
+    n_prompt, n_tok = (wl.prompt_len, 16) if wl.key == "c1" else (8, 2)
+    W = min(args.warmup, 1)
+    times, threads = oracle_sample(wl, n_prompt, n_tok, W + args.steps)
+    t = times[W:]
+    value = n_tok * len(t) / sum(t)
+    sample = (f"{wl.key} tensors and X, prompt shortened to {n_prompt} tokens (prefill untimed), "
+              f"{n_tok} committed DEX tokens per step, NumPy {'fp64' if wl.key == 'c1' else 'fp32'}")
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": W, "ms_per_step": 1e3 * sum(t) / len(t), "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64" if wl.key == "c1" else "f32", "data": "synthetic",
+        "config": {"workload": f"{wl.key}: {wl.shape.name} X={list(wl.depths)} (CPU oracle, bounded sample)", "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": int(threads), "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="dex", choices=["dex", "reference"])
+    ap.add_argument("--workload", default="c2")
+    ap.add_argument("--gen-len", type=int, default=0)
+    ap.add_argument("--prompt-len", type=int, default=0)
+    ap.add_argument("--act-planes", type=int, default=2)
+    ap.add_argument("--cpu-tokens", type=int, default=4)
+    ap.add_argument("--no-cpu", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        bench_reference(args)
+    else:
+        bench_dex(args)
+
+
+if __name__ == "__main__":
+    main()

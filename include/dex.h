@@ -135,6 +135,14 @@ int32_t dex_step(dex_ctx* ctx, uint32_t flags, dex_step_result* out);
  * Used by tests and by the parity harness to teacher-force the oracle's token (R17). */
 int32_t dex_collapse(dex_ctx* ctx, int32_t seq, int32_t branch_k, int32_t token);
 
+/* Roll sequence `seq` back to its first n committed tokens (1 <= n <= committed count): the
+ * lattice is emptied (q <- 0), committed K/V of positions >= n-1 is dropped (its pages return
+ * to the pool), token n-1 becomes the next root-slot input, a pending commit is cancelled and
+ * `done` is cleared.  K/V of positions < n-1 is untouched, so rewinding to the prompt length
+ * restores exactly the state dex_prefill left (used by bench.py to repeat a run without
+ * re-prefilling).  DEX_ESTATE if the sequence was never prefilled.  Enqueued, not synchronised. */
+int32_t dex_rewind(dex_ctx* ctx, int32_t seq, int32_t n);
+
 /* Committed tokens of a sequence (prompt included) -> host int32[cap]; *n_out = count. */
 int32_t dex_get_tokens(dex_ctx* ctx, int32_t seq, int32_t* out, int32_t cap, int32_t* n_out);
 

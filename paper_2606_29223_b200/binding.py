@@ -47,6 +47,7 @@ _SIGNATURES = {
     "dex_prefill": (C.c_int32, [C.c_void_p, C.c_int32, C.POINTER(C.c_int32), C.c_int32]),
     "dex_step": (C.c_int32, [C.c_void_p, C.c_uint32, C.POINTER(DexStepResult)]),
     "dex_collapse": (C.c_int32, [C.c_void_p, C.c_int32, C.c_int32, C.c_int32]),
+    "dex_rewind": (C.c_int32, [C.c_void_p, C.c_int32, C.c_int32]),
     "dex_get_tokens": (C.c_int32, [C.c_void_p, C.c_int32, C.POINTER(C.c_int32), C.c_int32, C.POINTER(C.c_int32)]),
     "dex_debug_read": (C.c_int32, [C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_void_p, C.c_size_t]),
     "dex_debug_gemm": (C.c_int32, [C.c_void_p, C.c_int32, C.c_int32, C.POINTER(C.c_float), C.c_int32, C.POINTER(C.c_float)]),
@@ -114,6 +115,10 @@ def dex_step(ctx, flags, results):
 
 def dex_collapse(ctx, seq, branch_k, token):
     _check(lib().dex_collapse(ctx, seq, branch_k, token), ctx)
+
+
+def dex_rewind(ctx, seq, n):
+    _check(lib().dex_rewind(ctx, seq, n), ctx)
 
 
 def dex_get_tokens(ctx, seq, cap):
@@ -191,6 +196,9 @@ class Dex:
 
     def collapse(self, seq, branch_k, token):
         dex_collapse(self.ctx, seq, branch_k, token)
+
+    def rewind(self, seq, n):
+        dex_rewind(self.ctx, seq, n)
 
     def tokens(self, seq=0, cap=None):
         return dex_get_tokens(self.ctx, seq, cap or (self.cfg.max_ctx + 1))

@@ -720,6 +720,23 @@ int32_t dex_collapse(dex_ctx* c, int32_t seq, int32_t branch_k, int32_t token) {
   return DEX_OK;
 }
 
+int32_t dex_rewind(dex_ctx* c, int32_t seq, int32_t n) {
+  if (!c) return fail(nullptr, DEX_EINVAL, "null ctx");
+  if (seq < 0 || seq >= c->cfg.max_seqs) return fail(c, DEX_EINVAL, "seq out of range");
+  HostSeq& hs = c->seqs[seq];
+  if (!hs.active) return fail(c, DEX_ESTATE, "sequence %d was never prefilled", seq);
+  if (n < 1 || n > hs.n_tok) return fail(c, DEX_EINVAL, "n must be in [1, %d]", hs.n_tok);
+  const int keep = (n + c->cfg.page_size - 1) / c->cfg.page_size;   // pages holding positions < n
+  while ((int)hs.pages.size() > keep) {
+    c->free_pages.push_back(hs.pages.back());
+    hs.pages.pop_back();
+  }
+  CU(c, launch_seq_init(c->D, seq, n, c->stream));
+  hs.q = 0; hs.ctx_len = n - 1; hs.n_tok = n; hs.pending = 0; hs.done = (n >= c->cfg.max_ctx);
+  hs.last_q_before = 0;
+  return DEX_OK;
+}
+
 int32_t dex_get_tokens(dex_ctx* c, int32_t seq, int32_t* out, int32_t cap, int32_t* n_out) {
   if (!c || !out || !n_out) return fail(c, DEX_EINVAL, "null argument");
   if (seq < 0 || seq >= c->cfg.max_seqs) return fail(c, DEX_EINVAL, "seq out of range");
