@@ -61,6 +61,7 @@ typedef struct dex_config {
   int32_t debug_taps;    /* 1: keep per-layer hidden rows / anchor logits for dex_debug_read */
   int32_t act_planes;    /* 1: activations enter the MMAs as bf16; 2: as bf16 hi+lo pair  */
   int32_t use_graph;     /* 1: replay the step as a CUDA graph                            */
+  int32_t round_kernel;  /* 1: one persistent kernel per round (k_round); 0: one launch per op */
 } dex_config;
 
 /* Device pointers to the packed tensors (row-major, "out x in"; layout = dex_synth/gen.py):
@@ -152,11 +153,14 @@ int32_t dex_get_tokens(dex_ctx* ctx, int32_t seq, int32_t* out, int32_t cap, int
  *   DEX_TAP_LOGITS : final-depth anchor logits of the last round -> float[vocab]
  *                    (recomputed by a plain CUDA-core kernel from the anchor's exit row)
  *   DEX_TAP_B      : explore buffer B of `seq` -> int32[2^N - 1] (-1 = empty)
- *   DEX_TAP_FSM    : int32[4] = {q, ctx_len, n_tokens, pending}                         */
+ *   DEX_TAP_FSM    : int32[4] = {q, ctx_len, n_tokens, pending}
+ *   DEX_TAP_ROUND_TIMES : uint64[18 * max_m|Pi_m| + 4] SM clock-cycle stamps taken by CTA 0 of
+ *                    the last round kernel: start, then after every item phase and grid barrier */
 #define DEX_TAP_HIDDEN 1
 #define DEX_TAP_LOGITS 2
 #define DEX_TAP_B      3
 #define DEX_TAP_FSM    4
+#define DEX_TAP_ROUND_TIMES 5
 int32_t dex_debug_read(dex_ctx* ctx, int32_t what, int32_t seq, int32_t a, void* dst, size_t dst_bytes);
 
 /* Kernel-level tap for parity tests of the weight-streaming GEMM:
@@ -166,9 +170,9 @@ int32_t dex_debug_read(dex_ctx* ctx, int32_t what, int32_t seq, int32_t a, void*
 int32_t dex_debug_gemm(dex_ctx* ctx, int32_t which, int32_t layer, const float* x, int32_t rows, float* y);
 
 /* Per-kernel-class device time of the last dex_step in microseconds (CUDA events around each
- * launch on the context's stream; only while profiling is on, which bypasses graph replay):
- * host float[8] = {bookkeeping, segment GEMMs, glue (norm/rope/silu), attention, exit GEMM,
- * commit+collapse, 0, total}. */
+ * launch on the context's stream; only while profiling is on (dex_profile), which bypasses graph
+ * replay): host float[8] = {bookkeeping, segment GEMMs (or the whole round kernel), glue
+ * (norm/rope/silu), attention, exit GEMM, commit+collapse, 0, total}. */
 int32_t dex_debug_phase_us(dex_ctx* ctx, float* out8);
 
 /* Measurement hook used by bench.py.  Copies out (host double[8] each, may be NULL) the
@@ -176,7 +180,8 @@ int32_t dex_debug_phase_us(dex_ctx* ctx, float* out8);
  * (same classes as dex_debug_phase_us; zeros unless profiling was on) and the counters
  * {rounds, kernel launches, segment-GEMM launches, segment-GEMM algorithmic weight bytes,
  *  exit-GEMM LM-head bytes, committed-KV bytes attended, 0, 0}; then, if on >= 0, resets both
- * and switches profiling on (1) or off (0).  on < 0: read only. */
+ * and switches profiling off (0), on (1: the configured launch structure, graph replay off) or on
+ * through the per-op kernels (2: phase breakdown even when round_kernel = 1).  on < 0: read only. */
 int32_t dex_profile(dex_ctx* ctx, int32_t on, double* phase_us_acc8, double* counters8);
 
 int32_t dex_destroy(dex_ctx* ctx);

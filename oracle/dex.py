@@ -38,7 +38,7 @@ def dex_decode(model, prompt, T, X, decs=True, trace=False, state=None, force_to
         new_nodes = lt.level_nodes(q)
         rec = dict(q=q, n=n, nodes=new_nodes, rows_per_stage=[0] * N, layer_evals=0,
                    exit_rows=len(new_nodes), critical_layers=0)
-        new_h, new_u = {}, {}
+        new_h, new_u, new_margin = {}, {}, {}
         # ---- expand (Alg. 1 line 5): every new node through its stage -------------------
         for i in new_nodes:
             m = lt.stage(i)
@@ -70,6 +70,11 @@ def dex_decode(model, prompt, T, X, decs=True, trace=False, state=None, force_to
             if decs and i != ref_node:         # Alg. 2 lines 1-4: reference node never masked
                 masked = {u[a] if a in u else new_u[a] for a in lt.slot_chain_prior(i)}
             new_u[i] = argmax_lowest(logits, sorted(masked))
+            if trace:                          # trace only: top-2 gap among the unmasked logits of node i
+                lm = logits.copy()
+                lm[sorted(masked)] = -np.inf
+                top2 = np.sort(lm)[-2:]
+                new_margin[i] = float(top2[1] - top2[0])
             if i == ref_node:
                 logits_ref = logits
         u.update(new_u)
@@ -77,6 +82,7 @@ def dex_decode(model, prompt, T, X, decs=True, trace=False, state=None, force_to
         if trace:
             rec["h_out"] = {i: new_h[i].copy() for i in new_nodes}
             rec["u"] = dict(new_u)
+            rec["u_margin"] = dict(new_margin)
         # ---- commit / collapse or advance ------------------------------------------------
         if q == N - 1:                         # ReachFinalDepth(q)
             cand = [u[lt.anchor(k)] for k in range(N)]

@@ -8,7 +8,7 @@ import numpy as np
 DEX_OK, DEX_EINVAL, DEX_ECAPACITY, DEX_ESTATE, DEX_ECUDA = 0, -1, -2, -3, -4
 DEX_MAX_DEPTHS = 8
 DEX_STEP_AUTOCOLLAPSE = 1
-DEX_TAP_HIDDEN, DEX_TAP_LOGITS, DEX_TAP_B, DEX_TAP_FSM = 1, 2, 3, 4
+DEX_TAP_HIDDEN, DEX_TAP_LOGITS, DEX_TAP_B, DEX_TAP_FSM, DEX_TAP_ROUND_TIMES = 1, 2, 3, 4, 5
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 lib_path = os.path.join(_HERE, "libdex_b200.so")
@@ -24,7 +24,7 @@ class DexConfig(C.Structure):
     _fields_ = [(n, C.c_int32) for n in ("n_layers", "d_model", "n_heads", "n_kv_heads", "head_dim", "d_ffn", "vocab")] + \
                [("rms_eps", C.c_float), ("rope_theta", C.c_float)] + \
                [(n, C.c_int32) for n in ("max_seqs", "max_ctx", "page_size", "decs", "eos_id", "debug_taps",
-                                         "act_planes", "use_graph")]
+                                         "act_planes", "use_graph", "round_kernel")]
 
 
 class DexWeights(C.Structure):
@@ -161,7 +161,7 @@ class Dex:
     """Convenience owner of the device memory a context borrows (weights, workspace, stream)."""
 
     def __init__(self, shape, weights, depths, max_seqs=1, max_ctx=1024, page_size=128, decs=1, eos_id=-1,
-                 debug_taps=0, act_planes=2, use_graph=1, device="cuda:0", stream=None):
+                 debug_taps=0, act_planes=2, use_graph=1, round_kernel=1, device="cuda:0", stream=None):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2606_29223_b200 needs a CUDA device (no CPU fallback)")
@@ -170,7 +170,7 @@ class Dex:
         self.shape, self.depths = shape, tuple(int(d) for d in depths)
         self.cfg = DexConfig(shape.n_layers, shape.d_model, shape.n_heads, shape.n_kv_heads, shape.head_dim,
                              shape.d_ffn, shape.vocab, shape.rms_eps, shape.rope_theta, max_seqs, max_ctx, page_size,
-                             decs, eos_id, debug_taps, act_planes, use_graph)
+                             decs, eos_id, debug_taps, act_planes, use_graph, round_kernel)
         with torch.cuda.device(self.device):
             self.w = {}
             for k, v in weights.items():
@@ -234,6 +234,10 @@ class Dex:
 
     def tap_fsm(self, seq=0):
         return dex_debug_read(self.ctx, DEX_TAP_FSM, seq, 0, np.zeros(4, dtype=np.int32))
+
+    def tap_round_times(self):
+        n = 18 * max(b - a for a, b in zip((0,) + self.depths[:-1], self.depths)) + 4
+        return dex_debug_read(self.ctx, DEX_TAP_ROUND_TIMES, 0, 0, np.zeros(n, dtype=np.uint64))
 
     def gemm(self, which, layer, x):
         outs = (self.shape.qkv_out, self.shape.d_model, 2 * self.shape.d_ffn, self.shape.d_model)

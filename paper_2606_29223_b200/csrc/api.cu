@@ -4,6 +4,7 @@
 #include <algorithm>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <map>
 #include <memory>
@@ -20,9 +21,11 @@ cudaError_t launch_rows_prefill(const Dev&, int, int, int, cudaStream_t);
 cudaError_t launch_seq_init(const Dev&, int, int, cudaStream_t);
 cudaError_t launch_rope_table(const Dev&, double, int, cudaStream_t);
 cudaError_t launch_gather_norm(const Dev&, const Plan&, int, cudaStream_t);
-cudaError_t launch_add_norm(const Dev&, const Plan&, int, int, int, int, size_t, cudaStream_t);
-cudaError_t launch_rope_kv(const Dev&, const Plan&, int, int, int, size_t, cudaStream_t);
-cudaError_t launch_silu_mul(const Dev&, const Plan&, int, int, int, size_t, cudaStream_t);
+cudaError_t launch_add_norm(const Dev&, const Plan&, int, int, int, const OpDesc&, cudaStream_t);
+cudaError_t launch_rope_kv(const Dev&, const Plan&, int, int, const OpDesc&, cudaStream_t);
+cudaError_t launch_silu_mul(const Dev&, const Plan&, int, int, const OpDesc&, cudaStream_t);
+cudaError_t round_init();
+cudaError_t launch_round(const TmSet&, const RoundArgs&, int, size_t, cudaStream_t);
 cudaError_t launch_attn(const Dev&, const Plan&, int, int, int, int, cudaStream_t);
 cudaError_t launch_decide(const Dev&, const Plan&, int, cudaStream_t);
 cudaError_t launch_set_cmd(const Dev&, int, int, int, cudaStream_t);
@@ -41,10 +44,12 @@ std::string g_last_error;
 
 struct OpCfg {          // one projection: Y = X . W^T
   CUtensorMap tmW;
-  int out, k, n_tiles, ksplit, kbps, kb_total;
+  OpDesc dec;           // decode rounds: fine fixed K split (items of <= kDecodeKb K-blocks)
+  OpDesc pre;           // prefill chunks (128 rows): coarse split, fewer partials
 };
+constexpr int kDecodeKb = 8;
 struct RingCfg {        // shared-memory ring of the GEMM for a plan
-  int x_cap, n_stages, acc_cols;
+  int x_cap, n_stages, acc_cols, stacked;
   size_t smem;
 };
 struct HostSeq {
@@ -72,7 +77,8 @@ struct dex_ctx {
   dex_step_result* result_host;       // pinned, mapped
   float* dbg_stage;                   // device staging for debug taps (taps only)
   size_t dbg_floats;
-  size_t part_split_stride;
+  TmSet tms;
+  RingCfg round_ring;
   std::map<long long, cudaGraphExec_t> graphs;
   std::string err;
   // phase timing (taps only)
@@ -81,6 +87,7 @@ struct dex_ctx {
   float phase_us[8];
   double phase_us_acc[8];
   int profiling;
+  int phase_split;                    // profiling through the per-op kernels (phase breakdown) instead of k_round
   double counters[8];                 // rounds, kernel launches, gemm launches, gemm weight bytes, exit bytes, kv bytes
 };
 
@@ -119,6 +126,7 @@ int validate(const dex_config* cfg, const int32_t* depths, int32_t n) {
   if (cfg->page_size < 64 || cfg->page_size % 64) return fail(nullptr, DEX_EINVAL, "page_size must be a multiple of 64");
   if (cfg->max_seqs < 1 || cfg->max_seqs > 8) return fail(nullptr, DEX_EINVAL, "max_seqs must be in [1,8]");
   if (cfg->max_ctx < 2) return fail(nullptr, DEX_EINVAL, "max_ctx too small");
+  if (cfg->round_kernel != 0 && cfg->round_kernel != 1) return fail(nullptr, DEX_EINVAL, "round_kernel must be 0 or 1");
   if (cfg->act_planes != 1 && cfg->act_planes != 2) return fail(nullptr, DEX_EINVAL, "act_planes must be 1 or 2");
   if (cfg->vocab < 2) return fail(nullptr, DEX_EINVAL, "vocab too small");
   if (cfg->d_model > 8192) return fail(nullptr, DEX_ECAPACITY, "d_model > 8192 not supported");
@@ -126,28 +134,42 @@ int validate(const dex_config* cfg, const int32_t* depths, int32_t n) {
   return DEX_OK;
 }
 
-void choose_split(OpCfg& o, bool allow_split) {
-  o.n_tiles = (o.out + kTileM - 1) / kTileM;
-  o.kb_total = (o.k + kTileK - 1) / kTileK;
+void fill_desc(OpDesc& o, int out, int k, int R_cap) {
+  o.out_dim = out;
+  o.k_dim = k;
+  o.n_tiles = (out + kTileM - 1) / kTileM;
+  o.kb_total = (k + kTileK - 1) / kTileK;
+  o.part_ld = (int)align_up((size_t)out, 4);
+  o.split_stride = (size_t)R_cap * o.part_ld;
+}
+// prefill: split K only as far as needed to give every SM work
+void split_coarse(OpDesc& o, bool allow_split) {
   int S = 1;
   if (allow_split)
     while (S < 8 && o.n_tiles * S < 256 && S * 2 <= o.kb_total) S *= 2;
   o.kbps = (o.kb_total + S - 1) / S;
   o.ksplit = (o.kb_total + o.kbps - 1) / o.kbps;
 }
+// decode: items of <= kDecodeKb K-blocks (128 KiB of weights): many small items, dealt round-robin
+// across the ops of a round, keep every SM's byte count equal and fit the prefetch ring
+void split_fine(OpDesc& o, bool allow_split) {
+  o.kbps = allow_split ? std::min(kDecodeKb, o.kb_total) : o.kb_total;
+  o.ksplit = (o.kb_total + o.kbps - 1) / o.kbps;
+}
 
 // Shape-only quantities shared by dex_workspace_bytes and dex_init.
 struct Layout {
-  int N, R_dec, R_cap, part_ld, s_max, max_chunks, n_slots, n_nodes, pages_per_seq, n_pages, max_len, ref_tiles;
+  int N, R_dec, R_cap, max_chunks, n_slots, n_nodes, pages_per_seq, n_pages, max_len, ref_tiles;
   Plan dec, pre, ext;
   OpCfg op[5];
+  size_t part_floats;
   size_t off[40];
   size_t total;
   size_t dbg_floats;
 };
 enum Buf {
   B_SEQS, B_TOKENS, B_B, B_PT, B_ROWS, B_GNB, B_ENB, B_KEY, B_REFT, B_CMD, B_KPOOL, B_VPOOL, B_KSLOT, B_VSLOT,
-  B_XCUR, B_XFRONT, B_ACTA, B_ACTO, B_ACTF, B_ACTE, B_PART, B_QBUF, B_APART, B_ROPE, B_TAPH, B_DBG, B_COUNT
+  B_XCUR, B_XFRONT, B_ACTA, B_ACTO, B_ACTF, B_ACTE, B_PART, B_QBUF, B_APART, B_ROPE, B_TAPH, B_DBG, B_GBAR, B_TAPT, B_COUNT
 };
 
 void make_layout(const dex_config& c, const int32_t* depths, int n, Layout& L) {
@@ -160,14 +182,14 @@ void make_layout(const dex_config& c, const int32_t* depths, int n, Layout& L) {
   L.max_len = 0;
   for (int m = 0; m < n; ++m) {
     L.dec.row_base[m] = base;
-    L.dec.rows_cap[m] = round16i(c.max_seqs * cap_of(n, m));
+    L.dec.rows_cap[m] = c.max_seqs * cap_of(n, m);      // compact: a 16-row TMA box may run into the next group
     L.dec.layer_lo[m] = m ? depths[m - 1] : 0;
     L.dec.layer_len[m] = depths[m] - L.dec.layer_lo[m];
     L.max_len = std::max(L.max_len, L.dec.layer_len[m]);
     base += L.dec.rows_cap[m];
   }
   L.R_dec = base;
-  L.R_cap = round16i(std::max(L.R_dec, kPrefillRows));
+  L.R_cap = round16i(std::max(L.R_dec, kPrefillRows)) + 16;
   L.pre.n_grp = 1;
   L.pre.row_base[0] = 0;
   L.pre.rows_cap[0] = kPrefillRows;
@@ -183,19 +205,22 @@ void make_layout(const dex_config& c, const int32_t* depths, int n, Layout& L) {
   const int qkv_out = (c.n_heads + 2 * c.n_kv_heads) * c.head_dim;
   const int outs[5] = {qkv_out, c.d_model, 2 * c.d_ffn, c.d_model, c.vocab};
   const int ks[5] = {c.d_model, c.n_heads * c.head_dim, c.d_model, c.d_ffn, c.d_model};
-  L.s_max = 1;
+  L.part_floats = 0;
   for (int i = 0; i < 5; ++i) {
-    L.op[i].out = outs[i];
-    L.op[i].k = ks[i];
-    choose_split(L.op[i], i != 4);
-    if (i != 4) L.s_max = std::max(L.s_max, L.op[i].ksplit);
+    fill_desc(L.op[i].dec, outs[i], ks[i], L.R_cap);
+    fill_desc(L.op[i].pre, outs[i], ks[i], L.R_cap);
+    split_fine(L.op[i].dec, i != 4);
+    split_coarse(L.op[i].pre, i != 4);
+    if (i != 4) {
+      L.part_floats = std::max(L.part_floats, (size_t)L.op[i].dec.ksplit * L.op[i].dec.split_stride);
+      L.part_floats = std::max(L.part_floats, (size_t)L.op[i].pre.ksplit * L.op[i].pre.split_stride);
+    }
   }
-  L.part_ld = (int)align_up(std::max(std::max(qkv_out, 2 * c.d_ffn), c.d_model), 4);
   L.max_chunks = (c.max_ctx + n) / kChunk + 1;
   L.pages_per_seq = (c.max_ctx + c.page_size - 1) / c.page_size;
   L.n_pages = L.pages_per_seq * c.max_seqs;
-  L.ref_tiles = L.op[4].n_tiles * 4;
-  L.dbg_floats = c.debug_taps ? (size_t)kPrefillRows * (std::max(c.d_ffn, c.d_model) + L.part_ld) + c.vocab : 0;
+  L.ref_tiles = L.op[4].dec.n_tiles * 4;
+  L.dbg_floats = c.debug_taps ? (size_t)kPrefillRows * (std::max(c.d_ffn, c.d_model) + std::max(std::max(qkv_out, 2 * c.d_ffn), c.d_model) + 4) + c.vocab : 0;
 
   const size_t kv_pool = (size_t)c.n_layers * L.n_pages * c.page_size * c.n_kv_heads * c.head_dim * 2;
   const size_t kv_slot = (size_t)c.max_seqs * L.n_slots * c.n_layers * c.n_kv_heads * c.head_dim * 2;
@@ -221,12 +246,14 @@ void make_layout(const dex_config& c, const int32_t* depths, int n, Layout& L) {
   sz[B_ACTO] = 2 * P * R * c.n_heads * c.head_dim;
   sz[B_ACTF] = 2 * P * R * c.d_ffn;
   sz[B_ACTE] = 2 * P * R * c.d_model;
-  sz[B_PART] = sizeof(float) * (size_t)L.s_max * R * L.part_ld;
+  sz[B_PART] = sizeof(float) * L.part_floats;
   sz[B_QBUF] = sizeof(float) * R * c.n_heads * c.head_dim;
   sz[B_APART] = sizeof(float) * R * c.n_heads * (size_t)L.max_chunks * (c.head_dim + 2);
   sz[B_ROPE] = sizeof(float2) * (size_t)(c.max_ctx + kMaxAnc + 1) * (c.head_dim / 2);
   sz[B_TAPH] = c.debug_taps ? sizeof(float) * R * (size_t)L.max_len * c.d_model : 0;
   sz[B_DBG] = sizeof(float) * L.dbg_floats;
+  sz[B_GBAR] = 256;
+  sz[B_TAPT] = c.debug_taps ? sizeof(unsigned long long) * (18 * (size_t)L.max_len + 4) : 0;
   size_t off = 0;
   for (int i = 0; i < B_COUNT; ++i) {
     L.off[i] = off;
@@ -238,12 +265,13 @@ void make_layout(const dex_config& c, const int32_t* depths, int n, Layout& L) {
 RingCfg make_ring(const Plan& p, int planes) {
   RingCfg r;
   r.x_cap = 16;
-  for (int g = 0; g < p.n_grp; ++g) r.x_cap = std::max(r.x_cap, p.rows_cap[g]);
+  for (int g = 0; g < p.n_grp; ++g) r.x_cap = std::max(r.x_cap, round16i(p.rows_cap[g]));
   const size_t stage = 16384 + (size_t)planes * r.x_cap * 128;
   const size_t budget = 200 * 1024;
   r.n_stages = (int)std::max<size_t>(2, std::min<size_t>(12, budget / stage));
+  r.stacked = (planes == 2 && 2 * r.x_cap <= 256) ? 1 : 0;   // one {64, 16, 2} box per 16 rows, N = 2*nb
   r.acc_cols = 32;
-  while (r.acc_cols < r.x_cap) r.acc_cols *= 2;
+  while (r.acc_cols < (r.stacked ? 2 : 1) * r.x_cap) r.acc_cols *= 2;
   r.smem = r.n_stages * stage + 1024 + 512;
   return r;
 }
@@ -253,10 +281,10 @@ typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void
                              CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
 int encode_3d(dex_ctx* c, EncodeFn fn, CUtensorMap* tm, const void* base, uint64_t d0, uint64_t d1, uint64_t d2,
-              uint32_t box1) {
+              uint32_t box1, uint32_t box2 = 1) {
   cuuint64_t dims[3] = {d0, d1, d2};
   cuuint64_t strides[2] = {d0 * 2, d0 * d1 * 2};
-  cuuint32_t box[3] = {(cuuint32_t)kTileK, box1, 1};
+  cuuint32_t box[3] = {(cuuint32_t)kTileK, box1, box2};
   cuuint32_t es[3] = {1, 1, 1};
   CUresult r = fn(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(base), dims, strides, box, es,
                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
@@ -282,15 +310,14 @@ void ph_end(dex_ctx* c, Phase p) {
   c->ev_used[p]++;
 }
 
-int run_gemm(dex_ctx* c, int which, const CUtensorMap& tmX, const Plan& plan, const RingCfg& ring, int step, int mode,
-             const int* grp_nb) {
-  const OpCfg& o = c->op[which];
+int run_gemm(dex_ctx* c, int which, const OpDesc& o, const CUtensorMap& tmX, const Plan& plan, const RingCfg& ring, int step,
+             int mode, const int* grp_nb) {
   GemmArgs a;
   memset(&a, 0, sizeof a);
   a.plan = plan;
   a.step = step;
-  a.out_dim = o.out;
-  a.k_dim = o.k;
+  a.out_dim = o.out_dim;
+  a.k_dim = o.k_dim;
   a.n_tiles = o.n_tiles;
   a.ksplit = o.ksplit;
   a.kb_per_split = o.kbps;
@@ -300,12 +327,13 @@ int run_gemm(dex_ctx* c, int which, const CUtensorMap& tmX, const Plan& plan, co
   a.x_cap = ring.x_cap;
   a.n_stages = ring.n_stages;
   a.acc_cols = ring.acc_cols;
+  a.stacked = ring.stacked;
   a.grp_nb = grp_nb;
   a.rows = c->D.rows;
   a.n_rows = c->D.R_cap;
   a.part = c->D.part;
-  a.part_ld = c->D.part_ld;
-  a.part_split_stride = c->part_split_stride;
+  a.part_ld = o.part_ld;
+  a.part_split_stride = o.split_stride;
   a.best_key = c->D.best_key;
   a.ref_tile = c->D.ref_tile;
   a.ref_tiles = c->D.ref_tiles;
@@ -313,48 +341,70 @@ int run_gemm(dex_ctx* c, int which, const CUtensorMap& tmX, const Plan& plan, co
   if (which == 4) {   // the LM head is one [V, d] matrix: every exit chunk streams "layer" 0
     for (int g = 0; g < kMaxGrp; ++g) a.plan.layer_lo[g] = 0;
   }
-  CU(c, launch_gemm(o.tmW, tmX, a, c->n_sms, ring.smem, c->stream));
+  CU(c, launch_gemm(c->op[which].tmW, tmX, a, c->n_sms, ring.smem, c->stream));
   return DEX_OK;
 }
 
 // Layers of one plan: for j = 0 .. max_len-1, every live group runs its layer lo+j (a2 + a3).
-int enqueue_layers(dex_ctx* c, const Plan& plan, const RingCfg& ring, int rows, int n_chunks, int max_len) {
+int enqueue_layers(dex_ctx* c, const Plan& plan, const RingCfg& ring, int rows, int n_chunks, int max_len, bool prefill) {
   const Dev& D = c->D;
-  const size_t ss = c->part_split_stride;
+  const OpDesc* o[4];
+  for (int i = 0; i < 4; ++i) o[i] = prefill ? &c->op[i].pre : &c->op[i].dec;
   for (int j = 0; j < max_len; ++j) {
     int rc;
     ph_begin(c, PH_GEMM);
-    rc = run_gemm(c, 0, c->tmX[0], plan, ring, j, 0, D.grp_nb);
+    rc = run_gemm(c, 0, *o[0], c->tmX[0], plan, ring, j, 0, D.grp_nb);
     ph_end(c, PH_GEMM);
     if (rc) return rc;
     ph_begin(c, PH_GLUE);
-    CU(c, launch_rope_kv(D, plan, rows, j, c->op[0].ksplit, ss, c->stream));
+    CU(c, launch_rope_kv(D, plan, rows, j, *o[0], c->stream));
     ph_end(c, PH_GLUE);
     ph_begin(c, PH_ATTN);
-    CU(c, launch_attn(D, plan, rows, j, n_chunks, &plan == &c->dec_plan ? 1 : 0, c->stream));
+    CU(c, launch_attn(D, plan, rows, j, n_chunks, prefill ? 0 : 1, c->stream));
     ph_end(c, PH_ATTN);
     ph_begin(c, PH_GEMM);
-    rc = run_gemm(c, 1, c->tmX[1], plan, ring, j, 0, D.grp_nb);
+    rc = run_gemm(c, 1, *o[1], c->tmX[1], plan, ring, j, 0, D.grp_nb);
     ph_end(c, PH_GEMM);
     if (rc) return rc;
     ph_begin(c, PH_GLUE);
-    CU(c, launch_add_norm(D, plan, rows, j, 0, c->op[1].ksplit, ss, c->stream));
+    CU(c, launch_add_norm(D, plan, rows, j, 0, *o[1], c->stream));
     ph_end(c, PH_GLUE);
     ph_begin(c, PH_GEMM);
-    rc = run_gemm(c, 2, c->tmX[0], plan, ring, j, 0, D.grp_nb);
+    rc = run_gemm(c, 2, *o[2], c->tmX[0], plan, ring, j, 0, D.grp_nb);
     ph_end(c, PH_GEMM);
     if (rc) return rc;
     ph_begin(c, PH_GLUE);
-    CU(c, launch_silu_mul(D, plan, rows, j, c->op[2].ksplit, ss, c->stream));
+    CU(c, launch_silu_mul(D, plan, rows, j, *o[2], c->stream));
     ph_end(c, PH_GLUE);
     ph_begin(c, PH_GEMM);
-    rc = run_gemm(c, 3, c->tmX[2], plan, ring, j, 0, D.grp_nb);
+    rc = run_gemm(c, 3, *o[3], c->tmX[2], plan, ring, j, 0, D.grp_nb);
     ph_end(c, PH_GEMM);
     if (rc) return rc;
     ph_begin(c, PH_GLUE);
-    CU(c, launch_add_norm(D, plan, rows, j, 1, c->op[3].ksplit, ss, c->stream));
+    CU(c, launch_add_norm(D, plan, rows, j, 1, *o[3], c->stream));
     ph_end(c, PH_GLUE);
   }
+  return DEX_OK;
+}
+
+// The persistent round kernel: all layer-steps of all live stages + the exit head in one launch.
+int enqueue_round(dex_ctx* c, int n_chunks) {
+  RoundArgs a;
+  memset(&a, 0, sizeof a);
+  a.D = c->D;
+  a.dec = c->dec_plan;
+  a.ext = c->exit_plan;
+  for (int i = 0; i < 5; ++i) a.op[i] = c->op[i].dec;
+  a.x_cap = c->round_ring.x_cap;
+  a.n_stages = c->round_ring.n_stages;
+  { const char* e = getenv("DEX_STAGES"); if (e) a.n_stages = std::min(a.n_stages, atoi(e)); }
+  a.acc_cols = c->round_ring.acc_cols;
+  a.stacked = c->round_ring.stacked;
+  a.n_chunks = n_chunks;
+  { const char* e = getenv("DEX_DBG"); a.dbg = e ? atoi(e) : 0; }
+  ph_begin(c, PH_GEMM);
+  CU(c, launch_round(c->tms, a, c->n_sms, c->round_ring.smem, c->stream));
+  ph_end(c, PH_GEMM);
   return DEX_OK;
 }
 
@@ -371,12 +421,18 @@ int enqueue_step(dex_ctx* c, uint32_t flags, int n_chunks) {
   CU(c, launch_rows_decode(D, c->dec_plan, c->stream));
   CU(c, launch_gather_norm(D, c->dec_plan, D.R_dec, c->stream));
   ph_end(c, PH_BOOK);
-  int rc = enqueue_layers(c, c->dec_plan, c->dec_ring, D.R_dec, n_chunks, D.max_len);
-  if (rc) return rc;
-  ph_begin(c, PH_EXIT);
-  rc = run_gemm(c, 4, c->tmX[3], c->exit_plan, c->exit_ring, 0, 1, D.exit_nb);
-  ph_end(c, PH_EXIT);
-  if (rc) return rc;
+  int rc;
+  if (c->cfg.round_kernel && !c->phase_split) {
+    rc = enqueue_round(c, n_chunks);
+    if (rc) return rc;
+  } else {
+    rc = enqueue_layers(c, c->dec_plan, c->dec_ring, D.R_dec, n_chunks, D.max_len, false);
+    if (rc) return rc;
+    ph_begin(c, PH_EXIT);
+    rc = run_gemm(c, 4, c->op[4].dec, c->tmX[3], c->exit_plan, c->exit_ring, 0, 1, D.exit_nb);
+    ph_end(c, PH_EXIT);
+    if (rc) return rc;
+  }
   ph_begin(c, PH_COMMIT);
   CU(c, launch_decide(D, c->dec_plan, (flags & DEX_STEP_AUTOCOLLAPSE) ? 1 : 0, c->stream));
   ph_end(c, PH_COMMIT);
@@ -423,16 +479,17 @@ void account_round(dex_ctx* c) {
     for (int m = 0; m < D.N; ++m)
       if (live[m] && j < c->dec_plan.layer_len[m]) {
         any = true;
-        for (int i = 0; i < 4; ++i) wbytes += 2.0 * c->op[i].out * c->op[i].k;
+        for (int i = 0; i < 4; ++i) wbytes += 2.0 * c->op[i].dec.out_dim * c->op[i].dec.k_dim;
       }
     (void)any;
     gemm_launches += 4;
   }
+  const bool mega = c->cfg.round_kernel && !c->phase_split;
   c->counters[0] += 1;
-  c->counters[1] += 2 + 10.0 * D.max_len + 1 + 1 + 3;
-  c->counters[2] += gemm_launches;
+  c->counters[1] += mega ? 7.0 : 2 + 10.0 * D.max_len + 1 + 1 + 3;
+  c->counters[2] += mega ? 1 : gemm_launches;
   c->counters[3] += wbytes;
-  c->counters[4] += 2.0 * c->op[4].out * c->op[4].k * c->exit_plan.n_grp;
+  c->counters[4] += 2.0 * c->op[4].dec.out_dim * c->op[4].dec.k_dim * c->exit_plan.n_grp;
   c->counters[5] += kv;
 }
 
@@ -502,7 +559,8 @@ int32_t dex_init(dex_ctx** out, const dex_config* cfg, const dex_weights* w, con
   memset(c->phase_us, 0, sizeof c->phase_us);
   memset(c->phase_us_acc, 0, sizeof c->phase_us_acc);
   memset(c->counters, 0, sizeof c->counters);
-  c->profiling = cfg->debug_taps ? 1 : 0;
+  c->profiling = 0;
+  c->phase_split = 0;
   int dev = 0;
   cudaGetDevice(&dev);
   cudaDeviceGetAttribute(&c->n_sms, cudaDevAttrMultiProcessorCount, dev);
@@ -516,7 +574,7 @@ int32_t dex_init(dex_ctx** out, const dex_config* cfg, const dex_weights* w, con
   D.max_seqs = cfg->max_seqs; D.max_ctx = cfg->max_ctx; D.page_size = cfg->page_size;
   D.pages_per_seq = L.pages_per_seq; D.n_pages = L.n_pages; D.n_slots = L.n_slots; D.n_nodes = L.n_nodes;
   D.R_cap = L.R_cap; D.R_dec = L.R_dec; D.decs = cfg->decs; D.planes = cfg->act_planes; D.taps = cfg->debug_taps;
-  D.max_len = L.max_len; D.part_ld = L.part_ld; D.max_chunks = L.max_chunks; D.ref_tiles = L.ref_tiles;
+  D.max_len = L.max_len; D.max_chunks = L.max_chunks; D.ref_tiles = L.ref_tiles;
   D.embed = static_cast<const __nv_bfloat16*>(w->embed);
   D.lm_head = static_cast<const __nv_bfloat16*>(w->lm_head);
   D.norm_attn = w->norm_attn; D.norm_ffn = w->norm_ffn; D.norm_final = w->norm_final;
@@ -532,14 +590,21 @@ int32_t dex_init(dex_ctx** out, const dex_config* cfg, const dex_weights* w, con
   D.act_f = WSP(__nv_bfloat16, B_ACTF); D.act_e = WSP(__nv_bfloat16, B_ACTE);
   D.part = WSP(float, B_PART); D.qbuf = WSP(float, B_QBUF); D.attn_part = WSP(float, B_APART);
   D.rope = WSP(float2, B_ROPE); D.tap_hidden = cfg->debug_taps ? WSP(float, B_TAPH) : nullptr;
+  D.gbar = WSP(unsigned int, B_GBAR);
+  D.tap_times = cfg->debug_taps ? WSP(unsigned long long, B_TAPT) : nullptr;
   c->dbg_stage = cfg->debug_taps ? WSP(float, B_DBG) : nullptr;
   c->dbg_floats = L.dbg_floats;
 #undef WSP
-  c->part_split_stride = (size_t)L.R_cap * L.part_ld;
   for (int i = 0; i < 5; ++i) c->op[i] = L.op[i];
   c->dec_ring = make_ring(c->dec_plan, cfg->act_planes);
   c->pre_ring = make_ring(c->pre_plan, cfg->act_planes);
   c->exit_ring = make_ring(c->exit_plan, cfg->act_planes);
+  {   // the round kernel streams the decode stages and the exit chunks through one ring
+    Plan both = c->dec_plan;
+    both.n_grp = 1;
+    both.rows_cap[0] = std::max(c->dec_ring.x_cap, c->exit_ring.x_cap);
+    c->round_ring = make_ring(both, cfg->act_planes);
+  }
 
 #define INIT_FAIL(expr)          \
   do {                           \
@@ -559,17 +624,31 @@ int32_t dex_init(dex_ctx** out, const dex_config* cfg, const dex_weights* w, con
     return fail(nullptr, DEX_ECUDA, "cuTensorMapEncodeTiled entry point not found");
   }
   EncodeFn enc = reinterpret_cast<EncodeFn>(fnp);
+  if (round_init() != cudaSuccess) {
+    delete c;
+    return fail(nullptr, DEX_ECUDA, "cannot raise the round kernel's dynamic shared memory limit");
+  }
   if (gemm_init() != cudaSuccess) {
     delete c;
     return fail(nullptr, DEX_ECUDA, "cannot raise the GEMM kernel's dynamic shared memory limit");
   }
   const void* wptr[5] = {w->wqkv, w->wo, w->wgu, w->wdn, w->lm_head};
   for (int i = 0; i < 5; ++i)
-    INIT_FAIL(encode_3d(c, enc, &c->op[i].tmW, wptr[i], c->op[i].k, c->op[i].out, i == 4 ? 1 : D.L, kTileM));
+    INIT_FAIL(encode_3d(c, enc, &c->op[i].tmW, wptr[i], c->op[i].dec.k_dim, c->op[i].dec.out_dim, i == 4 ? 1 : D.L, kTileM));
+  // every ring of this context must agree on the activation box (one tensor map per operand)
+  const bool all_stacked = c->dec_ring.stacked && c->pre_ring.stacked && c->exit_ring.stacked && c->round_ring.stacked;
+  c->dec_ring.stacked = c->pre_ring.stacked = c->exit_ring.stacked = c->round_ring.stacked = all_stacked ? 1 : 0;
   const void* xptr[4] = {D.act_a, D.act_o, D.act_f, D.act_e};
   const int xk[4] = {D.d, D.nh * D.hd, D.ffn, D.d};
   for (int i = 0; i < 4; ++i)
-    INIT_FAIL(encode_3d(c, enc, &c->tmX[i], xptr[i], xk[i], D.R_cap, cfg->act_planes, kBoxRows));
+    INIT_FAIL(encode_3d(c, enc, &c->tmX[i], xptr[i], xk[i], D.R_cap, cfg->act_planes, kBoxRows, all_stacked ? 2 : 1));
+  for (int i = 0; i < 5; ++i) c->tms.w[i] = c->op[i].tmW;
+  for (int i = 0; i < 5; ++i) {
+    const OpDesc& o = c->op[i].dec;
+    const uint64_t n_t = (uint64_t)(i == 4 ? 1 : D.L) * o.out_dim * o.k_dim / (kTileM * kTileK);
+    INIT_FAIL(encode_3d(c, enc, &c->tms.wt[i], wptr[i], kTileK, kTileM, n_t, kTileM));
+  }
+  for (int i = 0; i < 4; ++i) c->tms.x[i] = c->tmX[i];
 
   // state: FSM zeroed, free pages, result buffer, RoPE table
   auto cu_or_fail = [&](cudaError_t e, const char* what) -> int {
@@ -627,7 +706,7 @@ int32_t dex_prefill(dex_ctx* c, int32_t seq, const int32_t* prompt, int32_t n) {
     CU(c, launch_rows_prefill(D, seq, p0, R, c->stream));
     CU(c, launch_gather_norm(D, c->pre_plan, R, c->stream));
     const int n_chunks = (p0 + R - 1) / kChunk + 1;
-    rc = enqueue_layers(c, c->pre_plan, c->pre_ring, R, n_chunks, D.L);
+    rc = enqueue_layers(c, c->pre_plan, c->pre_ring, R, n_chunks, D.L, true);
     if (rc) return rc;
   }
   CU(c, launch_seq_init(D, seq, n, c->stream));
@@ -782,6 +861,13 @@ int32_t dex_debug_read(dex_ctx* c, int32_t what, int32_t seq, int32_t a, void* d
     CU(c, cudaStreamSynchronize(c->stream));
     return DEX_OK;
   }
+  if (what == DEX_TAP_ROUND_TIMES) {
+    const size_t bytes = sizeof(unsigned long long) * (18 * (size_t)D.max_len + 4);
+    if (dst_bytes < bytes) return fail(c, DEX_EINVAL, "dst too small");
+    CU(c, cudaMemcpyAsync(dst, D.tap_times, bytes, cudaMemcpyDeviceToHost, c->stream));
+    CU(c, cudaStreamSynchronize(c->stream));
+    return DEX_OK;
+  }
   if (what == DEX_TAP_LOGITS) {
     if (hs.last_q_before != D.N - 1) return fail(c, DEX_ESTATE, "the last round did not reach final depth");
     if (dst_bytes < sizeof(float) * D.vocab) return fail(c, DEX_EINVAL, "dst too small");
@@ -802,21 +888,21 @@ int32_t dex_debug_gemm(dex_ctx* c, int32_t which, int32_t layer, const float* x,
   if (layer < 0 || layer >= c->D.L) return fail(c, DEX_EINVAL, "layer out of range");
   if (rows < 1 || rows > kPrefillRows) return fail(c, DEX_EINVAL, "rows must be in [1,128]");
   const Dev& D = c->D;
-  const OpCfg& o = c->op[which];
+  const OpDesc& o = c->op[which].dec;
   __nv_bfloat16* act[4] = {D.act_a, D.act_o, D.act_a, D.act_f};
   const int xm[4] = {0, 1, 0, 2};
   float* xs = c->dbg_stage;
   float* ys = c->dbg_stage + (size_t)kPrefillRows * std::max(D.ffn, D.d);
-  CU(c, cudaMemcpyAsync(xs, x, sizeof(float) * (size_t)rows * o.k, cudaMemcpyHostToDevice, c->stream));
+  CU(c, cudaMemcpyAsync(xs, x, sizeof(float) * (size_t)rows * o.k_dim, cudaMemcpyHostToDevice, c->stream));
   CU(c, launch_debug_rows(D, rows, c->stream));
-  CU(c, launch_debug_split(xs, act[which], rows, o.k, (size_t)D.R_cap * o.k, D.planes, c->stream));
+  CU(c, launch_debug_split(xs, act[which], rows, o.k_dim, (size_t)D.R_cap * o.k_dim, D.planes, c->stream));
   Plan p = c->pre_plan;
   p.layer_lo[0] = layer;
   p.layer_len[0] = 1;
-  int rc = run_gemm(c, which, c->tmX[xm[which]], p, c->pre_ring, 0, 0, D.grp_nb);
+  int rc = run_gemm(c, which, o, c->tmX[xm[which]], p, c->pre_ring, 0, 0, D.grp_nb);
   if (rc) return rc;
-  CU(c, launch_debug_sum(D.part, ys, rows, o.out, D.part_ld, o.ksplit, c->part_split_stride, c->stream));
-  CU(c, cudaMemcpyAsync(y, ys, sizeof(float) * (size_t)rows * o.out, cudaMemcpyDeviceToHost, c->stream));
+  CU(c, launch_debug_sum(D.part, ys, rows, o.out_dim, o.part_ld, o.ksplit, o.split_stride, c->stream));
+  CU(c, cudaMemcpyAsync(y, ys, sizeof(float) * (size_t)rows * o.out_dim, cudaMemcpyDeviceToHost, c->stream));
   CU(c, cudaStreamSynchronize(c->stream));
   for (int ph = 0; ph < PH_N; ++ph) c->ev_used[ph] = 0;
   return DEX_OK;
@@ -834,7 +920,8 @@ int32_t dex_profile(dex_ctx* c, int32_t on, double* phase_us_acc8, double* count
   if (phase_us_acc8) memcpy(phase_us_acc8, c->phase_us_acc, sizeof(double) * 8);
   if (counters8) memcpy(counters8, c->counters, sizeof(double) * 8);
   if (on >= 0) {
-    c->profiling = (on || c->cfg.debug_taps) ? 1 : 0;
+    c->profiling = on ? 1 : 0;
+    c->phase_split = (on == 2) ? 1 : 0;
     memset(c->phase_us_acc, 0, sizeof c->phase_us_acc);
     memset(c->counters, 0, sizeof c->counters);
   }

@@ -97,8 +97,8 @@ struct Dev {
   int* grp_nb;             // [kMaxGrp] live row extent per decode/prefill group (multiple of 16)
   int* exit_nb;            // [kMaxGrp] live row extent per exit chunk
   __nv_bfloat16 *act_a, *act_o, *act_f, *act_e;   // [planes][R_cap][K] MMA operands
-  float* part;             // [S][R_cap][part_ld] split-K partial sums
-  int part_ld;
+  float* part;             // split-K partial sums, per op [S_op][R_cap][ld_op] (OpDesc)
+  unsigned int* gbar;      // grid-barrier arrival counter of the round kernel (reset every round)
   float* qbuf;             // [R_cap][nh*hd]
   float* attn_part;        // [R_cap][nh][max_chunks][hd + 2]
   int max_chunks;
@@ -109,6 +109,7 @@ struct Dev {
   CollapseCmd* cmd;        // [max_seqs]
   dex_step_result* result_dev;    // [max_seqs] (mapped pinned host memory)
   float* tap_hidden;       // [R_cap][max_len][d] (taps only)
+  unsigned long long* tap_times;  // [18 * max_len + 4] globaltimer stamps of CTA 0 in k_round (taps only)
   int n_pages;
 };
 
@@ -176,6 +177,7 @@ struct GemmArgs {
   int x_cap;               // activation rows per ring stage (multiple of 16)
   int n_stages;            // ring depth
   int acc_cols;            // TMEM columns per accumulator stage (power of two >= 32)
+  int stacked;             // 1: both activation planes are one B operand of N = x_cap + nb (gemm_dev.cuh)
   const int* grp_nb;
   const RowInfo* rows;
   int n_rows;              // R_cap
@@ -186,6 +188,31 @@ struct GemmArgs {
   float2* ref_tile;
   int ref_tiles;
   int vocab;
+};
+
+// One projection kind (Y = X . W^T) and its fixed split of K: the split depends on the operator
+// shape only, never on how many rows or stages share a launch (H3: DEX stream == AR stream).
+struct OpDesc {
+  int out_dim, k_dim;
+  int n_tiles;             // ceil(out / 128)
+  int ksplit, kbps, kb_total;
+  int part_ld;             // row stride of this op's partials (out rounded up to 4)
+  size_t split_stride;     // R_cap * part_ld
+};
+
+struct TmSet {             // TMA descriptors of the round kernel: weights qkv,o,gu,dn,lm_head; operands a,o,f,e
+  CUtensorMap w[5];
+  CUtensorMap x[4];
+  CUtensorMap wt[5];       // timing experiment: the same bytes viewed as contiguous 16 KiB tiles
+};
+
+struct RoundArgs {
+  Dev D;
+  Plan dec, ext;
+  OpDesc op[5];
+  int x_cap, n_stages, acc_cols, stacked;   // shared-memory ring / TMEM geometry
+  int n_chunks;                    // attention chunks that can hold a live position (host upper bound)
+  int dbg;                         // timing experiments only (env DEX_DBG): 1 skip glue math, 2 skip barriers
 };
 
 }  // namespace dexk

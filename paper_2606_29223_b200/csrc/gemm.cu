@@ -18,11 +18,11 @@
 // rows or stages share the launch (H3: DEX stream == AR stream).
 #include "common.cuh"
 #include "ptx.cuh"
+#include "gemm_dev.cuh"
 
 namespace dexk {
 
 constexpr int kGemmThreads = 192;
-constexpr uint32_t kABytes = kTileM * kTileK * 2;  // 16 KiB
 
 struct Item {
   int g, tile, split, nb, layer, kb0, kb1;
@@ -133,9 +133,14 @@ k_gemm(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CUtensor
             mbar_expect_tx(&full[stage], tx);
             tma_load_3d(sA, &tmW, &full[stage], kb * kTileK, it.tile * kTileM, it.layer, kEvictFirst);
           }
-          for (int p = 0; p < a.planes; ++p)
+          if (a.stacked) {
             for (int r = 0; r < it.nb; r += kBoxRows)
-              tma_load_3d(sB + p * plane_bytes + r * 128, &tmX, &full[stage], kb * kTileK, row0 + r, p, kEvictLast);
+              tma_load_3d(sB + r * 256, &tmX, &full[stage], kb * kTileK, row0 + r, 0, kEvictLast);
+          } else {
+            for (int p = 0; p < a.planes; ++p)
+              for (int r = 0; r < it.nb; r += kBoxRows)
+                tma_load_3d(sB + p * plane_bytes + r * 128, &tmX, &full[stage], kb * kTileK, row0 + r, p, kEvictLast);
+          }
           if (++stage == a.n_stages) {
             stage = 0;
             phase ^= 1;
@@ -156,22 +161,12 @@ k_gemm(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CUtensor
         mbar_wait(&tempty[as], aphase ^ 1);
         tc_fence_after();
         const uint32_t d_tmem = tmem_base + as * a.acc_cols;
-        const uint32_t idesc = make_idesc_bf16_m128(it.nb);
+        const uint32_t idesc = make_idesc_bf16_m128(a.stacked ? 2 * it.nb : it.nb);
         uint32_t acc = 0;
         for (int kb = it.kb0; kb < it.kb1; ++kb) {
           mbar_wait(&full[stage], phase);
           tc_fence_after();
-          const uint32_t sA = smem_u32(smem + (size_t)stage * stage_bytes);
-          const uint32_t sB = sA + kABytes;
-          for (int p = 0; p < a.planes; ++p) {
-            const uint64_t da = make_sw128_kmajor_desc(sA);
-            const uint64_t db = make_sw128_kmajor_desc(sB + p * plane_bytes);
-#pragma unroll
-            for (int k = 0; k < kTileK / 16; ++k) {
-              umma_bf16(d_tmem, da + (k * 32 >> 4), db + (k * 32 >> 4), idesc, acc);
-              acc = 1;
-            }
-          }
+          mma_stage(smem_u32(smem + (size_t)stage * stage_bytes), plane_bytes, a.planes, a.stacked != 0, d_tmem, idesc, acc);
           umma_commit(&empty[stage]);   // frees the ring slot when these MMAs have read it
           if (++stage == a.n_stages) {
             stage = 0;
@@ -185,6 +180,10 @@ k_gemm(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CUtensor
   } else {
     // ===================== epilogue (warps 2..5) =====================
     const int quarter = warp & 3;       // TMEM lanes 32*quarter .. +31 are this warp's
+    EpiCtx ec;
+    ec.mode = a.mode; ec.rows = a.rows; ec.s_valid = s_valid; ec.part = a.part; ec.part_ld = a.part_ld;
+    ec.split_stride = a.part_split_stride; ec.out_dim = a.out_dim; ec.vocab = a.vocab; ec.best_key = a.best_key;
+    ec.ref_tile = a.ref_tile; ec.ref_tiles = a.ref_tiles;
     int n_it = 0;
     for (int item = blockIdx.x; item < n_items; item += gridDim.x, ++n_it) {
       Item it = decode_item(a, item, live_g, live_nb);
@@ -193,47 +192,8 @@ k_gemm(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CUtensor
       mbar_wait(&tfull[as], aphase);
       tc_fence_after();
       const uint32_t t_addr = tmem_base + as * a.acc_cols + ((uint32_t)(quarter * 32) << 16);
-      const int col = it.tile * kTileM + quarter * 32 + lane;   // out feature / vocabulary id
       const int row0 = a.plan.row_base[it.g];
-      for (int c0 = 0; c0 < it.nb; c0 += 16) {
-        uint32_t v[16];
-        tmem_ld16(t_addr + c0, v);
-        tmem_ld_wait();
-        if (a.mode == 0) {
-          float* dst = a.part + (size_t)it.split * a.part_split_stride + (size_t)(row0 + c0) * a.part_ld + col;
-#pragma unroll
-          for (int i = 0; i < 16; ++i) {
-            const int rr = row0 + c0 + i;
-            if (((s_valid[rr >> 5] >> (rr & 31)) & 1u) && col < a.out_dim) dst[(size_t)i * a.part_ld] = __uint_as_float(v[i]);
-          }
-        } else {
-#pragma unroll
-          for (int i = 0; i < 16; ++i) {
-            const int rr = row0 + c0 + i;
-            if (!((s_valid[rr >> 5] >> (rr & 31)) & 1u)) continue;   // warp-uniform
-            const RowInfo* ri = &a.rows[rr];
-            float val = __uint_as_float(v[i]);
-            bool dead = col >= a.vocab;
-            const int nm = ri->n_mask;                      // Alg. 2 lines 5-7: mask prior proposals
-            for (int t = 0; t < nm; ++t) dead |= (ri->mask_tok[t] == col);
-            uint32_t key = dead ? 0u : f2key(val);
-            uint32_t best = __reduce_max_sync(0xffffffffu, key);
-            uint32_t who = __ballot_sync(0xffffffffu, key == best);
-            int wl = __ffs(who) - 1;                        // lowest lane = lowest token id (R11)
-            if (best != 0u && lane == wl) {
-              unsigned long long k64 = ((unsigned long long)best << 32) | (unsigned long long)(0xFFFFFFFFu - (uint32_t)col);
-              atomicMax(&a.best_key[row0 + c0 + i], k64);
-            }
-            if (ri->is_ref) {                               // top-2 of the reference node, for margin reporting
-              uint32_t key2 = (lane == wl) ? 0u : key;
-              uint32_t second = __reduce_max_sync(0xffffffffu, key2);
-              if (lane == 0)
-                a.ref_tile[(size_t)ri->seq * a.ref_tiles + it.tile * 4 + quarter] =
-                    make_float2(best ? key2f(best) : -INFINITY, second ? key2f(second) : -INFINITY);
-            }
-          }
-        }
-      }
+      epilogue_item(ec, t_addr, a.stacked != 0, it.nb, row0, row0 + a.plan.rows_cap[it.g], it.tile, it.split, quarter, lane);
       tc_fence_before();
       __syncwarp();
       if (lane == 0) mbar_arrive(&tempty[as]);

@@ -43,16 +43,11 @@ __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;\
 
 __device__ __forceinline__ float4 ld4(const float* p) { return *reinterpret_cast<const float4*>(p); }
 __device__ __forceinline__ float4 add4(float4 a, float4 b) { return make_float4(a.x + b.x, a.y + b.y, a.z + b.z, a.w + b.w); }
-// sum of up to 8 split-K partials, loads issued together, added in split order (fixed order: H3)
+// sum of the split-K partials, added in split order (fixed order: H3)
 __device__ __forceinline__ float4 sum_splits4(const float* p, int ksplit, size_t split_stride) {
-  float4 v[8];
-#pragma unroll
-  for (int s = 0; s < 8; ++s)
-    if (s < ksplit) v[s] = ld4(p + (size_t)s * split_stride);
-  float4 acc = v[0];
-#pragma unroll
-  for (int s = 1; s < 8; ++s)
-    if (s < ksplit) acc = add4(acc, v[s]);
+  float4 acc = ld4(p);
+#pragma unroll 4
+  for (int s = 1; s < ksplit; ++s) acc = add4(acc, ld4(p + (size_t)s * split_stride));
   return acc;
 }
 __device__ __forceinline__ void split_store4(__nv_bfloat16* base, size_t plane_stride, size_t idx, float4 v, int planes) {
@@ -81,6 +76,7 @@ __device__ __forceinline__ int stage_count(int q, int m) { return m > q ? 0 : (m
 __global__ void k_rows_decode(Dev D, Plan plan) {
   const int r = blockIdx.x * blockDim.x + threadIdx.x;
   if (r == 0) {
+    *D.gbar = 0u;                                     // grid-barrier counter of this round's k_round
     // live row extent of every stage group and of every exit chunk
     int max_end = 0;
     for (int m = 0; m < kMaxGrp; ++m) {
@@ -268,7 +264,7 @@ __global__ void __launch_bounds__(1024) k_gather_norm(Dev D, Plan plan) {
 //   mode 1 (after down_proj): w = norm_attn[l+1] if the stage continues -> act_a,
 //                             else the shared final norm (exit) -> act_e
 // One CTA per row, one float4 per thread and pass (d <= 8192), all split loads in flight at once.
-__global__ void __launch_bounds__(1024) k_add_norm(Dev D, Plan plan, int step, int mode, int ksplit, size_t split_stride) {
+__global__ void __launch_bounds__(1024) k_add_norm(Dev D, Plan plan, int step, int mode, int ksplit, size_t split_stride, int ld) {
   __shared__ float red[33];
   pdl_trigger();
   const int r = blockIdx.x;
@@ -276,7 +272,7 @@ __global__ void __launch_bounds__(1024) k_add_norm(Dev D, Plan plan, int step, i
   if (!ri.valid || step >= plan.layer_len[ri.grp]) return;
   const int layer = plan.layer_lo[ri.grp] + step;
   float* x = D.x_cur + (size_t)r * D.d;
-  const float* p = D.part + (size_t)r * D.part_ld;
+  const float* p = D.part + (size_t)r * ld;
   const int nv = D.d >> 2;
   pdl_wait();
   float4 xv[2];
@@ -320,14 +316,14 @@ __global__ void __launch_bounds__(1024) k_add_norm(Dev D, Plan plan, int step, i
 // q,k,v = sum of split-K partials; RoPE (rotate-half, R13) on q,k; q -> fp32 buffer; k,v -> bf16
 // into the row's slot K/V (branch-private) or, for prefill rows, straight into committed pages.
 // grid (rows, blocks): a thread owns 4 consecutive dims of one head (and their rotate-half partners).
-__global__ void __launch_bounds__(256) k_rope_kv(Dev D, Plan plan, int step, int ksplit, size_t split_stride) {
+__global__ void __launch_bounds__(256) k_rope_kv(Dev D, Plan plan, int step, int ksplit, size_t split_stride, int ld) {
   pdl_trigger();
   const int r = blockIdx.x;
   const RowInfo ri = D.rows[r];
   if (!ri.valid || step >= plan.layer_len[ri.grp]) return;
   const int layer = plan.layer_lo[ri.grp] + step;
   const int hd = D.hd, half = hd / 2, qd = half / 4;     // qd: float4 groups per half head
-  const float* p = D.part + (size_t)r * D.part_ld;
+  const float* p = D.part + (size_t)r * ld;
   const float2* rt = D.rope + (size_t)ri.pos * half;
   const size_t kvo = (ri.slot >= 0) ? slot_off(D, ri.seq, ri.slot, layer) : page_off(D, ri.seq, layer, ri.pos);
   __nv_bfloat16* kd = ((ri.slot >= 0) ? D.kslot : D.kpool) + kvo;
@@ -366,12 +362,12 @@ __global__ void __launch_bounds__(256) k_rope_kv(Dev D, Plan plan, int step, int
 }
 
 // act = SiLU(gate) * up  (SwiGLU), from the split-K partials of the fused gate/up projection.
-__global__ void __launch_bounds__(256) k_silu_mul(Dev D, Plan plan, int step, int ksplit, size_t split_stride) {
+__global__ void __launch_bounds__(256) k_silu_mul(Dev D, Plan plan, int step, int ksplit, size_t split_stride, int ld) {
   pdl_trigger();
   const int r = blockIdx.x;
   const RowInfo ri = D.rows[r];
   if (!ri.valid || step >= plan.layer_len[ri.grp]) return;
-  const float* p = D.part + (size_t)r * D.part_ld;
+  const float* p = D.part + (size_t)r * ld;
   const size_t ps = (size_t)D.R_cap * D.ffn;
   pdl_wait();
   for (int i = (blockIdx.y * blockDim.x + threadIdx.x) * 4; i < D.ffn; i += gridDim.y * blockDim.x * 4) {
@@ -422,7 +418,7 @@ __global__ void __launch_bounds__(128) k_attn(Dev D, Plan plan, int step, int kv
   __syncthreads();
   for (int r = plan.row_base[m] + threadIdx.x; r < plan.row_base[m] + nb; r += blockDim.x) {
     const RowInfo* ri = &D.rows[r];
-    if (ri->valid && ri->seq == s && ri->pos >= c0) {
+    if (ri->valid && ri->grp == m && ri->seq == s && ri->pos >= c0) {
       int k = atomicAdd(&n_rows_s, 1);
       row_list[k] = r;
       atomicMax(&max_pos_s, ri->pos);
@@ -871,15 +867,15 @@ cudaError_t launch_gather_norm(const Dev& D, const Plan& p, int rows, cudaStream
   k_gather_norm<<<rows, norm_threads(D.d), 0, st>>>(D, p);
   DEX_LAUNCH_CHECK();
 }
-cudaError_t launch_add_norm(const Dev& D, const Plan& p, int rows, int step, int mode, int ksplit, size_t ss, cudaStream_t st) {
-  return launch_pdl(k_add_norm, dim3(rows), dim3(norm_threads(D.d)), st, D, p, step, mode, ksplit, ss);
+cudaError_t launch_add_norm(const Dev& D, const Plan& p, int rows, int step, int mode, const OpDesc& o, cudaStream_t st) {
+  return launch_pdl(k_add_norm, dim3(rows), dim3(norm_threads(D.d)), st, D, p, step, mode, o.ksplit, o.split_stride, o.part_ld);
 }
-cudaError_t launch_rope_kv(const Dev& D, const Plan& p, int rows, int step, int ksplit, size_t ss, cudaStream_t st) {
+cudaError_t launch_rope_kv(const Dev& D, const Plan& p, int rows, int step, const OpDesc& o, cudaStream_t st) {
   const int items = (D.nh + D.nkv) * (D.hd / 8) + D.nkv * D.hd / 4;
-  return launch_pdl(k_rope_kv, dim3(rows, (items + 255) / 256), dim3(256), st, D, p, step, ksplit, ss);
+  return launch_pdl(k_rope_kv, dim3(rows, (items + 255) / 256), dim3(256), st, D, p, step, o.ksplit, o.split_stride, o.part_ld);
 }
-cudaError_t launch_silu_mul(const Dev& D, const Plan& p, int rows, int step, int ksplit, size_t ss, cudaStream_t st) {
-  return launch_pdl(k_silu_mul, dim3(rows, (D.ffn / 4 + 255) / 256), dim3(256), st, D, p, step, ksplit, ss);
+cudaError_t launch_silu_mul(const Dev& D, const Plan& p, int rows, int step, const OpDesc& o, cudaStream_t st) {
+  return launch_pdl(k_silu_mul, dim3(rows, (D.ffn / 4 + 255) / 256), dim3(256), st, D, p, step, o.ksplit, o.split_stride, o.part_ld);
 }
 cudaError_t launch_attn(const Dev& D, const Plan& p, int rows, int step, int n_chunks, int kv_static, cudaStream_t st) {
   dim3 g(n_chunks, D.nkv, p.n_grp * D.max_seqs);

@@ -93,7 +93,8 @@ def test_gemm_single_plane_is_bf16_rounded_input(P, c1):
     d.close()
 
 
-def test_c1_ar_hidden_logits_tokens(P, c1, c1_bf16):
+@pytest.mark.parametrize("rk", [1, 0])
+def test_c1_ar_hidden_logits_tokens(P, c1, c1_bf16, rk):
     """T3 on config c1 with X = {L} (the AR baseline): every layer's hidden state, the final
     logits and the token stream against oracle AR greedy."""
     from oracle import ar_greedy
@@ -101,7 +102,7 @@ def test_c1_ar_hidden_logits_tokens(P, c1, c1_bf16):
     T = wl.gen_len
     ar = ar_greedy(c1_bf16, p, T, keep_hidden=True, keep_logits=True)
     margins = np.array(ar["top1"]) - np.array(ar["top2"])
-    d = P.Dex(wl.shape, w, (wl.shape.n_layers,), max_ctx=128, debug_taps=1, use_graph=0)
+    d = P.Dex(wl.shape, w, (wl.shape.n_layers,), max_ctx=128, debug_taps=1, use_graph=0, round_kernel=rk)
     d.prefill(0, p)
     assert d.tap_fsm().tolist() == [0, len(p) - 1, len(p), 0]
     worst_h = worst_l = 0.0
@@ -127,9 +128,10 @@ def test_c1_ar_hidden_logits_tokens(P, c1, c1_bf16):
     d.close()
 
 
+@pytest.mark.parametrize("rk", [1, 0])
 @pytest.mark.parametrize("decs", [0, 1])
 @pytest.mark.parametrize("X", [(2, 4, 6, 8), (4, 8), (3, 8), (1, 3, 4, 8), tuple(range(1, 9))])
-def test_c1_dex_matches_oracle(P, c1, c1_bf16, decs, X):
+def test_c1_dex_matches_oracle(P, c1, c1_bf16, decs, X, rk):
     """T3/T4 on c1: DEX rounds against the oracle's Alg. 1 trace: committed tokens, selected
     branch b_k, per-round rows per stage / layer evaluations / critical layers (bit-exact),
     every new node's candidate token u and stage-boundary hidden state; and the GPU DEX stream
@@ -141,7 +143,7 @@ def test_c1_dex_matches_oracle(P, c1, c1_bf16, decs, X):
     margins = np.array(ar["top1"]) - np.array(ar["top2"])
     od = dex_decode(c1_bf16, p, T, X, decs=bool(decs), trace=True)
     assert np.array_equal(od["tokens"], ar["tokens"])            # losslessness
-    g = P.Dex(wl.shape, w, X, max_ctx=128, debug_taps=1, use_graph=0, decs=decs)
+    g = P.Dex(wl.shape, w, X, max_ctx=128, debug_taps=1, use_graph=0, decs=decs, round_kernel=rk)
     g.prefill(0, p)
     n_commit, flagged, worst_h = 0, 0, 0.0
     for ri, orec in enumerate(od["rounds"]):
@@ -155,12 +157,18 @@ def test_c1_dex_matches_oracle(P, c1, c1_bf16, decs, X):
             h = g.tap_hidden(node)
             worst_h = max(worst_h, rel_err(h[-1], orec["h_out"][node]))
             if B[node] != orec["u"][node]:
-                flagged += 1      # an intermediate exit may flip at a near-tie; the commit rule below decides
+                # an exit may flip only at a near-tie of the oracle's (masked) logits of that node (R17)
+                assert orec["u_margin"][node] < MARGIN, (ri, node, B[node], orec["u"][node], orec["u_margin"][node])
+                flagged += 1
+        if flagged:
+            # the lattices now explore different candidates: the node-by-node trace no longer applies.
+            # Finish the pending commit, if any; the stream checks below still hold.
+            if r.match_k >= 0:
+                g.collapse(0, r.match_k, r.token)
+            break
         if orec["committed"]:
             tok, k = r.token, r.match_k
-            if tok != orec["token"] or k != orec["match_k"]:
-                assert margins[n_commit] < MARGIN or flagged, (ri, tok, orec["token"], k, orec["match_k"])
-                pytest.skip("near-tie divergence; the forced-run test covers this path")
+            assert tok == orec["token"] and k == orec["match_k"], (ri, tok, orec["token"], k, orec["match_k"])
             assert abs(r.ref_top1 - orec["ref_top1"]) < LOGIT_TOL
             g.collapse(0, k, tok)
             n_commit += 1
@@ -168,24 +176,29 @@ def test_c1_dex_matches_oracle(P, c1, c1_bf16, decs, X):
         else:
             assert r.match_k == -1 and r.q_after == orec["q_after"]
     assert worst_h < HID_TOL, worst_h
-    assert flagged == 0
-    dex_tokens = g.tokens()[len(p):]
-    assert np.array_equal(dex_tokens, od["tokens"])
+    n_have = len(g.tokens()) - len(p)
+    if n_have < T:
+        g.generate(T - n_have)
+    dex_tokens = g.tokens()[len(p):len(p) + T]
+    bad = np.nonzero(dex_tokens != od["tokens"])[0]
+    if len(bad):                                                  # only a near-tie of the final-depth logits may differ
+        assert margins[bad[0]] < MARGIN, (bad[0], margins[bad[0]])
     g.close()
-    a = P.Dex(wl.shape, w, (wl.shape.n_layers,), max_ctx=128, decs=decs)
+    a = P.Dex(wl.shape, w, (wl.shape.n_layers,), max_ctx=128, decs=decs, round_kernel=rk)
     a.prefill(0, p)
     ar_gpu, _ = a.generate(T)
     a.close()
     assert np.array_equal(ar_gpu, dex_tokens)                    # H3: bit-identical streams
 
 
-def test_c1_full_run_graph_replay_and_counts(P, c1, c1_bf16):
+@pytest.mark.parametrize("rk", [1, 0])
+def test_c1_full_run_graph_replay_and_counts(P, c1, c1_bf16, rk):
     """The bench configuration of c1 (64 tokens, CUDA-graph replay, auto-collapse): tokens ==
     oracle, rounds and layer evaluations equal the closed forms of SURVEY 8(c)."""
     from oracle import dex_decode
     wl, w, p = c1
     od = dex_decode(c1_bf16, p, wl.gen_len, wl.depths, decs=True)
-    g = P.Dex(wl.shape, w, wl.depths, max_ctx=128, use_graph=1)
+    g = P.Dex(wl.shape, w, wl.depths, max_ctx=128, use_graph=1, round_kernel=rk)
     g.prefill(0, p)
     toks, recs = g.generate(wl.gen_len)
     assert np.array_equal(toks, od["tokens"])
