@@ -240,8 +240,10 @@ def bench_dex(args):
            "wall_ms_per_step": wall_ms / args.steps,
            "includes": "dex_prefill of the pinned host prompt, all rounds with per-round host results, dex_get_tokens"}
 
-    # ---- roofline of the dominant kernel (segment GEMM k_gemm): one profiled pass of the same
-    #      workload with CUDA events around every launch on the library's stream ----
+    # ---- roofline of the dominant kernel: k_round, the persistent round kernel (all layer-steps of all live
+    #      stages + the exit head of one round in one launch).  One profiled pass of the same workload with a
+    #      CUDA-event pair around every k_round launch on the library's stream (graph replay off);
+    #      algorithmic bytes = bf16 weights of the live stages + LM head + committed K/V attended.
     peak, peak_src = measured_hbm_peak()
     roofline, phases = None, None
     if rank == 0:
@@ -249,20 +251,26 @@ def bench_dex(args):
         g.profile(1)
         run_rounds(g, T, FL)
         ph, ct = g.profile(0)
-        gemm_us, gemm_launches, gemm_bytes = ph[1], ct[2], ct[3]
-        ach = gemm_bytes / (gemm_us * 1e-6) / 1e9
-        roofline = {"kernel": "k_gemm (segment projections, grouped over live stages)", "bound": "hbm",
-                    "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
+        k_us, k_launches, k_bytes = ph[1], ct[2], ct[3] + ct[4] + ct[5]
+        ach = k_bytes / (k_us * 1e-6) / 1e9
+        roofline = {"kernel": "k_round (persistent round kernel: segment GEMMs + glue + lattice attention + fused exit)",
+                    "bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
                     "frac_of_8TBs": ach / NOMINAL_HBM_GBS, "peak_source": peak_src, "traffic": None,
-                    "launches": int(gemm_launches), "avg_launch_us": gemm_us / max(1, gemm_launches),
-                    "algorithmic_bytes_per_launch": gemm_bytes / max(1, gemm_launches),
-                    "how": "profiled pass after the timed region: cudaEvent pair around each k_gemm launch on the "
-                           "library stream (graph replay and PDL overlap off), bytes = bf16 weights of the live stages"}
+                    "launches": int(k_launches), "avg_launch_us": k_us / max(1, k_launches),
+                    "algorithmic_bytes_per_launch": k_bytes / max(1, k_launches),
+                    "share_of_step": k_us / max(1e-9, ph[7] if ph[7] > 0 else sum(ph[:6])),
+                    "how": "profiled pass after the timed region: cudaEvent pair around each k_round launch on the "
+                           "library stream (graph replay off); bytes = bf16 weights of the live stages + LM head + "
+                           "committed K/V attended (dex_profile counters)"}
+        # the same rounds through the per-op kernels (round_kernel bypassed): where the time would go without k_round
+        g.rewind(0, n_prompt)
+        g.profile(2)
+        run_rounds(g, T, FL)
+        ph2, ct2 = g.profile(0)
         names = ("bookkeeping", "segment_gemm", "glue", "attention", "exit_gemm", "commit_collapse")
-        phases = {n: ph[i] / T for i, n in enumerate(names)}
-        phases["unit"] = "us per committed token (profiled pass, kernels serialised)"
-        exit_ach = ct[4] / (ph[4] * 1e-6) / 1e9 if ph[4] > 0 else None
-        phases["exit_gemm_GBs"] = exit_ach
+        phases = {n: ph2[i] / T for i, n in enumerate(names)}
+        phases["unit"] = "us per committed token, per-op kernel path (profiled pass, kernels serialised)"
+        phases["k_round_path"] = {"bookkeeping": ph[0] / T, "k_round": ph[1] / T, "commit_collapse": ph[5] / T}
 
     # whole-step roofline of the timed region (north_star: weight + KV bytes touched per step)
     step_bytes = (counters[3] + counters[4] + counters[5]) / args.steps

@@ -154,7 +154,7 @@ int32_t dex_get_tokens(dex_ctx* ctx, int32_t seq, int32_t* out, int32_t cap, int
  *                    (recomputed by a plain CUDA-core kernel from the anchor's exit row)
  *   DEX_TAP_B      : explore buffer B of `seq` -> int32[2^N - 1] (-1 = empty)
  *   DEX_TAP_FSM    : int32[4] = {q, ctx_len, n_tokens, pending}
- *   DEX_TAP_ROUND_TIMES : uint64[18 * max_m|Pi_m| + 4] SM clock-cycle stamps taken by CTA 0 of
+ *   DEX_TAP_ROUND_TIMES : uint64[20 * max_m|Pi_m| + 4] SM clock-cycle stamps taken by CTA 0 of
  *                    the last round kernel: start, then after every item phase and grid barrier */
 #define DEX_TAP_HIDDEN 1
 #define DEX_TAP_LOGITS 2

@@ -236,7 +236,7 @@ class Dex:
         return dex_debug_read(self.ctx, DEX_TAP_FSM, seq, 0, np.zeros(4, dtype=np.int32))
 
     def tap_round_times(self):
-        n = 18 * max(b - a for a, b in zip((0,) + self.depths[:-1], self.depths)) + 4
+        n = 20 * max(b - a for a, b in zip((0,) + self.depths[:-1], self.depths)) + 68
         return dex_debug_read(self.ctx, DEX_TAP_ROUND_TIMES, 0, 0, np.zeros(n, dtype=np.uint64))
 
     def gemm(self, which, layer, x):

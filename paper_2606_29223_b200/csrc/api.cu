@@ -4,7 +4,6 @@
 #include <algorithm>
 #include <cstdarg>
 #include <cstdio>
-#include <cstdlib>
 #include <cstring>
 #include <map>
 #include <memory>
@@ -25,6 +24,7 @@ cudaError_t launch_add_norm(const Dev&, const Plan&, int, int, int, const OpDesc
 cudaError_t launch_rope_kv(const Dev&, const Plan&, int, int, const OpDesc&, cudaStream_t);
 cudaError_t launch_silu_mul(const Dev&, const Plan&, int, int, const OpDesc&, cudaStream_t);
 cudaError_t round_init();
+size_t round_attn_smem(int);
 cudaError_t launch_round(const TmSet&, const RoundArgs&, int, size_t, cudaStream_t);
 cudaError_t launch_attn(const Dev&, const Plan&, int, int, int, int, cudaStream_t);
 cudaError_t launch_decide(const Dev&, const Plan&, int, cudaStream_t);
@@ -79,6 +79,7 @@ struct dex_ctx {
   size_t dbg_floats;
   TmSet tms;
   RingCfg round_ring;
+  int round_attn_off;
   std::map<long long, cudaGraphExec_t> graphs;
   std::string err;
   // phase timing (taps only)
@@ -168,7 +169,7 @@ struct Layout {
   size_t dbg_floats;
 };
 enum Buf {
-  B_SEQS, B_TOKENS, B_B, B_PT, B_ROWS, B_GNB, B_ENB, B_KEY, B_REFT, B_CMD, B_KPOOL, B_VPOOL, B_KSLOT, B_VSLOT,
+  B_SEQS, B_TOKENS, B_B, B_PT, B_ROWS, B_GNB, B_ENB, B_KEY, B_REFT, B_CMD, B_SS, B_ACNT, B_KPOOL, B_VPOOL, B_KSLOT, B_VSLOT,
   B_XCUR, B_XFRONT, B_ACTA, B_ACTO, B_ACTF, B_ACTE, B_PART, B_QBUF, B_APART, B_ROPE, B_TAPH, B_DBG, B_GBAR, B_TAPT, B_COUNT
 };
 
@@ -236,6 +237,8 @@ void make_layout(const dex_config& c, const int32_t* depths, int n, Layout& L) {
   sz[B_KEY] = sizeof(unsigned long long) * R;
   sz[B_REFT] = sizeof(float2) * (size_t)c.max_seqs * L.ref_tiles;
   sz[B_CMD] = sizeof(CollapseCmd) * c.max_seqs;
+  sz[B_SS] = sizeof(float) * R * kSsSeg;
+  sz[B_ACNT] = sizeof(int) * R * c.n_heads;
   sz[B_KPOOL] = kv_pool;
   sz[B_VPOOL] = kv_pool;
   sz[B_KSLOT] = kv_slot;
@@ -253,7 +256,7 @@ void make_layout(const dex_config& c, const int32_t* depths, int n, Layout& L) {
   sz[B_TAPH] = c.debug_taps ? sizeof(float) * R * (size_t)L.max_len * c.d_model : 0;
   sz[B_DBG] = sizeof(float) * L.dbg_floats;
   sz[B_GBAR] = 256;
-  sz[B_TAPT] = c.debug_taps ? sizeof(unsigned long long) * (18 * (size_t)L.max_len + 4) : 0;
+  sz[B_TAPT] = c.debug_taps ? sizeof(unsigned long long) * (20 * (size_t)L.max_len + 68) : 0;
   size_t off = 0;
   for (int i = 0; i < B_COUNT; ++i) {
     L.off[i] = off;
@@ -397,11 +400,10 @@ int enqueue_round(dex_ctx* c, int n_chunks) {
   for (int i = 0; i < 5; ++i) a.op[i] = c->op[i].dec;
   a.x_cap = c->round_ring.x_cap;
   a.n_stages = c->round_ring.n_stages;
-  { const char* e = getenv("DEX_STAGES"); if (e) a.n_stages = std::min(a.n_stages, atoi(e)); }
   a.acc_cols = c->round_ring.acc_cols;
   a.stacked = c->round_ring.stacked;
   a.n_chunks = n_chunks;
-  { const char* e = getenv("DEX_DBG"); a.dbg = e ? atoi(e) : 0; }
+  a.attn_smem_off = c->round_attn_off;
   ph_begin(c, PH_GEMM);
   CU(c, launch_round(c->tms, a, c->n_sms, c->round_ring.smem, c->stream));
   ph_end(c, PH_GEMM);
@@ -583,6 +585,7 @@ int32_t dex_init(dex_ctx** out, const dex_config* cfg, const dex_weights* w, con
   D.seqs = WSP(SeqState, B_SEQS); D.tokens = WSP(int, B_TOKENS); D.B = WSP(int, B_B); D.page_table = WSP(int, B_PT);
   D.rows = WSP(RowInfo, B_ROWS); D.grp_nb = WSP(int, B_GNB); D.exit_nb = WSP(int, B_ENB);
   D.best_key = WSP(unsigned long long, B_KEY); D.ref_tile = WSP(float2, B_REFT); D.cmd = WSP(CollapseCmd, B_CMD);
+  D.ss_part = WSP(float, B_SS); D.attn_cnt = WSP(int, B_ACNT);
   D.kpool = WSP(__nv_bfloat16, B_KPOOL); D.vpool = WSP(__nv_bfloat16, B_VPOOL);
   D.kslot = WSP(__nv_bfloat16, B_KSLOT); D.vslot = WSP(__nv_bfloat16, B_VSLOT);
   D.x_cur = WSP(float, B_XCUR); D.x_front = WSP(float, B_XFRONT);
@@ -604,6 +607,13 @@ int32_t dex_init(dex_ctx** out, const dex_config* cfg, const dex_weights* w, con
     both.n_grp = 1;
     both.rows_cap[0] = std::max(c->dec_ring.x_cap, c->exit_ring.x_cap);
     c->round_ring = make_ring(both, cfg->act_planes);
+    // the round kernel also carves its attention scratch out of dynamic shared memory: fewer ring stages
+    const size_t stage = 16384 + (size_t)cfg->act_planes * c->round_ring.x_cap * 128;
+    const size_t attn = (round_attn_smem(cfg->head_dim) + 1023) / 1024 * 1024;
+    const size_t budget = 222 * 1024 - attn - 2048;
+    c->round_ring.n_stages = (int)std::max<size_t>(2, std::min<size_t>(12, budget / stage));
+    c->round_attn_off = (int)((c->round_ring.n_stages * stage + 1023 + 512) / 1024 * 1024);
+    c->round_ring.smem = c->round_attn_off + attn + 1024;
   }
 
 #define INIT_FAIL(expr)          \
@@ -643,11 +653,6 @@ int32_t dex_init(dex_ctx** out, const dex_config* cfg, const dex_weights* w, con
   for (int i = 0; i < 4; ++i)
     INIT_FAIL(encode_3d(c, enc, &c->tmX[i], xptr[i], xk[i], D.R_cap, cfg->act_planes, kBoxRows, all_stacked ? 2 : 1));
   for (int i = 0; i < 5; ++i) c->tms.w[i] = c->op[i].tmW;
-  for (int i = 0; i < 5; ++i) {
-    const OpDesc& o = c->op[i].dec;
-    const uint64_t n_t = (uint64_t)(i == 4 ? 1 : D.L) * o.out_dim * o.k_dim / (kTileM * kTileK);
-    INIT_FAIL(encode_3d(c, enc, &c->tms.wt[i], wptr[i], kTileK, kTileM, n_t, kTileM));
-  }
   for (int i = 0; i < 4; ++i) c->tms.x[i] = c->tmX[i];
 
   // state: FSM zeroed, free pages, result buffer, RoPE table
@@ -862,7 +867,7 @@ int32_t dex_debug_read(dex_ctx* c, int32_t what, int32_t seq, int32_t a, void* d
     return DEX_OK;
   }
   if (what == DEX_TAP_ROUND_TIMES) {
-    const size_t bytes = sizeof(unsigned long long) * (18 * (size_t)D.max_len + 4);
+    const size_t bytes = sizeof(unsigned long long) * (20 * (size_t)D.max_len + 68);
     if (dst_bytes < bytes) return fail(c, DEX_EINVAL, "dst too small");
     CU(c, cudaMemcpyAsync(dst, D.tap_times, bytes, cudaMemcpyDeviceToHost, c->stream));
     CU(c, cudaStreamSynchronize(c->stream));

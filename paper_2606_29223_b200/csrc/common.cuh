@@ -16,6 +16,7 @@ constexpr int kTileM = 128;         // GEMM: weight rows (out features) per MMA 
 constexpr int kTileK = 64;          // GEMM: bf16 K elements per pipeline stage (128 B rows, SW128)
 constexpr int kBoxRows = 16;        // activation rows per TMA box
 constexpr int kPrefillRows = 128;   // rows per prefill chunk
+constexpr int kSsSeg = 16;          // sum-of-squares segments per row (512 elements each, d <= 8192)
 
 // A "plan" = groups of stacked rows, each streaming its own layer segment.  Decode: group m =
 // explorer E_m with stage Pi_m = Layers(d_{m-1}, d_m].  Prefill: one group
@@ -93,6 +94,10 @@ struct Dev {
   __nv_bfloat16 *kslot, *vslot;   // [max_seqs][n_slots][L][nkv][hd]
   float* x_cur;            // [R_cap][d] residual stream of this round's rows
   float* x_front;          // [R_cap][d] frontier hidden (h_out of the previous level)
+  float* ss_part;          // [R_cap][kSsSeg] sum of squares of the row the last norm was taken of, per 512-element
+                           // segment.  The RMSNorm scale is DEFERRED: operand planes hold x*w, consumers of the GEMM
+                           // output multiply by inv_rms(row) = rsqrt(sum_seg ss / d + eps) (exact: the scale is per row)
+  int* attn_cnt;           // [R_cap][nh] chunk partials written (last writer merges them)
   RowInfo* rows;           // [R_cap]
   int* grp_nb;             // [kMaxGrp] live row extent per decode/prefill group (multiple of 16)
   int* exit_nb;            // [kMaxGrp] live row extent per exit chunk
@@ -109,7 +114,7 @@ struct Dev {
   CollapseCmd* cmd;        // [max_seqs]
   dex_step_result* result_dev;    // [max_seqs] (mapped pinned host memory)
   float* tap_hidden;       // [R_cap][max_len][d] (taps only)
-  unsigned long long* tap_times;  // [18 * max_len + 4] globaltimer stamps of CTA 0 in k_round (taps only)
+  unsigned long long* tap_times;  // [20 * max_len + 4] globaltimer stamps of CTA 0 in k_round (taps only)
   int n_pages;
 };
 
@@ -133,6 +138,14 @@ __device__ __forceinline__ uint32_t f2key(float f) {
 __device__ __forceinline__ float key2f(uint32_t k) {
   uint32_t u = (k & 0x80000000u) ? (k & 0x7FFFFFFFu) : ~k;
   return __uint_as_float(u);
+}
+
+__device__ __forceinline__ float inv_rms(const Dev& D, int r) {
+  const float* p = D.ss_part + (size_t)r * kSsSeg;
+  float ss = 0.f;
+#pragma unroll
+  for (int i = 0; i < kSsSeg; ++i) ss += p[i];          // fixed order (unused segments hold 0)
+  return 1.0f / sqrtf(ss / (float)D.d + D.eps);
 }
 
 // fp32 -> bf16 hi (+ lo residual) planes.
@@ -203,7 +216,6 @@ struct OpDesc {
 struct TmSet {             // TMA descriptors of the round kernel: weights qkv,o,gu,dn,lm_head; operands a,o,f,e
   CUtensorMap w[5];
   CUtensorMap x[4];
-  CUtensorMap wt[5];       // timing experiment: the same bytes viewed as contiguous 16 KiB tiles
 };
 
 struct RoundArgs {
@@ -212,7 +224,7 @@ struct RoundArgs {
   OpDesc op[5];
   int x_cap, n_stages, acc_cols, stacked;   // shared-memory ring / TMEM geometry
   int n_chunks;                    // attention chunks that can hold a live position (host upper bound)
-  int dbg;                         // timing experiments only (env DEX_DBG): 1 skip glue math, 2 skip barriers
+  int attn_smem_off;               // byte offset of the attention scratch (AttnSmem) in dynamic shared memory
 };
 
 }  // namespace dexk

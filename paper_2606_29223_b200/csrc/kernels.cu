@@ -245,7 +245,7 @@ __global__ void __launch_bounds__(1024) k_gather_norm(Dev D, Plan plan) {
     }
   }
   ss = block_sum(ss, red);
-  const float inv = 1.0f / sqrtf(ss / (float)D.d + D.eps);
+  if (threadIdx.x < kSsSeg) D.ss_part[(size_t)r * kSsSeg + threadIdx.x] = threadIdx.x == 0 ? ss : 0.f;   // deferred scale
   const float* w = D.norm_attn + (size_t)plan.layer_lo[ri.grp] * D.d;
   const size_t ps = (size_t)D.R_cap * D.d;
 #pragma unroll
@@ -254,7 +254,7 @@ __global__ void __launch_bounds__(1024) k_gather_norm(Dev D, Plan plan) {
     if (i < nv) {
       const float4 wv = ld4(w + 4 * i), v = xv[it];
       split_store4(D.act_a, ps, (size_t)r * D.d + 4 * i,
-                   make_float4(v.x * inv * wv.x, v.y * inv * wv.y, v.z * inv * wv.z, v.w * inv * wv.w), D.planes);
+                   make_float4(v.x * wv.x, v.y * wv.y, v.z * wv.z, v.w * wv.w), D.planes);
     }
   }
 }
@@ -290,7 +290,7 @@ __global__ void __launch_bounds__(1024) k_add_norm(Dev D, Plan plan, int step, i
     }
   }
   ss = block_sum(ss, red);
-  const float inv = 1.0f / sqrtf(ss / (float)D.d + D.eps);
+  if (threadIdx.x < kSsSeg) D.ss_part[(size_t)r * kSsSeg + threadIdx.x] = threadIdx.x == 0 ? ss : 0.f;   // deferred scale
   const float* w;
   __nv_bfloat16* dst = D.act_a;
   if (mode == 0) {
@@ -308,7 +308,7 @@ __global__ void __launch_bounds__(1024) k_add_norm(Dev D, Plan plan, int step, i
     if (i < nv) {
       const float4 wv = ld4(w + 4 * i), v = xv[it];
       split_store4(dst, ps, (size_t)r * D.d + 4 * i,
-                   make_float4(v.x * inv * wv.x, v.y * inv * wv.y, v.z * inv * wv.z, v.w * inv * wv.w), D.planes);
+                   make_float4(v.x * wv.x, v.y * wv.y, v.z * wv.z, v.w * wv.w), D.planes);
     }
   }
 }
@@ -332,12 +332,15 @@ __global__ void __launch_bounds__(256) k_rope_kv(Dev D, Plan plan, int step, int
   const int n_rot = (D.nh + D.nkv) * qd;                 // rotated float4 pair groups
   const int n_v = nk / 4;
   pdl_wait();
+  const float inv = inv_rms(D, r);                       // deferred RMSNorm scale of the QKV input
   for (int t = blockIdx.y * blockDim.x + threadIdx.x; t < n_rot + n_v; t += gridDim.y * blockDim.x) {
     if (t < n_rot) {
       const int h = t / qd, i = (t % qd) * 4;
       const int i1 = h * hd + i, i2 = i1 + half;
-      const float4 a = sum_splits4(p + i1, ksplit, split_stride);
-      const float4 b = sum_splits4(p + i2, ksplit, split_stride);
+      float4 a = sum_splits4(p + i1, ksplit, split_stride);
+      float4 b = sum_splits4(p + i2, ksplit, split_stride);
+      a.x *= inv; a.y *= inv; a.z *= inv; a.w *= inv;
+      b.x *= inv; b.y *= inv; b.z *= inv; b.w *= inv;
       const float2 c0 = rt[i], c1 = rt[i + 1], c2 = rt[i + 2], c3 = rt[i + 3];
       const float4 o1 = make_float4(a.x * c0.x - b.x * c0.y, a.y * c1.x - b.y * c1.y, a.z * c2.x - b.z * c2.y, a.w * c3.x - b.w * c3.y);
       const float4 o2 = make_float4(b.x * c0.x + a.x * c0.y, b.y * c1.x + a.y * c1.y, b.z * c2.x + a.z * c2.y, b.w * c3.x + a.w * c3.y);
@@ -355,8 +358,8 @@ __global__ void __launch_bounds__(256) k_rope_kv(Dev D, Plan plan, int step, int
     } else {
       const int i = (t - n_rot) * 4;
       const float4 a = sum_splits4(p + nq + nk + i, ksplit, split_stride);
-      *reinterpret_cast<__nv_bfloat162*>(vd + i) = __floats2bfloat162_rn(a.x, a.y);
-      *reinterpret_cast<__nv_bfloat162*>(vd + i + 2) = __floats2bfloat162_rn(a.z, a.w);
+      *reinterpret_cast<__nv_bfloat162*>(vd + i) = __floats2bfloat162_rn(a.x * inv, a.y * inv);
+      *reinterpret_cast<__nv_bfloat162*>(vd + i + 2) = __floats2bfloat162_rn(a.z * inv, a.w * inv);
     }
   }
 }
@@ -370,9 +373,12 @@ __global__ void __launch_bounds__(256) k_silu_mul(Dev D, Plan plan, int step, in
   const float* p = D.part + (size_t)r * ld;
   const size_t ps = (size_t)D.R_cap * D.ffn;
   pdl_wait();
+  const float inv = inv_rms(D, r);                       // deferred RMSNorm scale of the gate/up input
   for (int i = (blockIdx.y * blockDim.x + threadIdx.x) * 4; i < D.ffn; i += gridDim.y * blockDim.x * 4) {
-    const float4 g = sum_splits4(p + i, ksplit, split_stride);
-    const float4 u = sum_splits4(p + D.ffn + i, ksplit, split_stride);
+    float4 g = sum_splits4(p + i, ksplit, split_stride);
+    float4 u = sum_splits4(p + D.ffn + i, ksplit, split_stride);
+    g.x *= inv; g.y *= inv; g.z *= inv; g.w *= inv;
+    u.x *= inv; u.y *= inv; u.z *= inv; u.w *= inv;
     float4 a;
     a.x = g.x / (1.0f + expf(-g.x)) * u.x;
     a.y = g.y / (1.0f + expf(-g.y)) * u.y;
@@ -600,6 +606,10 @@ __global__ void k_decide(Dev D, Plan plan, int auto_collapse) {
       t2 = fmaxf(lo, fmaxf(t2, a2));
       t1 = hi;
     }
+    // the exit head saw x*w_final: apply the deferred RMSNorm scale of the anchor row
+    const float inv = inv_rms(D, plan.row_base[N - 1] + s * cap_of(N, N - 1));
+    t1 *= inv;
+    t2 *= inv;
   }
   if (lane != 0) return;
   res->active = 1;
@@ -794,7 +804,7 @@ __global__ void k_tap_logits(Dev D, int row, float* out) {
     acc = fmaf(x, __bfloat162float(w[i]), acc);
   }
   acc = warp_sum(acc);
-  if (lane == 0) out[v] = acc;
+  if (lane == 0) out[v] = acc * inv_rms(D, row);
 }
 
 __global__ void k_debug_rows(Dev D, int R) {

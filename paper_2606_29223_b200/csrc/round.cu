@@ -50,13 +50,13 @@ __device__ __forceinline__ float4 r_ld4(const float* p) { return *reinterpret_ca
 __device__ __forceinline__ float4 r_add4(float4 a, float4 b) { return make_float4(a.x + b.x, a.y + b.y, a.z + b.z, a.w + b.w); }
 __device__ __forceinline__ float4 r_sum4(const float* p, int S, size_t stride) {
   float4 acc = r_ld4(p);
-#pragma unroll 4
+#pragma unroll 8
   for (int s = 1; s < S; ++s) acc = r_add4(acc, r_ld4(p + (size_t)s * stride));
   return acc;
 }
 __device__ __forceinline__ float r_sum1(const float* p, int S, size_t stride) {
   float acc = p[0];
-#pragma unroll 4
+#pragma unroll 8
   for (int s = 1; s < S; ++s) acc += p[(size_t)s * stride];
   return acc;
 }
@@ -123,11 +123,12 @@ struct Seq {               // shared by all roles: same deterministic walk
     it.row0 = p.row_base[it.g];
     it.row_end = it.row0 + p.rows_cap[it.g];
   }
-  // grid barriers that must have completed before op t's operand may be read (9 per step)
+  // grid barriers that must have completed before op t's operand may be read (9 per step: one after
+  // every GEMM's epilogue, one after every glue phase; the QKV output takes two glue phases)
   __device__ __forceinline__ unsigned dep(int t) const {
     if (t >= 4 * n_steps) return 9u * n_steps;
     const int k = t & 3;
-    return 9u * (t >> 2) + (k == 0 ? 0u : (k == 1 ? 3u : (k == 2 ? 5u : 7u)));
+    return 9u * (t >> 2) + (k == 0 ? 0u : 2u * k + 1u);
   }
 };
 
@@ -161,8 +162,7 @@ struct Walker {            // this CTA's items, in order
 };
 
 // ---------------------------------------------------------------- grid barrier (epilogue groups)
-__device__ __forceinline__ void grid_bar(unsigned* gbar, unsigned target, int tid_e, volatile unsigned* s_seen, unsigned gb, int dbg = 0) {
-  if (dbg & 2) return;
+__device__ __forceinline__ void grid_bar(unsigned* gbar, unsigned target, int tid_e, volatile unsigned* s_seen, unsigned gb) {
   __threadfence();
   fence_proxy_async();           // generic-proxy writes (operand planes) -> later TMA reads
   bar_epi();
@@ -193,63 +193,68 @@ __device__ __forceinline__ float group_sum(float v, float* red /*[4]*/, int tid_
   return (red[0] + red[1]) + (red[2] + red[3]);
 }
 
-// x += sum_s part[s]; RMSNorm -> operand planes.  mode 0: after o_proj (w = norm_ffn[l] -> act_a);
-// mode 1: after down_proj (next layer's attention norm -> act_a, or the shared final norm -> act_e).
+// Every glue phase is laid out for memory-level parallelism: a thread issues all of its loads in one or two
+// batches (a dependent load under the weight stream costs microseconds), and the work is spread over all CTAs.
+
+// x += sum_s part[s]; operand planes <- x * w (RMSNorm scale deferred: Dev::ss_part).  Unit = (row, 512-element
+// segment), one per CTA pass.  mode 0: after o_proj (w = norm_ffn[l] -> act_a); mode 1: after down_proj (next
+// layer's attention norm -> act_a, or the shared final norm -> act_e).
 __device__ void glue_add_norm(const RoundArgs& a, int j, int mode, const OpDesc& op, float* red, int tid_e, int cta, int G) {
   const Dev& D = a.D;
-  const int nv = D.d >> 2;
-  for (int r = cta; r < D.R_dec; r += G) {
+  const int n_seg = (D.d + 511) / 512;
+  for (int u = cta; u < D.R_dec * n_seg; u += G) {
+    const int r = u / n_seg, seg = u - r * n_seg;
     const RowInfo* ri = &D.rows[r];
     if (!ri->valid) continue;
     const int grp = ri->grp;
     if (j >= a.dec.layer_len[grp]) continue;
     const int layer = a.dec.layer_lo[grp] + j;
-    float* x = D.x_cur + (size_t)r * D.d;
-    const float* p = D.part + (size_t)r * op.part_ld;
+    const int i = seg * 512 + tid_e * 4;
     float ss = 0.f;
-    for (int i = tid_e; i < nv; i += kEpiThreads) {
-      const float4 s4 = r_sum4(p + 4 * i, op.ksplit, op.split_stride);
-      const float4 v = r_add4(r_ld4(x + 4 * i), s4);
-      *reinterpret_cast<float4*>(x + 4 * i) = v;
-      ss += v.x * v.x + v.y * v.y + v.z * v.z + v.w * v.w;
-      if (mode == 1 && D.taps) *reinterpret_cast<float4*>(D.tap_hidden + ((size_t)r * D.max_len + j) * D.d + 4 * i) = v;
+    if (i < D.d) {
+      const float* w;
+      __nv_bfloat16* dst = D.act_a;
+      if (mode == 0) {
+        w = D.norm_ffn + (size_t)layer * D.d;
+      } else if (j + 1 < a.dec.layer_len[grp]) {
+        w = D.norm_attn + (size_t)(layer + 1) * D.d;
+      } else {
+        w = D.norm_final;
+        dst = D.act_e;
+      }
+      float* x = D.x_cur + (size_t)r * D.d + i;
+      const float4 xv = r_ld4(x), wv = r_ld4(w + i);
+      const float4 s4 = r_sum4(D.part + (size_t)r * op.part_ld + i, op.ksplit, op.split_stride);
+      const float4 v = r_add4(xv, s4);
+      *reinterpret_cast<float4*>(x) = v;
+      ss = v.x * v.x + v.y * v.y + v.z * v.z + v.w * v.w;
+      if (mode == 1 && D.taps) *reinterpret_cast<float4*>(D.tap_hidden + ((size_t)r * D.max_len + j) * D.d + i) = v;
+      r_split_store4(dst, (size_t)D.R_cap * D.d, (size_t)r * D.d + i, make_float4(v.x * wv.x, v.y * wv.y, v.z * wv.z, v.w * wv.w),
+                     D.planes);
     }
     ss = group_sum(ss, red, tid_e);
-    const float inv = 1.0f / sqrtf(ss / (float)D.d + D.eps);
-    const float* w;
-    __nv_bfloat16* dst = D.act_a;
-    if (mode == 0) {
-      w = D.norm_ffn + (size_t)layer * D.d;
-    } else if (j + 1 < a.dec.layer_len[grp]) {
-      w = D.norm_attn + (size_t)(layer + 1) * D.d;
-    } else {
-      w = D.norm_final;
-      dst = D.act_e;
-    }
-    const size_t ps = (size_t)D.R_cap * D.d;
-    for (int i = tid_e; i < nv; i += kEpiThreads) {
-      const float4 v = r_ld4(x + 4 * i), wv = r_ld4(w + 4 * i);   // own writes of the loop above
-      r_split_store4(dst, ps, (size_t)r * D.d + 4 * i,
-                     make_float4(v.x * inv * wv.x, v.y * inv * wv.y, v.z * inv * wv.z, v.w * inv * wv.w), D.planes);
-    }
+    if (tid_e == 0) D.ss_part[(size_t)r * kSsSeg + seg] = ss;
   }
 }
 
-// act_f = SiLU(gate) * up from the split-K partials of the fused gate/up projection.
-__device__ void glue_silu(const RoundArgs& a, int j, const OpDesc& op, int tid_e, int cta, int G) {
+// act_f = SiLU(gate) * up from the split-K partials of the fused gate/up projection (scaled by the deferred
+// RMSNorm factor of the row).  Warp unit = (row, 128 elements).
+__device__ void glue_silu(const RoundArgs& a, int j, const OpDesc& op, int gw, int n_gw, int lane) {
   const Dev& D = a.D;
-  const int blk = kEpiThreads * 4;
-  const int nblk = (D.ffn + blk - 1) / blk;
+  const int nblk = (D.ffn + 127) / 128;
   const size_t ps = (size_t)D.R_cap * D.ffn;
-  for (int u = cta; u < D.R_dec * nblk; u += G) {
+  for (int u = gw; u < D.R_dec * nblk; u += n_gw) {
     const int r = u / nblk, b = u - r * nblk;
     const RowInfo* ri = &D.rows[r];
     if (!ri->valid || j >= a.dec.layer_len[ri->grp]) continue;
-    const int i = b * blk + tid_e * 4;
+    const int i = b * 128 + lane * 4;
     if (i >= D.ffn) continue;
     const float* p = D.part + (size_t)r * op.part_ld;
-    const float4 g = r_sum4(p + i, op.ksplit, op.split_stride);
-    const float4 up = r_sum4(p + D.ffn + i, op.ksplit, op.split_stride);
+    const float inv = inv_rms(D, r);
+    float4 g = r_sum4(p + i, op.ksplit, op.split_stride);
+    float4 up = r_sum4(p + D.ffn + i, op.ksplit, op.split_stride);
+    g.x *= inv; g.y *= inv; g.z *= inv; g.w *= inv;
+    up.x *= inv; up.y *= inv; up.z *= inv; up.w *= inv;
     float4 o;
     o.x = g.x / (1.0f + expf(-g.x)) * up.x;
     o.y = g.y / (1.0f + expf(-g.y)) * up.y;
@@ -259,45 +264,7 @@ __device__ void glue_silu(const RoundArgs& a, int j, const OpDesc& op, int tid_e
   }
 }
 
-// Merge the per-chunk attention partials in ascending chunk order -> act_o planes.  Warp per (row, head).
-template <int HD>
-__device__ void glue_combine(const RoundArgs& a, int j, int gw, int n_gw, int lane) {
-  const Dev& D = a.D;
-  constexpr int DPL = HD / 32;
-  const int K = D.nh * HD;
-  for (int u = gw; u < D.R_dec * D.nh; u += n_gw) {
-    const int r = u / D.nh, h = u - r * D.nh;
-    const RowInfo* ri = &D.rows[r];
-    if (!ri->valid || j >= a.dec.layer_len[ri->grp]) continue;
-    const int nc = ri->pos / kChunk + 1;
-    const float* src = D.attn_part + ((size_t)r * D.nh + h) * D.max_chunks * (HD + 2);
-    float M = -INFINITY;
-    for (int c = 0; c < nc; ++c) M = fmaxf(M, src[(size_t)c * (HD + 2) + HD]);
-    float num[DPL], den = 0.f;
-#pragma unroll
-    for (int t = 0; t < DPL; ++t) num[t] = 0.f;
-    for (int c = 0; c < nc; ++c) {
-      const float* sc = src + (size_t)c * (HD + 2);
-      const float w = expf(sc[HD] - M);
-#pragma unroll
-      for (int t = 0; t < DPL; ++t) num[t] = fmaf(w, sc[lane * DPL + t], num[t]);
-      den = fmaf(w, sc[HD + 1], den);
-    }
-    const size_t ps = (size_t)D.R_cap * K;
-    const size_t idx = (size_t)r * K + h * HD + lane * DPL;
-#pragma unroll
-    for (int t = 0; t < DPL; ++t) {
-      const float v = num[t] / den;
-      const __nv_bfloat16 hi = __float2bfloat16_rn(v);
-      D.act_o[idx + t] = hi;
-      if (D.planes > 1) D.act_o[ps + idx + t] = __float2bfloat16_rn(v - __bfloat162float(hi));
-    }
-  }
-}
-
-// 16 consecutive bf16 (two 16-byte loads) -> fp32
-__device__ __forceinline__ void ld_bf16x16(const __nv_bfloat16* p, float (&f)[16]) {
-  const uint4 u0 = *reinterpret_cast<const uint4*>(p), u1 = *reinterpret_cast<const uint4*>(p + 8);
+__device__ __forceinline__ void cvt_bf16x16(const uint4& u0, const uint4& u1, float (&f)[16]) {
   const __nv_bfloat162* a = reinterpret_cast<const __nv_bfloat162*>(&u0);
   const __nv_bfloat162* b = reinterpret_cast<const __nv_bfloat162*>(&u1);
 #pragma unroll
@@ -307,223 +274,349 @@ __device__ __forceinline__ void ld_bf16x16(const __nv_bfloat16* p, float (&f)[16
     f[8 + 2 * i] = y.x; f[8 + 2 * i + 1] = y.y;
   }
 }
+__device__ __forceinline__ float bf16_rt(float v) { return __bfloat162float(__float2bfloat16_rn(v)); }
 
-// a3: one warp = one unit (stage m, sequence s, KV head g, 64-position chunk c of ABSOLUTE position).
-// The warp first finishes K/V of the rows whose own position lies in the chunk (split-K sum, RoPE,
-// bf16 store into the row's slot), then attends up to 4 (row, query head) pairs at a time: LP lanes
-// share a position (16 dims each), 32/LP positions per pass, so the committed K/V of the chunk is
-// loaded once for the 4 pairs.  Positions >= n_paged are the row's private suffix (ancestor slots,
-// own slot) and are fetched per pair.  fp32 scores, warp-shuffle softmax, per-chunk (o, max, sum).
+// Merge the per-chunk partials of (row, head) in ascending chunk order (fixed order: H3) -> act_o planes.
+// Blocks of 16 chunks are loaded in one batch (a dependent load costs microseconds under the weight stream).
 template <int HD>
-__device__ void attn_unit(const RoundArgs& a, int j, int m, int s, int g, int c, int lane, const OpDesc& op) {
-  constexpr int LP = HD / 16, PI = 32 / LP, NIT = kChunk / PI, HALF = HD / 2;
-  constexpr int PB = (HD == 128) ? 2 : 4;                   // (row, head) pairs per pass (register budget)
-  const Dev& D = a.D;
-  const SeqState st = D.seqs[s];
-  if (!r_seq_live(st) || st.q < m || j >= a.dec.layer_len[m]) return;
-  const int c0 = c * kChunk;
-  if (c0 > st.ctx_len + st.q) return;                       // beyond every row's position
-  const int cnt = r_stage_count(st.q, m);
-  const int layer = a.dec.layer_lo[m] + j;
-  const int r0 = a.dec.row_base[m] + s * cap_of(D.N, m);
-  const int n_paged = st.ctx_len;
-  const int G = D.nh / D.nkv;
-  const int nq = D.nh * HD, nk = D.nkv * HD;
-  const int sub = lane % LP, pg = lane / LP;
-  const int S = op.ksplit;
-  const size_t sst = op.split_stride;
-
-  // (1) own K/V of rows positioned in this chunk
-  for (int jr = 0; jr < cnt; ++jr) {
-    const RowInfo* ri = &D.rows[r0 + jr];
-    const int pos = ri->pos;
-    if (pos < c0 || pos >= c0 + kChunk) continue;
-    const float* p = D.part + (size_t)(r0 + jr) * op.part_ld;
-    const float2* rt = D.rope + (size_t)pos * HALF;
-    const size_t kvo = slot_off(D, s, ri->slot, layer) + (size_t)g * HD;
-    __nv_bfloat16* kd = D.kslot + kvo;
-    __nv_bfloat16* vd = D.vslot + kvo;
-    for (int e = lane; e < HALF; e += 32) {
-      const float x1 = r_sum1(p + nq + g * HD + e, S, sst), x2 = r_sum1(p + nq + g * HD + e + HALF, S, sst);
-      const float2 cs = rt[e];
-      kd[e] = __float2bfloat16_rn(x1 * cs.x - x2 * cs.y);
-      kd[e + HALF] = __float2bfloat16_rn(x2 * cs.x + x1 * cs.y);
-    }
-    for (int e = lane; e < HD; e += 32) vd[e] = __float2bfloat16_rn(r_sum1(p + nq + nk + g * HD + e, S, sst));
+__device__ __forceinline__ void attn_merge(const Dev& D, int r, int h, int nc, int lane) {
+  constexpr int DPL = HD / 32;
+  const float* src = D.attn_part + ((size_t)r * D.nh + h) * D.max_chunks * (HD + 2);
+  float M = -INFINITY;
+  for (int cb = 0; cb < nc; cb += 16) {
+    float mv[16];
+#pragma unroll
+    for (int i = 0; i < 16; ++i) mv[i] = (cb + i < nc) ? __ldcg(src + (size_t)(cb + i) * (HD + 2) + HD) : -INFINITY;
+#pragma unroll
+    for (int i = 0; i < 16; ++i) M = fmaxf(M, mv[i]);
   }
-  __syncwarp();
+  float num[DPL], den = 0.f;
+#pragma unroll
+  for (int t = 0; t < DPL; ++t) num[t] = 0.f;
+  for (int cb = 0; cb < nc; cb += 16) {
+    float mv[16], lv[16], ov[16][DPL];
+#pragma unroll
+    for (int i = 0; i < 16; ++i) {
+      const bool on = cb + i < nc;
+      const float* sc = src + (size_t)(cb + i) * (HD + 2);
+      mv[i] = on ? __ldcg(sc + HD) : -INFINITY;
+      lv[i] = on ? __ldcg(sc + HD + 1) : 0.f;
+#pragma unroll
+      for (int t = 0; t < DPL; ++t) ov[i][t] = on ? __ldcg(sc + lane * DPL + t) : 0.f;
+    }
+#pragma unroll
+    for (int i = 0; i < 16; ++i) {
+      if (cb + i < nc) {
+        const float w = expf(mv[i] - M);
+#pragma unroll
+        for (int t = 0; t < DPL; ++t) num[t] = fmaf(w, ov[i][t], num[t]);
+        den = fmaf(w, lv[i], den);
+      }
+    }
+  }
+  const int K = D.nh * HD;
+  const size_t ps = (size_t)D.R_cap * K;
+  const size_t idx = (size_t)r * K + h * HD + lane * DPL;
+#pragma unroll
+  for (int t = 0; t < DPL; ++t) {
+    const float v = num[t] / den;
+    const __nv_bfloat16 hi = __float2bfloat16_rn(v);
+    D.act_o[idx + t] = hi;
+    if (D.planes > 1) D.act_o[ps + idx + t] = __float2bfloat16_rn(v - __bfloat162float(hi));
+  }
+}
 
-  const float scale = 1.0f / sqrtf((float)HD);
-  const int n_pairs = cnt * G;
-  const size_t kv_stride = (size_t)D.nkv * HD;
-  const size_t page_base = (c0 < n_paged) ? page_off(D, s, layer, c0) + (size_t)g * HD + sub * 16 : 0;
-
-  for (int pb = 0; pb < n_pairs; pb += PB) {
-    int prow[PB], phead[PB], ppos[PB];
-    float q[PB][16];
+// ---------------------------------------------------------------- QKV finalize + a3: lattice-masked decode attention
+// Phase Q (warp = (row, head of the fused QKV output)): split-K sum, deferred RMSNorm scale, RoPE (rotate-half,
+// R13); query heads -> fp32 qbuf, key / value heads -> bf16 into the row's branch-private slot.
+template <int HD>
+__device__ void glue_qkv_finalize(const RoundArgs& a, int j, int gw, int n_gw, int lane) {
+  constexpr int DPL = HD / 32, HH = HD / 2;
+  const Dev& D = a.D;
+  const OpDesc& op = a.op[0];
+  const int heads = D.nh + 2 * D.nkv;
+  for (int u = gw; u < D.R_dec * heads; u += n_gw) {
+    const int r = u / heads, hh = u - r * heads;
+    const RowInfo* ri = &D.rows[r];
+    if (!ri->valid) continue;
+    const int m = ri->grp;
+    if (j >= a.dec.layer_len[m]) continue;
+    const int layer = a.dec.layer_lo[m] + j, pos = ri->pos;
+    const float inv = inv_rms(D, r);
+    const int d0 = lane * DPL;
+    const float* p = D.part + (size_t)r * op.part_ld + (size_t)hh * HD + d0;
+    float x[DPL];
 #pragma unroll
-    for (int p = 0; p < PB; ++p) {
-      prow[p] = -1; phead[p] = 0; ppos[p] = -1;
-      if (pb + p < n_pairs) {
-        const int row = r0 + (pb + p) / G;
-        const int pos = D.rows[row].pos;
-        if (pos >= c0) {
-          prow[p] = row; phead[p] = g * G + (pb + p) % G; ppos[p] = pos;
-          // q = RoPE(sum of split-K partials), this lane's 16 dims
-          const float* pr = D.part + (size_t)row * op.part_ld + phead[p] * HD;
-          const float2* rt = D.rope + (size_t)pos * HALF;
-          const int i0 = sub * 16;
-          const bool lo = i0 < HALF;
-          const int ia = lo ? i0 : i0 - HALF;              // index in the first half
+    for (int t = 0; t < DPL; ++t) x[t] = 0.f;
+    for (int s0 = 0; s0 < op.ksplit; s0 += 8) {              // all split-K partial loads of a pass in one batch
+      float tv[8][DPL];
 #pragma unroll
-          for (int e = 0; e < 16; e += 4) {
-            const float4 x1 = r_sum4(pr + ia + e, S, sst), x2 = r_sum4(pr + ia + e + HALF, S, sst);
-            const float2 c0_ = rt[ia + e], c1_ = rt[ia + e + 1], c2_ = rt[ia + e + 2], c3_ = rt[ia + e + 3];
-            if (lo) {
-              q[p][e] = x1.x * c0_.x - x2.x * c0_.y; q[p][e + 1] = x1.y * c1_.x - x2.y * c1_.y;
-              q[p][e + 2] = x1.z * c2_.x - x2.z * c2_.y; q[p][e + 3] = x1.w * c3_.x - x2.w * c3_.y;
-            } else {
-              q[p][e] = x2.x * c0_.x + x1.x * c0_.y; q[p][e + 1] = x2.y * c1_.x + x1.y * c1_.y;
-              q[p][e + 2] = x2.z * c2_.x + x1.z * c2_.y; q[p][e + 3] = x2.w * c3_.x + x1.w * c3_.y;
-            }
-          }
-        }
+      for (int i = 0; i < 8; ++i) {
+        const bool on = s0 + i < op.ksplit;
+        const size_t so = (size_t)(s0 + i) * op.split_stride;
+#pragma unroll
+        for (int t = 0; t < DPL; ++t) tv[i][t] = on ? p[so + t] : 0.f;
       }
+#pragma unroll
+      for (int i = 0; i < 8; ++i)
+#pragma unroll
+        for (int t = 0; t < DPL; ++t)
+          if (s0 + i < op.ksplit) x[t] += tv[i][t];          // split order (H3)
     }
-    bool any = false;
+    const bool is_v = hh >= D.nh + D.nkv;
+    const bool lo = lane < 16;
+    const float2* rt = D.rope + (size_t)pos * HH + (lo ? d0 : d0 - HH);
+    float o[DPL];
 #pragma unroll
-    for (int p = 0; p < PB; ++p) any |= prow[p] >= 0;
-    if (!any) continue;
-
-    // scores
-    float sc[PB][NIT];
-#pragma unroll
-    for (int it = 0; it < NIT; ++it) {
-      const int pl = it * PI + pg, pos = c0 + pl;
-      const bool shared_it = (c0 + it * PI + PI - 1) < n_paged;     // warp-uniform
-      float kf[16];
-      if (shared_it) ld_bf16x16(D.kpool + page_base + (size_t)pl * kv_stride, kf);
-#pragma unroll
-      for (int p = 0; p < PB; ++p) {
-        float dot = -INFINITY;
-        if (prow[p] >= 0) {                                            // warp-uniform
-          bool vis = true;
-          if (!shared_it) {
-            vis = pos <= ppos[p];
-            if (vis) {
-              const __nv_bfloat16* kp;
-              if (pos < n_paged) {
-                kp = D.kpool + page_base + (size_t)pl * kv_stride;
-              } else {
-                const RowInfo* ri = &D.rows[prow[p]];
-                const int ai = pos - n_paged;
-                const int slot = (ai < ri->n_anc) ? ri->anc[ai] : ri->slot;
-                kp = D.kslot + slot_off(D, s, slot, layer) + (size_t)g * HD + sub * 16;
-              }
-              ld_bf16x16(kp, kf);
-            }
-          }
-          float acc = 0.f;
-          if (vis) {
-#pragma unroll
-            for (int e = 0; e < 16; ++e) acc = fmaf(q[p][e], kf[e], acc);
-          }
-#pragma unroll
-          for (int o = 1; o < LP; o <<= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
-          dot = vis ? acc * scale : -INFINITY;
-        }
-        sc[p][it] = dot;
-      }
+    for (int t = 0; t < DPL; ++t) {
+      const float xa = x[t] * inv;
+      const float xb = __shfl_xor_sync(0xffffffffu, xa, 16); // rotate-half partner dim lives in lane ^ 16
+      const float2 cs = is_v ? make_float2(1.f, 0.f) : rt[t];
+      o[t] = is_v ? xa : (lo ? (xa * cs.x - xb * cs.y) : (xa * cs.x + xb * cs.y));
     }
-    // softmax statistics of the chunk
-    float mx[PB], lsum[PB];
+    if (hh < D.nh) {
+      float* q = D.qbuf + ((size_t)r * D.nh + hh) * HD + d0;
 #pragma unroll
-    for (int p = 0; p < PB; ++p) {
-      float v = -INFINITY;
+      for (int t = 0; t < DPL; ++t) q[t] = o[t];
+    } else {
+      const int g = is_v ? hh - D.nh - D.nkv : hh - D.nh;
+      __nv_bfloat16* dst = (is_v ? D.vslot : D.kslot) + slot_off(D, ri->seq, ri->slot, layer) + (size_t)g * HD + d0;
 #pragma unroll
-      for (int it = 0; it < NIT; ++it) v = fmaxf(v, sc[p][it]);
-#pragma unroll
-      for (int o = LP; o < 32; o <<= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, o));
-      mx[p] = v;                                   // finite for an active pair: position c0 <= ppos is visible
-      float t = 0.f;
-#pragma unroll
-      for (int it = 0; it < NIT; ++it) {
-        const float e = (sc[p][it] == -INFINITY) ? 0.f : expf(sc[p][it] - v);
-        sc[p][it] = e;
-        t += e;
-      }
-#pragma unroll
-      for (int o = LP; o < 32; o <<= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
-      lsum[p] = t;
-    }
-    // P.V (q[][] is dead: reuse as the output accumulator)
-#pragma unroll
-    for (int p = 0; p < PB; ++p)
-#pragma unroll
-      for (int e = 0; e < 16; ++e) q[p][e] = 0.f;
-#pragma unroll
-    for (int it = 0; it < NIT; ++it) {
-      const int pl = it * PI + pg, pos = c0 + pl;
-      const bool shared_it = (c0 + it * PI + PI - 1) < n_paged;
-      float vf[16];
-      if (shared_it) ld_bf16x16(D.vpool + page_base + (size_t)pl * kv_stride, vf);
-#pragma unroll
-      for (int p = 0; p < PB; ++p) {
-        if (prow[p] < 0) continue;
-        const float pr = sc[p][it];
-        if (!shared_it) {
-          if (pos > ppos[p]) continue;
-          const __nv_bfloat16* vp;
-          if (pos < n_paged) {
-            vp = D.vpool + page_base + (size_t)pl * kv_stride;
-          } else {
-            const RowInfo* ri = &D.rows[prow[p]];
-            const int ai = pos - n_paged;
-            const int slot = (ai < ri->n_anc) ? ri->anc[ai] : ri->slot;
-            vp = D.vslot + slot_off(D, s, slot, layer) + (size_t)g * HD + sub * 16;
-          }
-          ld_bf16x16(vp, vf);
-        }
-#pragma unroll
-        for (int e = 0; e < 16; ++e) q[p][e] = fmaf(pr, vf[e], q[p][e]);
-      }
-    }
-#pragma unroll
-    for (int p = 0; p < PB; ++p) {
-      if (prow[p] < 0) continue;
-#pragma unroll
-      for (int e = 0; e < 16; ++e) {
-        float v = q[p][e];
-#pragma unroll
-        for (int o = LP; o < 32; o <<= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-        q[p][e] = v;
-      }
-      float* dst = D.attn_part + (((size_t)prow[p] * D.nh + phead[p]) * D.max_chunks + c) * (HD + 2);
-      if (pg == 0) {
-#pragma unroll
-        for (int e = 0; e < 16; e += 4)
-          *reinterpret_cast<float2*>(dst + sub * 16 + e) = make_float2(q[p][e], q[p][e + 1]),
-          *reinterpret_cast<float2*>(dst + sub * 16 + e + 2) = make_float2(q[p][e + 2], q[p][e + 3]);
-      }
-      if (lane == 0) {
-        dst[HD] = mx[p];
-        dst[HD + 1] = lsum[p];
-      }
+      for (int t = 0; t < DPL; ++t) dst[t] = __float2bfloat16_rn(o[t]);
     }
   }
 }
 
+// Phase A.  Task (one CTA's epilogue group) = (stage m, sequence s, KV head g, range of 64-position chunks of
+// ABSOLUTE position); the range length is chosen so that the live tasks about fill the grid.  Per task the
+// committed K/V of each chunk is staged in shared memory with cp.async (double buffered) and applied to every
+// (row, query head) pair of (m, s, g).  The four warps split the chunk's positions (16 each): LP lanes share a
+// position (two 8-dim pieces each: conflict-free 16-byte shared loads); fp32 scores, warp-shuffle softmax over
+// the warp's 16 positions, then the four sub-partials are merged in warp order into the chunk's (o, max, sum).
+// Positions >= n_paged are the row's private suffix - ancestor slots and its own slot, read from global memory:
+// the "ancestry mask" of north_star (b).  When all chunks of (row, head) are written, the last writer merges
+// them in ascending chunk order.  A position contributes the same bits wherever its K/V lives (slot before
+// commit, page after) and whatever else shares the task: DEX stream == AR stream (H3).
+constexpr int kAttnPairs = 8;        // pairs per pass of a task
+
 template <int HD>
-__device__ void glue_attention(const RoundArgs& a, int j, int gw, int n_gw, int lane) {
+struct AttnSmem {
+  __nv_bfloat16 kv[2][2][kChunk * HD];          // [buffer][K / V][row][dim]
+  float q[kAttnPairs][HD];
+  float xch[4][kAttnPairs][HD + 2];             // per warp: (o, max, sum) over its 16 positions
+};
+
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(smem_u32(smem_dst)), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
+
+// Sub-partial of one pair over the 16 positions [c0 + 16*w, +16) of a chunk, by warp w.
+template <int HD>
+__device__ __forceinline__ void attn_sub(const Dev& D, const RowInfo* ri, int g, int c0, int w, int layer,
+                                         const __nv_bfloat16* kbuf, const __nv_bfloat16* vbuf, const float* sq, float* out,
+                                         int lane) {
+  constexpr int LP = HD / 16, PI = 32 / LP, WIT = 16 / PI, HH = HD / 2;
+  const int pos = ri->pos, s = ri->seq, n_paged = ri->n_paged, n_anc = ri->n_anc;
+  const int sub = lane % LP, pg = lane / LP;
+  const int da = sub * 8, db = HH + sub * 8;                // this lane's two 8-dim pieces
+  const float scale = 1.0f / sqrtf((float)HD);
+  float qf[16];
+#pragma unroll
+  for (int e = 0; e < 8; ++e) {
+    qf[e] = sq[da + e];
+    qf[8 + e] = sq[db + e];
+  }
+  const int pl0 = 16 * w + pg;                               // + it * PI
+  const bool all_pool = c0 + 16 * w + 16 <= n_paged;        // warp-uniform fast path: every position committed
+  const size_t slot_g = (size_t)g * HD;
+  float sc[WIT];
+#pragma unroll
+  for (int it = 0; it < WIT; ++it) {
+    const int pl = pl0 + it * PI, pp = c0 + pl;
+    float kf[16];
+    if (all_pool || pp < n_paged) {
+      cvt_bf16x16(*reinterpret_cast<const uint4*>(kbuf + pl * HD + da), *reinterpret_cast<const uint4*>(kbuf + pl * HD + db), kf);
+    } else {
+      const int ai = pp - n_paged;
+      const int slot = (ai < n_anc) ? ri->anc[ai & (kMaxAnc - 1)] : ri->slot;   // pp > pos: any valid slot (masked below)
+      const __nv_bfloat16* kp = D.kslot + slot_off(D, s, slot, layer) + slot_g;
+      cvt_bf16x16(*reinterpret_cast<const uint4*>(kp + da), *reinterpret_cast<const uint4*>(kp + db), kf);
+    }
+    float acc = 0.f, acc2 = 0.f;
+#pragma unroll
+    for (int e = 0; e < 16; e += 2) {
+      acc = fmaf(qf[e], kf[e], acc);
+      acc2 = fmaf(qf[e + 1], kf[e + 1], acc2);
+    }
+    acc += acc2;
+#pragma unroll
+    for (int o = 1; o < LP; o <<= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    sc[it] = (pp <= pos) ? acc * scale : -INFINITY;
+  }
+  float mx = sc[0];
+#pragma unroll
+  for (int it = 1; it < WIT; ++it) mx = fmaxf(mx, sc[it]);
+#pragma unroll
+  for (int o = LP; o < 32; o <<= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+  float lsum = 0.f;
+#pragma unroll
+  for (int it = 0; it < WIT; ++it) {
+    const float e = (sc[it] == -INFINITY) ? 0.f : expf(sc[it] - mx);   // mx = -inf only if every sc is -inf
+    sc[it] = e;
+    lsum += e;
+  }
+#pragma unroll
+  for (int o = LP; o < 32; o <<= 1) lsum += __shfl_xor_sync(0xffffffffu, lsum, o);
+  float of[16];
+#pragma unroll
+  for (int e = 0; e < 16; ++e) of[e] = 0.f;
+#pragma unroll
+  for (int it = 0; it < WIT; ++it) {
+    const int pl = pl0 + it * PI, pp = c0 + pl;
+    float vf[16];
+    if (all_pool || pp < n_paged) {
+      cvt_bf16x16(*reinterpret_cast<const uint4*>(vbuf + pl * HD + da), *reinterpret_cast<const uint4*>(vbuf + pl * HD + db), vf);
+    } else {
+      const int ai = pp - n_paged;
+      const int slot = (ai < n_anc) ? ri->anc[ai & (kMaxAnc - 1)] : ri->slot;
+      const __nv_bfloat16* vp = D.vslot + slot_off(D, s, slot, layer) + slot_g;
+      cvt_bf16x16(*reinterpret_cast<const uint4*>(vp + da), *reinterpret_cast<const uint4*>(vp + db), vf);
+    }
+    const float pr = sc[it];
+    if (pp <= pos) {
+#pragma unroll
+      for (int e = 0; e < 16; ++e) of[e] = fmaf(pr, vf[e], of[e]);
+    }
+  }
+#pragma unroll
+  for (int e = 0; e < 16; ++e) {
+    float v = of[e];
+#pragma unroll
+    for (int o = LP; o < 32; o <<= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    of[e] = v;
+  }
+  if (pg == 0) {
+#pragma unroll
+    for (int e = 0; e < 8; ++e) {
+      out[da + e] = of[e];
+      out[db + e] = of[8 + e];
+    }
+  }
+  if (lane == 0) {
+    out[HD] = mx;
+    out[HD + 1] = lsum;
+  }
+}
+
+template <int HD>
+__device__ void glue_attention(const RoundArgs& a, int j, int tid_e, int lane, int we, int cta, int G, AttnSmem<HD>* sm,
+                               int n_live_ms) {
+  constexpr int CPR = HD / 8;                                // 16-byte pieces per K/V row
   const Dev& D = a.D;
-  const OpDesc& op = a.op[0];
-  const int per_ms = D.nkv * a.n_chunks;
-  const int n_units = D.N * D.max_seqs * per_ms;
-  for (int u = gw; u < n_units; u += n_gw) {
+  const int n_msg = max(1, n_live_ms) * D.nkv;
+  const int n_ranges = max(1, min(a.n_chunks, G / n_msg));
+  const int CR = (a.n_chunks + n_ranges - 1) / n_ranges;     // chunks per task
+  const int per_ms = D.nkv * n_ranges;
+  const int n_tasks = D.N * D.max_seqs * per_ms;
+  const int Gq = D.nh / D.nkv;
+  const size_t kv_stride = (size_t)D.nkv * HD;
+
+  for (int u = cta; u < n_tasks; u += G) {
     const int ms = u / per_ms, rem = u - ms * per_ms;
     const int m = ms / D.max_seqs, s = ms - m * D.max_seqs;
-    const int g = rem / a.n_chunks, c = rem - g * a.n_chunks;
-    attn_unit<HD>(a, j, m, s, g, c, lane, op);
+    const int g = rem / n_ranges, rg = rem - g * n_ranges;
+    const SeqState st = D.seqs[s];
+    if (!r_seq_live(st) || st.q < m || j >= a.dec.layer_len[m]) continue;
+    const int ca = rg * CR;
+    const int cb = min(min(ca + CR, a.n_chunks), (st.ctx_len + st.q) / kChunk + 1);   // no row lies beyond ctx_len + q
+    if (ca >= cb) continue;
+    const int cnt = r_stage_count(st.q, m);
+    const int layer = a.dec.layer_lo[m] + j;
+    const int r0 = a.dec.row_base[m] + s * cap_of(D.N, m);
+    const int n_paged = st.ctx_len;
+    const int n_pairs = cnt * Gq;
+
+    for (int pb = 0; pb < n_pairs; pb += kAttnPairs) {
+      const int np = min(kAttnPairs, n_pairs - pb);
+      // ---- chunks of the range: stage committed K/V (double buffered), every pair of the pass attends
+      auto stage = [&](int c, int buf) {
+        const int c0 = c * kChunk;
+        const int n_rows = min(kChunk, n_paged - c0);        // committed rows of the chunk (one page: page_size % 64 == 0)
+        if (n_rows > 0) {
+          const size_t base = page_off(D, s, layer, c0) + (size_t)g * HD;
+          for (int id = tid_e; id < n_rows * CPR; id += kEpiThreads) {
+            const int pl = id / CPR, cj = id - pl * CPR;
+            cp_async16(&sm->kv[buf][0][pl * HD + cj * 8], D.kpool + base + (size_t)pl * kv_stride + cj * 8);
+            cp_async16(&sm->kv[buf][1][pl * HD + cj * 8], D.vpool + base + (size_t)pl * kv_stride + cj * 8);
+          }
+        }
+        cp_async_commit();
+      };
+      stage(ca, 0);
+      // ---- q of the pass's pairs (phase Q wrote it), in flight together with the first chunk
+      for (int id = tid_e; id < np * HD; id += kEpiThreads) {
+        const int pi = id / HD, t = id - pi * HD;
+        const int r = r0 + (pb + pi) / Gq, h = g * Gq + (pb + pi) % Gq;
+        sm->q[pi][t] = D.qbuf[((size_t)r * D.nh + h) * HD + t];
+      }
+      for (int c = ca; c < cb; ++c) {
+        const int buf = (c - ca) & 1, c0 = c * kChunk;
+        if (c + 1 < cb) stage(c + 1, buf ^ 1);
+        else cp_async_commit();
+        cp_async_wait<1>();
+        bar_epi();                                           // chunk c staged by all threads; q written
+        for (int pi = 0; pi < np; ++pi) {
+          const RowInfo* ri = &D.rows[r0 + (pb + pi) / Gq];
+          if (ri->pos < c0) continue;
+          attn_sub<HD>(D, ri, g, c0, we, layer, sm->kv[buf][0], sm->kv[buf][1], sm->q[pi], sm->xch[we][pi], lane);
+        }
+        bar_epi();                                           // sub-partials of all four warps written
+        for (int id = tid_e; id < np * HD; id += kEpiThreads) {
+          const int pi = id / HD, t = id - pi * HD;
+          const int r = r0 + (pb + pi) / Gq, h = g * Gq + (pb + pi) % Gq;
+          if (D.rows[r].pos < c0) continue;
+          float M = sm->xch[0][pi][HD];                      // finite: warp 0 holds position c0 <= pos
+#pragma unroll
+          for (int w = 1; w < 4; ++w) M = fmaxf(M, sm->xch[w][pi][HD]);
+          float num = 0.f, den = 0.f;
+#pragma unroll
+          for (int w = 0; w < 4; ++w) {                      // warp order (fixed: H3)
+            const float wgt = expf(sm->xch[w][pi][HD] - M);  // exp(-inf) = 0 for a warp without visible positions
+            num = fmaf(wgt, sm->xch[w][pi][t], num);
+            den = fmaf(wgt, sm->xch[w][pi][HD + 1], den);
+          }
+          float* dst = D.attn_part + (((size_t)r * D.nh + h) * D.max_chunks + c) * (HD + 2);
+          dst[t] = num;
+          if (t == 0) {
+            dst[HD] = M;
+            dst[HD + 1] = den;
+          }
+        }
+        bar_epi();                                           // kv buffer and xch free for the next chunk
+      }
+      // ---- all chunk partials of this pass are written: count them in; the last writer of (row, head) merges
+      __threadfence();
+      bar_epi();
+      for (int pi = we; pi < np; pi += 4) {
+        const int r = r0 + (pb + pi) / Gq, h = g * Gq + (pb + pi) % Gq;
+        const int pos = D.rows[r].pos;
+        const int mine = min(cb, pos / kChunk + 1) - ca;     // chunks of this range visible to the row
+        if (mine <= 0) continue;
+        const int nc = pos / kChunk + 1;
+        int old = 0;
+        if (lane == 0) old = atomicAdd(&D.attn_cnt[r * D.nh + h], mine);
+        old = __shfl_sync(0xffffffffu, old, 0);
+        if (old + mine == nc) {
+          __threadfence();
+          attn_merge<HD>(D, r, h, nc, lane);
+          if (lane == 0) D.attn_cnt[r * D.nh + h] = 0;
+        }
+      }
+      bar_epi();
+    }
   }
 }
 
@@ -545,6 +638,7 @@ __global__ void __launch_bounds__(kRoundThreads, 1) k_round(const __grid_constan
   __shared__ int s_nb[16];
   __shared__ uint32_t s_valid[32];
   __shared__ float s_red[4];
+  __shared__ int s_live_ms;
   __shared__ int s_steps;
   __shared__ unsigned s_seen;
 
@@ -563,6 +657,12 @@ __global__ void __launch_bounds__(kRoundThreads, 1) k_round(const __grid_constan
     }
     s_steps = steps;
     s_seen = 0;
+    int lm = 0;
+    for (int s = 0; s < D.max_seqs; ++s) {
+      const SeqState st = D.seqs[s];
+      if (r_seq_live(st)) lm += min(st.q, D.N - 1) + 1;
+    }
+    s_live_ms = lm;
     for (int i = 0; i < NS; ++i) {
       mbar_init(&full[i], 1);
       mbar_init(&empty[i], 1);
@@ -596,18 +696,15 @@ __global__ void __launch_bounds__(kRoundThreads, 1) k_round(const __grid_constan
       Walker w;
       unsigned st = 0, ph = 0;
       bool wrapped = false;
-      const bool tiled = (a.dbg & 4) != 0;
       for (w.start(sq); w.valid; w.next(sq)) {
-        const CUtensorMap* desc = tiled ? &tm.wt[w.o.which] : &tm.w[w.o.which];
-        const uint32_t tx = kABytes + ((a.dbg & 8) ? 0 : D.planes * w.it.nb * 128);
+        const CUtensorMap* desc = &tm.w[w.o.which];
+        const uint32_t tx = kABytes + D.planes * w.it.nb * 128;
         const int c1 = w.it.tile * kTileM, c2 = w.it.layer;
-        const int tbase = (w.it.layer * (w.o.n_tiles - (a.op[w.o.which].out_dim % kTileM ? 1 : 0)) + min(w.it.tile, w.o.n_tiles - 2)) * (a.op[w.o.which].k_dim / kTileK);
         for (int kb = w.it.kb0; kb < w.it.kb1; ++kb) {
           if (wrapped) mbar_wait(&empty[st], ph ^ 1u);
           if (elect_one()) {
             mbar_expect_tx(&full[st], tx);
-            if (tiled) tma_load_3d(smem + (size_t)st * stage_bytes, desc, &full[st], 0, 0, tbase + min(kb, a.op[w.o.which].k_dim / kTileK - 1), kEvictFirst);
-            else tma_load_3d(smem + (size_t)st * stage_bytes, desc, &full[st], kb * kTileK, c1, c2, kEvictFirst);
+            tma_load_3d(smem + (size_t)st * stage_bytes, desc, &full[st], kb * kTileK, c1, c2, kEvictFirst);
           }
           __syncwarp();
           if (++st == (unsigned)NS) { st = 0; ph ^= 1u; wrapped = true; }
@@ -620,7 +717,7 @@ __global__ void __launch_bounds__(kRoundThreads, 1) k_round(const __grid_constan
       bool wrapped = false;
       unsigned seen = 0;
       for (w.start(sq); w.valid; w.next(sq)) {
-        const unsigned need = (a.dbg & 2) ? 0u : sq.dep(w.t);
+        const unsigned need = sq.dep(w.t);
         if (seen < need) {
           unsigned spins = 0;
           while ((seen = *reinterpret_cast<volatile unsigned*>(&s_seen)) < need) {
@@ -637,7 +734,7 @@ __global__ void __launch_bounds__(kRoundThreads, 1) k_round(const __grid_constan
           // slot free (its previous tile consumed) => full[st] is in this tile's phase; the bytes may
           // land before the weight producer arms the phase (tx-count goes negative, arrival still pending)
           if (wrapped) mbar_wait(&empty[st], ph ^ 1u);
-          if (!(a.dbg & 8) && elect_one()) {
+          if (elect_one()) {
             uint8_t* sB = smem + (size_t)st * stage_bytes + kABytes;
             if (a.stacked) {
               for (int r = 0; r < nb; r += kBoxRows)
@@ -716,23 +813,32 @@ __global__ void __launch_bounds__(kRoundThreads, 1) k_round(const __grid_constan
       };
       for (int j = 0; j < sq.n_steps; ++j) {
         run_items(4 * j); stamp();
-        ++gb; grid_bar(D.gbar, gb * G, tid_e, &s_seen, gb, a.dbg); stamp();
-        if (!(a.dbg & 1)) { if (D.hd == 128) glue_attention<128>(a, j, gw, n_gw, lane); else glue_attention<64>(a, j, gw, n_gw, lane); }
-        ++gb; grid_bar(D.gbar, gb * G, tid_e, &s_seen, gb, a.dbg); stamp();
-        if (!(a.dbg & 1)) { if (D.hd == 128) glue_combine<128>(a, j, gw, n_gw, lane); else glue_combine<64>(a, j, gw, n_gw, lane); }
-        ++gb; grid_bar(D.gbar, gb * G, tid_e, &s_seen, gb, a.dbg); stamp();
+        ++gb; grid_bar(D.gbar, gb * G, tid_e, &s_seen, gb); stamp();
+        if (D.hd == 128) glue_qkv_finalize<128>(a, j, gw, n_gw, lane); else glue_qkv_finalize<64>(a, j, gw, n_gw, lane);
+        stamp();
+        ++gb; grid_bar(D.gbar, gb * G, tid_e, &s_seen, gb); stamp();
+        {
+          void* asm_ = smem + a.attn_smem_off;
+          if (D.hd == 128) glue_attention<128>(a, j, tid_e, lane, we, blockIdx.x, G, reinterpret_cast<AttnSmem<128>*>(asm_), s_live_ms);
+          else glue_attention<64>(a, j, tid_e, lane, we, blockIdx.x, G, reinterpret_cast<AttnSmem<64>*>(asm_), s_live_ms);
+        }
+        stamp();
+        ++gb; grid_bar(D.gbar, gb * G, tid_e, &s_seen, gb); stamp();
         run_items(4 * j + 1); stamp();
-        ++gb; grid_bar(D.gbar, gb * G, tid_e, &s_seen, gb, a.dbg); stamp();
-        if (!(a.dbg & 1)) glue_add_norm(a, j, 0, a.op[1], s_red, tid_e, blockIdx.x, G);
-        ++gb; grid_bar(D.gbar, gb * G, tid_e, &s_seen, gb, a.dbg); stamp();
+        ++gb; grid_bar(D.gbar, gb * G, tid_e, &s_seen, gb); stamp();
+        glue_add_norm(a, j, 0, a.op[1], s_red, tid_e, blockIdx.x, G);
+        stamp();
+        ++gb; grid_bar(D.gbar, gb * G, tid_e, &s_seen, gb); stamp();
         run_items(4 * j + 2); stamp();
-        ++gb; grid_bar(D.gbar, gb * G, tid_e, &s_seen, gb, a.dbg); stamp();
-        if (!(a.dbg & 1)) glue_silu(a, j, a.op[2], tid_e, blockIdx.x, G);
-        ++gb; grid_bar(D.gbar, gb * G, tid_e, &s_seen, gb, a.dbg); stamp();
+        ++gb; grid_bar(D.gbar, gb * G, tid_e, &s_seen, gb); stamp();
+        glue_silu(a, j, a.op[2], gw, n_gw, lane);
+        stamp();
+        ++gb; grid_bar(D.gbar, gb * G, tid_e, &s_seen, gb); stamp();
         run_items(4 * j + 3); stamp();
-        ++gb; grid_bar(D.gbar, gb * G, tid_e, &s_seen, gb, a.dbg); stamp();
-        if (!(a.dbg & 1)) glue_add_norm(a, j, 1, a.op[3], s_red, tid_e, blockIdx.x, G);
-        ++gb; grid_bar(D.gbar, gb * G, tid_e, &s_seen, gb, a.dbg); stamp();
+        ++gb; grid_bar(D.gbar, gb * G, tid_e, &s_seen, gb); stamp();
+        glue_add_norm(a, j, 1, a.op[3], s_red, tid_e, blockIdx.x, G);
+        stamp();
+        ++gb; grid_bar(D.gbar, gb * G, tid_e, &s_seen, gb); stamp();
       }
       run_items(4 * sq.n_steps); stamp();
     }
@@ -743,8 +849,10 @@ __global__ void __launch_bounds__(kRoundThreads, 1) k_round(const __grid_constan
   if (warp == 1) tmem_dealloc(tmem_base, 2 * a.acc_cols);
 }
 
+size_t round_attn_smem(int hd) { return hd == 128 ? sizeof(AttnSmem<128>) : sizeof(AttnSmem<64>); }
+
 cudaError_t round_init() {
-  return cudaFuncSetAttribute(k_round, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024);
+  return cudaFuncSetAttribute(k_round, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024);
 }
 
 // Cooperative launch: all CTAs must be co-resident (they meet at grid barriers).
