@@ -16,7 +16,7 @@ constexpr int kTileM = 128;         // GEMM: weight rows (out features) per MMA 
 constexpr int kTileK = 64;          // GEMM: bf16 K elements per pipeline stage (128 B rows, SW128)
 constexpr int kBoxRows = 16;        // activation rows per TMA box
 constexpr int kPrefillRows = 128;   // rows per prefill chunk
-constexpr int kSsSeg = 16;          // sum-of-squares segments per row (512 elements each, d <= 8192)
+constexpr int kSsSeg = 64;          // sum-of-squares segments per row (128 elements each, d <= 8192)
 
 // A "plan" = groups of stacked rows, each streaming its own layer segment.  Decode: group m =
 // explorer E_m with stage Pi_m = Layers(d_{m-1}, d_m].  Prefill: one group
@@ -94,7 +94,7 @@ struct Dev {
   __nv_bfloat16 *kslot, *vslot;   // [max_seqs][n_slots][L][nkv][hd]
   float* x_cur;            // [R_cap][d] residual stream of this round's rows
   float* x_front;          // [R_cap][d] frontier hidden (h_out of the previous level)
-  float* ss_part;          // [R_cap][kSsSeg] sum of squares of the row the last norm was taken of, per 512-element
+  float* ss_part;          // [R_cap][kSsSeg] sum of squares of the row the last norm was taken of, per 128-element
                            // segment.  The RMSNorm scale is DEFERRED: operand planes hold x*w, consumers of the GEMM
                            // output multiply by inv_rms(row) = rsqrt(sum_seg ss / d + eps) (exact: the scale is per row)
   int* attn_cnt;           // [R_cap][nh] chunk partials written (last writer merges them)
@@ -141,10 +141,14 @@ __device__ __forceinline__ float key2f(uint32_t k) {
 }
 
 __device__ __forceinline__ float inv_rms(const Dev& D, int r) {
-  const float* p = D.ss_part + (size_t)r * kSsSeg;
+  const float4* p = reinterpret_cast<const float4*>(D.ss_part + (size_t)r * kSsSeg);
+  const int n4 = ((D.d + 127) / 128 + 3) / 4;            // float4 groups that hold segments (unused segments hold 0)
+  float4 v[kSsSeg / 4];
+#pragma unroll
+  for (int i = 0; i < kSsSeg / 4; ++i) v[i] = (i < n4) ? p[i] : make_float4(0.f, 0.f, 0.f, 0.f);   // one batch of loads
   float ss = 0.f;
 #pragma unroll
-  for (int i = 0; i < kSsSeg; ++i) ss += p[i];          // fixed order (unused segments hold 0)
+  for (int i = 0; i < kSsSeg / 4; ++i) ss += (v[i].x + v[i].y) + (v[i].z + v[i].w);   // fixed order
   return 1.0f / sqrtf(ss / (float)D.d + D.eps);
 }
 

@@ -29,11 +29,14 @@
 
 namespace dexk {
 
-constexpr int kRoundThreads = 224;      // warps: 0 weight TMA, 1 MMA, 2-5 epilogue/glue, 6 activation TMA
-constexpr int kEpiThreads = 128;
+// warps: 0 weight TMA, 1 MMA, 2-5 GEMM epilogue + glue, 6 activation TMA, 7-10 glue only.  A lone warp per
+// scheduler runs the glue phases latency-bound; two per scheduler measured best (12 glue warps push the kernel
+// under 128 registers and spill).
+constexpr int kRoundThreads = 352;
 
 // ---------------------------------------------------------------- small device helpers
-__device__ __forceinline__ void bar_epi() { asm volatile("bar.sync 1, 128;\n" ::: "memory"); }
+template <int GT>
+__device__ __forceinline__ void bar_epi() { asm volatile("bar.sync 1, %0;\n" ::"n"(GT) : "memory"); }
 __device__ __forceinline__ unsigned ld_acquire_u32(const unsigned* p) {
   unsigned v;
   asm volatile("ld.acquire.gpu.global.u32 %0, [%1];\n" : "=r"(v) : "l"(p) : "memory");
@@ -162,21 +165,24 @@ struct Walker {            // this CTA's items, in order
 };
 
 // ---------------------------------------------------------------- grid barrier (epilogue groups)
+// Every epilogue thread orders its generic-proxy global writes against later async-proxy (TMA) reads, the CTA
+// barrier collects them, and ONE thread publishes them gpu-wide (fence cumulativity, as in a cooperative-groups
+// grid sync), arrives, waits for all CTAs, and invalidates this SM's L1 (gpu-scope fence) before the group goes on.
+template <int GT>
 __device__ __forceinline__ void grid_bar(unsigned* gbar, unsigned target, int tid_e, volatile unsigned* s_seen, unsigned gb) {
   __threadfence();
-  fence_proxy_async();           // generic-proxy writes (operand planes) -> later TMA reads
-  bar_epi();
+  fence_proxy_async();
+  bar_epi<GT>();
   if (tid_e == 0) {
     red_release_add(gbar, 1u);
     unsigned spins = 0;
     while (ld_acquire_u32(gbar) < target) {
-      __nanosleep(32);
-      if (++spins > 100000000u) __trap();   // protocol bug: trap instead of hanging the box
+      if (++spins > 400000000u) __trap();   // protocol bug: trap instead of hanging the box
     }
     __threadfence();
-    *s_seen = gb;                // the producer of this CTA learns of the barrier without polling HBM/L2
+    *s_seen = gb;                // the activation producer of this CTA learns of the barrier without polling L2
   }
-  bar_epi();
+  bar_epi<GT>();
 }
 
 // ---------------------------------------------------------------- glue phases (epilogue group)
@@ -185,31 +191,23 @@ __device__ __forceinline__ float r_warp_sum(float v) {
   for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
   return v;
 }
-__device__ __forceinline__ float group_sum(float v, float* red /*[4]*/, int tid_e) {
-  v = r_warp_sum(v);
-  bar_epi();
-  if ((tid_e & 31) == 0) red[tid_e >> 5] = v;
-  bar_epi();
-  return (red[0] + red[1]) + (red[2] + red[3]);
-}
-
 // Every glue phase is laid out for memory-level parallelism: a thread issues all of its loads in one or two
 // batches (a dependent load under the weight stream costs microseconds), and the work is spread over all CTAs.
 
-// x += sum_s part[s]; operand planes <- x * w (RMSNorm scale deferred: Dev::ss_part).  Unit = (row, 512-element
-// segment), one per CTA pass.  mode 0: after o_proj (w = norm_ffn[l] -> act_a); mode 1: after down_proj (next
-// layer's attention norm -> act_a, or the shared final norm -> act_e).
-__device__ void glue_add_norm(const RoundArgs& a, int j, int mode, const OpDesc& op, float* red, int tid_e, int cta, int G) {
+// x += sum_s part[s]; operand planes <- x * w (RMSNorm scale deferred: Dev::ss_part).  Warp unit = (row,
+// 128-element segment).  mode 0: after o_proj (w = norm_ffn[l] -> act_a); mode 1: after down_proj (next layer's
+// attention norm -> act_a, or the shared final norm -> act_e).
+__device__ void glue_add_norm(const RoundArgs& a, int j, int mode, const OpDesc& op, int gw, int n_gw, int lane) {
   const Dev& D = a.D;
-  const int n_seg = (D.d + 511) / 512;
-  for (int u = cta; u < D.R_dec * n_seg; u += G) {
+  const int n_seg = (D.d + 127) / 128;
+  for (int u = gw; u < D.R_dec * n_seg; u += n_gw) {
     const int r = u / n_seg, seg = u - r * n_seg;
     const RowInfo* ri = &D.rows[r];
     if (!ri->valid) continue;
     const int grp = ri->grp;
     if (j >= a.dec.layer_len[grp]) continue;
     const int layer = a.dec.layer_lo[grp] + j;
-    const int i = seg * 512 + tid_e * 4;
+    const int i = seg * 128 + lane * 4;
     float ss = 0.f;
     if (i < D.d) {
       const float* w;
@@ -232,8 +230,8 @@ __device__ void glue_add_norm(const RoundArgs& a, int j, int mode, const OpDesc&
       r_split_store4(dst, (size_t)D.R_cap * D.d, (size_t)r * D.d + i, make_float4(v.x * wv.x, v.y * wv.y, v.z * wv.z, v.w * wv.w),
                      D.planes);
     }
-    ss = group_sum(ss, red, tid_e);
-    if (tid_e == 0) D.ss_part[(size_t)r * kSsSeg + seg] = ss;
+    ss = r_warp_sum(ss);
+    if (lane == 0) D.ss_part[(size_t)r * kSsSeg + seg] = ss;
   }
 }
 
@@ -511,14 +509,20 @@ __device__ __forceinline__ void attn_sub(const Dev& D, const RowInfo* ri, int g,
   }
 }
 
-template <int HD>
-__device__ void glue_attention(const RoundArgs& a, int j, int tid_e, int lane, int we, int cta, int G, AttnSmem<HD>* sm,
-                               int n_live_ms) {
+template <int HD, int GT>
+__device__ void glue_attention(const RoundArgs& a, int j, int tid_e, int lane, int we, int cta, int G,
+                               AttnSmem<HD>* sm, int n_live_ms) {
+  constexpr int kGlueWarps = GT / 32, kEpiThreads = GT;
   constexpr int CPR = HD / 8;                                // 16-byte pieces per K/V row
   const Dev& D = a.D;
   const int n_msg = max(1, n_live_ms) * D.nkv;
-  const int n_ranges = max(1, min(a.n_chunks, G / n_msg));
-  const int CR = (a.n_chunks + n_ranges - 1) / n_ranges;     // chunks per task
+  // chunks per task: one wave of tasks over the grid when a task then has <= 6 chunks (one-row rounds),
+  // else fine-grained tasks of 3 chunks dealt round-robin (lattice rounds: many (stage, head) families)
+  const int nr_fit = G / n_msg;
+  const int cr_fit = nr_fit >= 1 ? (a.n_chunks + nr_fit - 1) / nr_fit : a.n_chunks;
+  const int CR = cr_fit <= 6 ? max(1, cr_fit) : 3;
+  const int n_ranges = (a.n_chunks + CR - 1) / CR;
+  const int team = we >> 2, quarter = we & 3;               // teams of four warps: team = pair, warp = position quarter
   const int per_ms = D.nkv * n_ranges;
   const int n_tasks = D.N * D.max_seqs * per_ms;
   const int Gq = D.nh / D.nkv;
@@ -567,13 +571,13 @@ __device__ void glue_attention(const RoundArgs& a, int j, int tid_e, int lane, i
         if (c + 1 < cb) stage(c + 1, buf ^ 1);
         else cp_async_commit();
         cp_async_wait<1>();
-        bar_epi();                                           // chunk c staged by all threads; q written
-        for (int pi = 0; pi < np; ++pi) {
+        bar_epi<GT>();                                           // chunk c staged by all threads; q written
+        for (int pi = team; pi < np; pi += kGlueWarps / 4) {
           const RowInfo* ri = &D.rows[r0 + (pb + pi) / Gq];
           if (ri->pos < c0) continue;
-          attn_sub<HD>(D, ri, g, c0, we, layer, sm->kv[buf][0], sm->kv[buf][1], sm->q[pi], sm->xch[we][pi], lane);
+          attn_sub<HD>(D, ri, g, c0, quarter, layer, sm->kv[buf][0], sm->kv[buf][1], sm->q[pi], sm->xch[quarter][pi], lane);
         }
-        bar_epi();                                           // sub-partials of all four warps written
+        bar_epi<GT>();                                           // sub-partials of all four warps written
         for (int id = tid_e; id < np * HD; id += kEpiThreads) {
           const int pi = id / HD, t = id - pi * HD;
           const int r = r0 + (pb + pi) / Gq, h = g * Gq + (pb + pi) % Gq;
@@ -595,12 +599,12 @@ __device__ void glue_attention(const RoundArgs& a, int j, int tid_e, int lane, i
             dst[HD + 1] = den;
           }
         }
-        bar_epi();                                           // kv buffer and xch free for the next chunk
+        bar_epi<GT>();                                           // kv buffer and xch free for the next chunk
       }
       // ---- all chunk partials of this pass are written: count them in; the last writer of (row, head) merges
       __threadfence();
-      bar_epi();
-      for (int pi = we; pi < np; pi += 4) {
+      bar_epi<GT>();
+      for (int pi = we; pi < np; pi += kGlueWarps) {
         const int r = r0 + (pb + pi) / Gq, h = g * Gq + (pb + pi) % Gq;
         const int pos = D.rows[r].pos;
         const int mine = min(cb, pos / kChunk + 1) - ca;     // chunks of this range visible to the row
@@ -615,13 +619,14 @@ __device__ void glue_attention(const RoundArgs& a, int j, int tid_e, int lane, i
           if (lane == 0) D.attn_cnt[r * D.nh + h] = 0;
         }
       }
-      bar_epi();
+      bar_epi<GT>();
     }
   }
 }
 
 // ---------------------------------------------------------------- the kernel
-__global__ void __launch_bounds__(kRoundThreads, 1) k_round(const __grid_constant__ TmSet tm, const __grid_constant__ RoundArgs a) {
+template <int kMaxThreads>
+__global__ void __launch_bounds__(kMaxThreads, 1) k_round(const __grid_constant__ TmSet tm, const __grid_constant__ RoundArgs a) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   const Dev& D = a.D;
@@ -637,7 +642,6 @@ __global__ void __launch_bounds__(kRoundThreads, 1) k_round(const __grid_constan
 
   __shared__ int s_nb[16];
   __shared__ uint32_t s_valid[32];
-  __shared__ float s_red[4];
   __shared__ int s_live_ms;
   __shared__ int s_steps;
   __shared__ unsigned s_seen;
@@ -645,7 +649,7 @@ __global__ void __launch_bounds__(kRoundThreads, 1) k_round(const __grid_constan
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   if (threadIdx.x < 32) s_valid[threadIdx.x] = 0;
   __syncthreads();
-  for (int r = threadIdx.x; r < D.R_cap; r += kRoundThreads)
+  for (int r = threadIdx.x; r < D.R_cap; r += blockDim.x)
     if (D.rows[r].valid) atomicOr(&s_valid[r >> 5], 1u << (r & 31));
   if (threadIdx.x == 0) {
     int steps = 0;
@@ -776,11 +780,13 @@ __global__ void __launch_bounds__(kRoundThreads, 1) k_round(const __grid_constan
         if (elect_one()) umma_commit(&tfull[as]);   // accumulator complete -> epilogue
         __syncwarp();
       }
-    } else if (warp < 6) {
-      // ===================== epilogue group: GEMM epilogues + glue + grid barriers =====================
-      const int tid_e = threadIdx.x - 64, we = warp - 2;
+    } else {
+      // ===================== glue group (12 warps): GEMM epilogues (warps 2-5) + glue + grid barriers =====================
+      const int we = warp < 6 ? warp - 2 : warp - 3;        // 0 .. glue warps - 1
+      const int tid_e = we * 32 + lane;
+      constexpr int GT = kMaxThreads - 96, kGlueWarps = GT / 32;   // glue threads / warps
       const int quarter = warp & 3;
-      const int gw = blockIdx.x * 4 + we, n_gw = gridDim.x * 4;
+      const int gw = blockIdx.x * kGlueWarps + we, n_gw = gridDim.x * kGlueWarps;
       EpiCtx ec;
       ec.rows = D.rows; ec.s_valid = s_valid; ec.part = D.part; ec.vocab = D.vocab; ec.best_key = D.best_key;
       ec.ref_tile = D.ref_tile; ec.ref_tiles = D.ref_tiles;
@@ -800,6 +806,7 @@ __global__ void __launch_bounds__(kRoundThreads, 1) k_round(const __grid_constan
         const OpDesc& od = a.op[t < 4 * sq.n_steps ? (t & 3) : 4];
         ec.mode = (t < 4 * sq.n_steps) ? 0 : 1;
         ec.part_ld = od.part_ld; ec.split_stride = od.split_stride; ec.out_dim = od.out_dim;
+        if (we >= 4) return;                                 // TMEM lane quarters belong to warps 2-5
         for (; w.valid && w.t == t; w.next(sq), ++n_it) {
           const int as = n_it & 1;
           mbar_wait(&tfull[as], (n_it >> 1) & 1);
@@ -813,32 +820,32 @@ __global__ void __launch_bounds__(kRoundThreads, 1) k_round(const __grid_constan
       };
       for (int j = 0; j < sq.n_steps; ++j) {
         run_items(4 * j); stamp();
-        ++gb; grid_bar(D.gbar, gb * G, tid_e, &s_seen, gb); stamp();
+        ++gb; grid_bar<GT>(D.gbar, gb * G, tid_e, &s_seen, gb); stamp();
         if (D.hd == 128) glue_qkv_finalize<128>(a, j, gw, n_gw, lane); else glue_qkv_finalize<64>(a, j, gw, n_gw, lane);
         stamp();
-        ++gb; grid_bar(D.gbar, gb * G, tid_e, &s_seen, gb); stamp();
+        ++gb; grid_bar<GT>(D.gbar, gb * G, tid_e, &s_seen, gb); stamp();
         {
           void* asm_ = smem + a.attn_smem_off;
-          if (D.hd == 128) glue_attention<128>(a, j, tid_e, lane, we, blockIdx.x, G, reinterpret_cast<AttnSmem<128>*>(asm_), s_live_ms);
-          else glue_attention<64>(a, j, tid_e, lane, we, blockIdx.x, G, reinterpret_cast<AttnSmem<64>*>(asm_), s_live_ms);
+          if (D.hd == 128) glue_attention<128, GT>(a, j, tid_e, lane, we, blockIdx.x, G, reinterpret_cast<AttnSmem<128>*>(asm_), s_live_ms);
+          else glue_attention<64, GT>(a, j, tid_e, lane, we, blockIdx.x, G, reinterpret_cast<AttnSmem<64>*>(asm_), s_live_ms);
         }
         stamp();
-        ++gb; grid_bar(D.gbar, gb * G, tid_e, &s_seen, gb); stamp();
+        ++gb; grid_bar<GT>(D.gbar, gb * G, tid_e, &s_seen, gb); stamp();
         run_items(4 * j + 1); stamp();
-        ++gb; grid_bar(D.gbar, gb * G, tid_e, &s_seen, gb); stamp();
-        glue_add_norm(a, j, 0, a.op[1], s_red, tid_e, blockIdx.x, G);
+        ++gb; grid_bar<GT>(D.gbar, gb * G, tid_e, &s_seen, gb); stamp();
+        glue_add_norm(a, j, 0, a.op[1], gw, n_gw, lane);
         stamp();
-        ++gb; grid_bar(D.gbar, gb * G, tid_e, &s_seen, gb); stamp();
+        ++gb; grid_bar<GT>(D.gbar, gb * G, tid_e, &s_seen, gb); stamp();
         run_items(4 * j + 2); stamp();
-        ++gb; grid_bar(D.gbar, gb * G, tid_e, &s_seen, gb); stamp();
+        ++gb; grid_bar<GT>(D.gbar, gb * G, tid_e, &s_seen, gb); stamp();
         glue_silu(a, j, a.op[2], gw, n_gw, lane);
         stamp();
-        ++gb; grid_bar(D.gbar, gb * G, tid_e, &s_seen, gb); stamp();
+        ++gb; grid_bar<GT>(D.gbar, gb * G, tid_e, &s_seen, gb); stamp();
         run_items(4 * j + 3); stamp();
-        ++gb; grid_bar(D.gbar, gb * G, tid_e, &s_seen, gb); stamp();
-        glue_add_norm(a, j, 1, a.op[3], s_red, tid_e, blockIdx.x, G);
+        ++gb; grid_bar<GT>(D.gbar, gb * G, tid_e, &s_seen, gb); stamp();
+        glue_add_norm(a, j, 1, a.op[3], gw, n_gw, lane);
         stamp();
-        ++gb; grid_bar(D.gbar, gb * G, tid_e, &s_seen, gb); stamp();
+        ++gb; grid_bar<GT>(D.gbar, gb * G, tid_e, &s_seen, gb); stamp();
       }
       run_items(4 * sq.n_steps); stamp();
     }
@@ -852,7 +859,7 @@ __global__ void __launch_bounds__(kRoundThreads, 1) k_round(const __grid_constan
 size_t round_attn_smem(int hd) { return hd == 128 ? sizeof(AttnSmem<128>) : sizeof(AttnSmem<64>); }
 
 cudaError_t round_init() {
-  return cudaFuncSetAttribute(k_round, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024);
+  return cudaFuncSetAttribute(k_round<kRoundThreads>, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024);
 }
 
 // Cooperative launch: all CTAs must be co-resident (they meet at grid barriers).
@@ -867,7 +874,7 @@ cudaError_t launch_round(const TmSet& tm, const RoundArgs& a, int grid, size_t s
   at[0].val.cooperative = 1;
   cfg.attrs = at;
   cfg.numAttrs = 1;
-  return cudaLaunchKernelEx(&cfg, k_round, tm, a);
+  return cudaLaunchKernelEx(&cfg, k_round<kRoundThreads>, tm, a);
 }
 
 }  // namespace dexk
