@@ -49,6 +49,22 @@ def measured_hbm_peak():
         return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
 
 
+def ncu_traffic_ratio():
+    """DRAM (read + write) bytes / algorithmic bytes of k_round from the committed `ncu --set full` capture
+    (profiles/k_round_r*_traffic.csv, newest round); None if absent."""
+    import csv
+    import glob
+    files = sorted(glob.glob(os.path.join(ROOT, "profiles", "k_round_r*_traffic.csv")))
+    if not files:
+        return None, None
+    dram = alg = 0.0
+    with open(files[-1]) as f:
+        for row in csv.DictReader(f):
+            dram += float(row["dram_read_bytes"]) + float(row["dram_write_bytes"])
+            alg += float(row["algorithmic_bytes"])
+    return (dram / alg if alg > 0 else None), os.path.relpath(files[-1], ROOT)
+
+
 # ------------------------------------------------------------------------------------------------
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
@@ -105,6 +121,28 @@ class ClockSampler:
 # ------------------------------------------------------------------------------------------------
 def dist_env():
     return int(os.environ.get("RANK", 0)), int(os.environ.get("LOCAL_RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
+
+
+def replica_prompt_seq(rank):
+    """Multi-GPU = replicas only: rank r decodes its own independent sequence, drawn
+    from the workload's prompt seed with sequence id r.  No data-path collective exists."""
+    return int(rank)
+
+
+def max_over_ranks(ms, world, device=None):
+    """Device time of the slowest rank (the job's time); identity at world == 1."""
+    if world == 1:
+        return float(ms)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms], dtype=torch.float64, device=device if device is not None else "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_tokens_per_s(world, steps, tokens_per_step, ms_max):
+    """Whole-job throughput: tokens committed by ALL ranks / time of the slowest rank."""
+    return world * steps * tokens_per_step / (ms_max * 1e-3)
 
 
 def run_rounds(g, T, flags):
@@ -164,7 +202,7 @@ def bench_dex(args):
     # the prompt lives in PINNED host memory: dex_prefill copies it to the device inside the e2e region
     prompt_pin = torch.empty(n_prompt, dtype=torch.int32).pin_memory()
     prompt = prompt_pin.numpy()
-    prompt[:] = dex_synth.make_prompt(shape.vocab, n_prompt, wl.prompt_seed, seq=rank)
+    prompt[:] = dex_synth.make_prompt(shape.vocab, n_prompt, wl.prompt_seed, seq=replica_prompt_seq(rank))
     max_ctx = n_prompt + T + 8
     FL = P.DEX_STEP_AUTOCOLLAPSE
     g = P.Dex(shape, w_dev, X, max_ctx=max_ctx, device=dev, act_planes=args.act_planes)
@@ -178,12 +216,8 @@ def bench_dex(args):
             dist.barrier()
             torch.cuda.synchronize()
 
-    def max_over_ranks(ms):
-        if world == 1:
-            return ms
-        t = torch.tensor([ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+    def max_ranks(ms):
+        return max_over_ranks(ms, world, dev)
 
     # ---- warm-up (>= 3 steps), also captures the CUDA graphs ----
     W = max(3, args.warmup)
@@ -203,9 +237,9 @@ def bench_dex(args):
     barrier()
     clk = clocks.stop()
     _, counters = g.profile(-1)
-    ms = max_over_ranks(ms)
+    ms = max_ranks(ms)
     dex_tokens = g.tokens()[n_prompt:n_prompt + T].copy()
-    value = world * args.steps * T / (ms * 1e-3)
+    value = job_tokens_per_s(world, args.steps, T, ms)
 
     # ---- same-kernel AR baseline (X = {L}) ----
     a.profile(0)
@@ -213,9 +247,9 @@ def bench_dex(args):
     ms_ar, (rounds_ar, _, _, _) = time_steps(torch, a, n_prompt, T, args.steps, FL)
     barrier()
     _, counters_ar = a.profile(-1)
-    ms_ar = max_over_ranks(ms_ar)
+    ms_ar = max_ranks(ms_ar)
     ar_tokens = a.tokens()[n_prompt:n_prompt + T].copy()
-    ar_value = world * args.steps * T / (ms_ar * 1e-3)
+    ar_value = job_tokens_per_s(world, args.steps, T, ms_ar)
     lossless = bool(np.array_equal(dex_tokens, ar_tokens))
 
     # ---- e2e: host prompt -> dex_prefill -> rounds -> dex_get_tokens (host), per step ----
@@ -231,7 +265,7 @@ def bench_dex(args):
     e1.record(g.stream)
     barrier()
     wall_ms = (time.perf_counter() - t0) * 1e3
-    ms_e2e = max_over_ranks(max(e0.elapsed_time(e1), 0.0))
+    ms_e2e = max_ranks(max(e0.elapsed_time(e1), 0.0))
     assert np.array_equal(out[n_prompt:], dex_tokens)
     res_bytes = __import__("ctypes").sizeof(P.DexStepResult)
     e2e = {"value": world * args.steps * T / (ms_e2e * 1e-3), "unit": UNIT,
@@ -253,9 +287,13 @@ def bench_dex(args):
         ph, ct = g.profile(0)
         k_us, k_launches, k_bytes = ph[1], ct[2], ct[3] + ct[4] + ct[5]
         ach = k_bytes / (k_us * 1e-6) / 1e9
+        ratio, ratio_src = ncu_traffic_ratio()
         roofline = {"kernel": "k_round (persistent round kernel: segment GEMMs + glue + lattice attention + fused exit)",
                     "bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
-                    "frac_of_8TBs": ach / NOMINAL_HBM_GBS, "peak_source": peak_src, "traffic": None,
+                    "frac_of_8TBs": ach / NOMINAL_HBM_GBS, "peak_source": peak_src,
+                    "traffic": (ratio * k_bytes / max(1, k_launches)) if ratio else None,
+                    "traffic_source": (f"dram read+write / algorithmic = {ratio:.4f} from {ratio_src} (ncu --set full), "
+                                       "x algorithmic bytes per launch") if ratio else None,
                     "launches": int(k_launches), "avg_launch_us": k_us / max(1, k_launches),
                     "algorithmic_bytes_per_launch": k_bytes / max(1, k_launches),
                     "share_of_step": k_us / max(1e-9, ph[7] if ph[7] > 0 else sum(ph[:6])),
