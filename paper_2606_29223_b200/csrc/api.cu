@@ -80,6 +80,7 @@ struct dex_ctx {
   TmSet tms;
   RingCfg round_ring;
   int round_attn_off;
+  bool round_ok;                      // the round kernel's ring + attention scratch fit shared memory
   std::map<long long, cudaGraphExec_t> graphs;
   std::string err;
   // phase timing (taps only)
@@ -160,7 +161,7 @@ void split_fine(OpDesc& o, bool allow_split) {
 
 // Shape-only quantities shared by dex_workspace_bytes and dex_init.
 struct Layout {
-  int N, R_dec, R_cap, max_chunks, n_slots, n_nodes, pages_per_seq, n_pages, max_len, ref_tiles;
+  int N, R_dec, R_cap, exit_chunk, max_chunks, n_slots, n_nodes, pages_per_seq, n_pages, max_len, ref_tiles;
   Plan dec, pre, ext;
   OpCfg op[5];
   size_t part_floats;
@@ -196,10 +197,13 @@ void make_layout(const dex_config& c, const int32_t* depths, int n, Layout& L) {
   L.pre.rows_cap[0] = kPrefillRows;
   L.pre.layer_lo[0] = 0;
   L.pre.layer_len[0] = c.n_layers;
-  L.ext.n_grp = (L.R_dec + 255) / 256;
+  // exit-head groups: chunks of the largest decode group's size, so the exit op fits the decode ring geometry
+  // (the LM head is streamed once per chunk: 2 chunks at N = 8, where all rows = 2 x the stage-0 rows)
+  L.exit_chunk = std::min(256, round16i(L.dec.rows_cap[0]));
+  L.ext.n_grp = (L.R_dec + L.exit_chunk - 1) / L.exit_chunk;
   for (int g = 0; g < L.ext.n_grp; ++g) {
-    L.ext.row_base[g] = 256 * g;
-    L.ext.rows_cap[g] = std::min(256, L.R_dec - 256 * g);
+    L.ext.row_base[g] = L.exit_chunk * g;
+    L.ext.rows_cap[g] = std::min(L.exit_chunk, L.R_dec - L.exit_chunk * g);
     L.ext.layer_lo[g] = 0;
     L.ext.layer_len[g] = 1;
   }
@@ -424,7 +428,7 @@ int enqueue_step(dex_ctx* c, uint32_t flags, int n_chunks) {
   CU(c, launch_gather_norm(D, c->dec_plan, D.R_dec, c->stream));
   ph_end(c, PH_BOOK);
   int rc;
-  if (c->cfg.round_kernel && !c->phase_split) {
+  if (c->cfg.round_kernel && c->round_ok && !c->phase_split) {
     rc = enqueue_round(c, n_chunks);
     if (rc) return rc;
   } else {
@@ -486,7 +490,7 @@ void account_round(dex_ctx* c) {
     (void)any;
     gemm_launches += 4;
   }
-  const bool mega = c->cfg.round_kernel && !c->phase_split;
+  const bool mega = c->cfg.round_kernel && c->round_ok && !c->phase_split;
   c->counters[0] += 1;
   c->counters[1] += mega ? 7.0 : 2 + 10.0 * D.max_len + 1 + 1 + 3;
   c->counters[2] += mega ? 1 : gemm_launches;
@@ -575,7 +579,7 @@ int32_t dex_init(dex_ctx** out, const dex_config* cfg, const dex_weights* w, con
   for (int i = 0; i < n_depths; ++i) D.depths[i] = depths[i];
   D.max_seqs = cfg->max_seqs; D.max_ctx = cfg->max_ctx; D.page_size = cfg->page_size;
   D.pages_per_seq = L.pages_per_seq; D.n_pages = L.n_pages; D.n_slots = L.n_slots; D.n_nodes = L.n_nodes;
-  D.R_cap = L.R_cap; D.R_dec = L.R_dec; D.decs = cfg->decs; D.planes = cfg->act_planes; D.taps = cfg->debug_taps;
+  D.R_cap = L.R_cap; D.R_dec = L.R_dec; D.exit_chunk = L.exit_chunk; D.decs = cfg->decs; D.planes = cfg->act_planes; D.taps = cfg->debug_taps;
   D.max_len = L.max_len; D.max_chunks = L.max_chunks; D.ref_tiles = L.ref_tiles;
   D.embed = static_cast<const __nv_bfloat16*>(w->embed);
   D.lm_head = static_cast<const __nv_bfloat16*>(w->lm_head);
@@ -611,6 +615,7 @@ int32_t dex_init(dex_ctx** out, const dex_config* cfg, const dex_weights* w, con
     const size_t stage = 16384 + (size_t)cfg->act_planes * c->round_ring.x_cap * 128;
     const size_t attn = (round_attn_smem(cfg->head_dim) + 1023) / 1024 * 1024;
     const size_t budget = 222 * 1024 - attn - 2048;
+    c->round_ok = budget / stage >= 3;                    // too few ring stages (very wide stages): per-op path
     c->round_ring.n_stages = (int)std::max<size_t>(2, std::min<size_t>(12, budget / stage));
     c->round_attn_off = (int)((c->round_ring.n_stages * stage + 1023 + 512) / 1024 * 1024);
     c->round_ring.smem = c->round_attn_off + attn + 1024;

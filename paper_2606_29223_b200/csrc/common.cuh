@@ -80,6 +80,7 @@ struct Dev {
   int n_nodes;             // 2^N - 1
   int R_cap;               // rows of every row-indexed buffer
   int R_dec;               // rows used by the decode plan
+  int exit_chunk;          // rows per exit-head group (= largest decode group, rounded to 16: the exit shares the ring)
   int decs, planes, taps;
   int max_len;             // max_m |Pi_m|
   // weights

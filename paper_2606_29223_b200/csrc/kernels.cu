@@ -92,7 +92,7 @@ __global__ void k_rows_decode(Dev D, Plan plan) {
       D.grp_nb[m] = round16(ext);
     }
     for (int c = 0; c < kMaxGrp; ++c) {
-      int e = min(256, max_end - 256 * c);
+      int e = min(D.exit_chunk, max_end - D.exit_chunk * c);
       D.exit_nb[c] = e > 0 ? round16(e) : 0;
     }
   }
