@@ -57,6 +57,27 @@ __device__ __forceinline__ float4 r_sum4(const float* p, int S, size_t stride) {
   for (int s = 1; s < S; ++s) acc = r_add4(acc, r_ld4(p + (size_t)s * stride));
   return acc;
 }
+// NV float4 split-K sums at once: the loads of up to 8 splits of all NV values are issued together (one
+// round trip), then added in split order (H3).
+template <int NV, int NB = 8>
+__device__ __forceinline__ void r_sum4_batch(const float* const (&p)[NV], int S, size_t stride, float4 (&out)[NV]) {
+#pragma unroll
+  for (int v = 0; v < NV; ++v) out[v] = make_float4(0.f, 0.f, 0.f, 0.f);
+  for (int s0 = 0; s0 < S; s0 += NB) {
+    float4 t[NB][NV];
+#pragma unroll
+    for (int i = 0; i < NB; ++i)
+#pragma unroll
+      for (int v = 0; v < NV; ++v)
+        t[i][v] = (s0 + i < S) ? r_ld4(p[v] + (size_t)(s0 + i) * stride) : make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+    for (int i = 0; i < NB; ++i)
+      if (s0 + i < S) {
+#pragma unroll
+        for (int v = 0; v < NV; ++v) out[v] = r_add4(out[v], t[i][v]);
+      }
+  }
+}
 __device__ __forceinline__ float r_sum1(const float* p, int S, size_t stride) {
   float acc = p[0];
 #pragma unroll 8
@@ -202,14 +223,21 @@ __device__ void glue_add_norm(const RoundArgs& a, int j, int mode, const OpDesc&
   const int n_seg = (D.d + 127) / 128;
   for (int u = gw; u < D.R_dec * n_seg; u += n_gw) {
     const int r = u / n_seg, seg = u - r * n_seg;
+    // the row table, x and the partials are loaded together (addresses depend on r only); w needs the layer
     const RowInfo* ri = &D.rows[r];
-    if (!ri->valid) continue;
-    const int grp = ri->grp;
+    const int valid = ri->valid, grp = ri->grp;
+    const int i = seg * 128 + lane * 4;
+    const bool in = i < D.d;
+    float* x = D.x_cur + (size_t)r * D.d + (in ? i : 0);
+    const float4 xv = r_ld4(x);
+    const float* const pp[1] = {D.part + (size_t)r * op.part_ld + (in ? i : 0)};
+    float4 sv[1];
+    r_sum4_batch<1, 12>(pp, op.ksplit, op.split_stride, sv);
+    if (!valid) continue;
     if (j >= a.dec.layer_len[grp]) continue;
     const int layer = a.dec.layer_lo[grp] + j;
-    const int i = seg * 128 + lane * 4;
     float ss = 0.f;
-    if (i < D.d) {
+    if (in) {
       const float* w;
       __nv_bfloat16* dst = D.act_a;
       if (mode == 0) {
@@ -220,9 +248,8 @@ __device__ void glue_add_norm(const RoundArgs& a, int j, int mode, const OpDesc&
         w = D.norm_final;
         dst = D.act_e;
       }
-      float* x = D.x_cur + (size_t)r * D.d + i;
-      const float4 xv = r_ld4(x), wv = r_ld4(w + i);
-      const float4 s4 = r_sum4(D.part + (size_t)r * op.part_ld + i, op.ksplit, op.split_stride);
+      const float4 wv = r_ld4(w + i);
+      const float4 s4 = sv[0];
       const float4 v = r_add4(xv, s4);
       *reinterpret_cast<float4*>(x) = v;
       ss = v.x * v.x + v.y * v.y + v.z * v.z + v.w * v.w;
@@ -243,14 +270,18 @@ __device__ void glue_silu(const RoundArgs& a, int j, const OpDesc& op, int gw, i
   const size_t ps = (size_t)D.R_cap * D.ffn;
   for (int u = gw; u < D.R_dec * nblk; u += n_gw) {
     const int r = u / nblk, b = u - r * nblk;
-    const RowInfo* ri = &D.rows[r];
-    if (!ri->valid || j >= a.dec.layer_len[ri->grp]) continue;
     const int i = b * 128 + lane * 4;
     if (i >= D.ffn) continue;
+    // the row table, the deferred norm scale and the partials are loaded together (addresses depend on r only)
+    const RowInfo* ri = &D.rows[r];
+    const int valid = ri->valid, grp = ri->grp;
     const float* p = D.part + (size_t)r * op.part_ld;
+    const float* const pp[2] = {p + i, p + D.ffn + i};
+    float4 gu[2];
+    r_sum4_batch<2>(pp, op.ksplit, op.split_stride, gu);
     const float inv = inv_rms(D, r);
-    float4 g = r_sum4(p + i, op.ksplit, op.split_stride);
-    float4 up = r_sum4(p + D.ffn + i, op.ksplit, op.split_stride);
+    if (!valid || j >= a.dec.layer_len[grp]) continue;
+    float4 g = gu[0], up = gu[1];
     g.x *= inv; g.y *= inv; g.z *= inv; g.w *= inv;
     up.x *= inv; up.y *= inv; up.z *= inv; up.w *= inv;
     float4 o;
