@@ -255,7 +255,7 @@ void make_layout(const dex_config& c, const int32_t* depths, int n, Layout& L) {
   sz[B_ACTE] = 2 * P * R * c.d_model;
   sz[B_PART] = sizeof(float) * L.part_floats;
   sz[B_QBUF] = sizeof(float) * R * c.n_heads * c.head_dim;
-  sz[B_APART] = sizeof(float) * R * c.n_heads * (size_t)L.max_chunks * (c.head_dim + 2);
+  sz[B_APART] = sizeof(float) * R * c.n_heads * (size_t)L.max_chunks * 4 * (c.head_dim + 2);   // k_round: 4 sub-partials per chunk
   sz[B_ROPE] = sizeof(float2) * (size_t)(c.max_ctx + kMaxAnc + 1) * (c.head_dim / 2);
   sz[B_TAPH] = c.debug_taps ? sizeof(float) * R * (size_t)L.max_len * c.d_model : 0;
   sz[B_DBG] = sizeof(float) * L.dbg_floats;

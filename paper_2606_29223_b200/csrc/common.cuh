@@ -106,7 +106,7 @@ struct Dev {
   float* part;             // split-K partial sums, per op [S_op][R_cap][ld_op] (OpDesc)
   unsigned int* gbar;      // grid-barrier arrival counter of the round kernel (reset every round)
   float* qbuf;             // [R_cap][nh*hd]
-  float* attn_part;        // [R_cap][nh][max_chunks][hd + 2]
+  float* attn_part;        // [R_cap][nh][4 * max_chunks][hd + 2]: (o, max, sum) per 16 positions (k_round) / per chunk (k_attn)
   int max_chunks;
   float2* rope;            // [max_ctx + kMaxAnc + 1][hd/2] (cos, sin)
   unsigned long long* best_key;   // [R_cap]

@@ -305,28 +305,21 @@ __device__ __forceinline__ void cvt_bf16x16(const uint4& u0, const uint4& u1, fl
 }
 __device__ __forceinline__ float bf16_rt(float v) { return __bfloat162float(__float2bfloat16_rn(v)); }
 
-// Merge the per-chunk partials of (row, head) in ascending chunk order (fixed order: H3) -> act_o planes.
-// Blocks of 16 chunks are loaded in one batch (a dependent load costs microseconds under the weight stream).
+// Merge the sub-partials of (row, head) - one per 16 positions - in ascending position order (fixed order: H3)
+// -> act_o planes.  One pass with a running maximum; blocks of 16 sub-partials are loaded in one batch (a
+// dependent load costs microseconds under the weight stream).
 template <int HD>
-__device__ __forceinline__ void attn_merge(const Dev& D, int r, int h, int nc, int lane) {
+__device__ __forceinline__ void attn_merge(const Dev& D, int r, int h, int n_sub, int lane) {
   constexpr int DPL = HD / 32;
-  const float* src = D.attn_part + ((size_t)r * D.nh + h) * D.max_chunks * (HD + 2);
-  float M = -INFINITY;
-  for (int cb = 0; cb < nc; cb += 16) {
-    float mv[16];
-#pragma unroll
-    for (int i = 0; i < 16; ++i) mv[i] = (cb + i < nc) ? __ldcg(src + (size_t)(cb + i) * (HD + 2) + HD) : -INFINITY;
-#pragma unroll
-    for (int i = 0; i < 16; ++i) M = fmaxf(M, mv[i]);
-  }
-  float num[DPL], den = 0.f;
+  const float* src = D.attn_part + ((size_t)r * D.nh + h) * (size_t)(D.max_chunks * 4) * (HD + 2);
+  float M = -INFINITY, den = 0.f, num[DPL];
 #pragma unroll
   for (int t = 0; t < DPL; ++t) num[t] = 0.f;
-  for (int cb = 0; cb < nc; cb += 16) {
+  for (int cb = 0; cb < n_sub; cb += 16) {
     float mv[16], lv[16], ov[16][DPL];
 #pragma unroll
     for (int i = 0; i < 16; ++i) {
-      const bool on = cb + i < nc;
+      const bool on = cb + i < n_sub;
       const float* sc = src + (size_t)(cb + i) * (HD + 2);
       mv[i] = on ? __ldcg(sc + HD) : -INFINITY;
       lv[i] = on ? __ldcg(sc + HD + 1) : 0.f;
@@ -335,12 +328,18 @@ __device__ __forceinline__ void attn_merge(const Dev& D, int r, int h, int nc, i
     }
 #pragma unroll
     for (int i = 0; i < 16; ++i) {
-      if (cb + i < nc) {
-        const float w = expf(mv[i] - M);
+      if (mv[i] == -INFINITY) continue;                      // absent, or a tile without visible positions
+      if (mv[i] > M) {
+        const float sc = expf(M - mv[i]);                    // exp(-inf) = 0 on the first one
+        den *= sc;
 #pragma unroll
-        for (int t = 0; t < DPL; ++t) num[t] = fmaf(w, ov[i][t], num[t]);
-        den = fmaf(w, lv[i], den);
+        for (int t = 0; t < DPL; ++t) num[t] *= sc;
+        M = mv[i];
       }
+      const float w = expf(mv[i] - M);
+#pragma unroll
+      for (int t = 0; t < DPL; ++t) num[t] = fmaf(w, ov[i][t], num[t]);
+      den = fmaf(w, lv[i], den);
     }
   }
   const int K = D.nh * HD;
@@ -416,23 +415,31 @@ __device__ void glue_qkv_finalize(const RoundArgs& a, int j, int gw, int n_gw, i
   }
 }
 
-// Phase A.  Task (one CTA's epilogue group) = (stage m, sequence s, KV head g, range of 64-position chunks of
-// ABSOLUTE position); the range length is chosen so that the live tasks about fill the grid.  Per task the
-// committed K/V of each chunk is staged in shared memory with cp.async (double buffered) and applied to every
-// (row, query head) pair of (m, s, g).  The four warps split the chunk's positions (16 each): LP lanes share a
-// position (two 8-dim pieces each: conflict-free 16-byte shared loads); fp32 scores, warp-shuffle softmax over
-// the warp's 16 positions, then the four sub-partials are merged in warp order into the chunk's (o, max, sum).
-// Positions >= n_paged are the row's private suffix - ancestor slots and its own slot, read from global memory:
-// the "ancestry mask" of north_star (b).  When all chunks of (row, head) are written, the last writer merges
-// them in ascending chunk order.  A position contributes the same bits wherever its K/V lives (slot before
-// commit, page after) and whatever else shares the task: DEX stream == AR stream (H3).
-constexpr int kAttnPairs = 8;        // pairs per pass of a task
+// Phase A.  Task (one CTA's glue group) = (stage m, sequence s, KV head g, range of 64-position chunks of
+// ABSOLUTE position).  The committed K/V of each chunk is staged in shared memory with cp.async (128-bit,
+// double buffered, 16-byte pieces XOR-swizzled by row) and applied to up to 16 (row, query head) pairs of
+// (m, s, g) at once on the tensor cores (mma.sync m16n8k16, bf16 x bf16 -> fp32):
+//   S^T[pair][pos] = Q[pair][:] . K[pos][:]   A = q as bf16 hi + lo (two MMAs: fp32-grade products, R23),
+//                                             B = K rows straight from the staged tile (ldmatrix)
+//   softmax over the warp's 16 positions      fp32, in the accumulator fragment (quad shuffles)
+//   O[pair][dim]  = P[pair][pos] . V[pos][:]  A = P as bf16 hi + lo (the score fragment IS the A fragment),
+//                                             B = V rows (ldmatrix.trans)
+// Warp w of the first four handles positions [16w, 16w+16) of the chunk and writes one (o, max, sum)
+// sub-partial per pair.  Positions >= n_paged are a row's private suffix - its ancestor slots and its own
+// slot, the "ancestry mask" of north_star (b): for the chunk(s) that hold them the rows are processed one
+// lattice row at a time, after that row's private K/V rows are patched into the staged tile at their
+// positions.  Every position therefore goes through the same instructions wherever its K/V lives (slot before
+// commit, page after) and whatever else shares the MMA: DEX stream == AR stream (H3).  When all chunks of
+// (row, head) are written, the last writer merges the sub-partials in ascending position order.
+constexpr int kAttnPairs = 16;       // pairs per pass of a task (the M of the MMAs)
 
 template <int HD>
 struct AttnSmem {
-  __nv_bfloat16 kv[2][2][kChunk * HD];          // [buffer][K / V][row][dim]
-  float q[kAttnPairs][HD];
-  float xch[4][kAttnPairs][HD + 2];             // per warp: (o, max, sum) over its 16 positions
+  __nv_bfloat16 kv[2][2][kChunk * HD];          // [buffer][K / V][row][dim], 16-byte pieces swizzled: j ^ (row & 7)
+  __nv_bfloat16 qh[kAttnPairs][HD + 8];         // q hi / lo planes (row stride padded: conflict-free fragment loads)
+  __nv_bfloat16 ql[kAttnPairs][HD + 8];
+  int ppos[kAttnPairs];                         // position of the pair's row; -1: not in this pass
+  int prow[kAttnPairs], phead[kAttnPairs];
 };
 
 __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc) {
@@ -442,118 +449,173 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
 
-// Sub-partial of one pair over the 16 positions [c0 + 16*w, +16) of a chunk, by warp w.
+__device__ __forceinline__ void ldsm_x4(uint32_t addr, uint32_t (&r)[4]) {
+  asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0, %1, %2, %3}, [%4];\n"
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(addr));
+}
+__device__ __forceinline__ void ldsm_x4_t(uint32_t addr, uint32_t (&r)[4]) {
+  asm volatile("ldmatrix.sync.aligned.m8n8.x4.trans.shared.b16 {%0, %1, %2, %3}, [%4];\n"
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(addr));
+}
+__device__ __forceinline__ void mma_bf16(float (&d)[4], const uint32_t (&a)[4], uint32_t b0, uint32_t b1) {
+  asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0, %1, %2, %3}, {%4, %5, %6, %7}, {%8, %9}, {%0, %1, %2, %3};\n"
+               : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3])
+               : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
+}
+__device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
+  const __nv_bfloat162 v = __floats2bfloat162_rn(lo, hi);
+  return *reinterpret_cast<const uint32_t*>(&v);
+}
+
+// Positions [c0 + 16*t, +16) of the staged chunk against the pass's pairs [p_lo, p_hi): one sub-partial per pair.
+// kbase / vbase: shared-memory tiles whose row `row0 + i` holds position c*64 + 16*t + i.
 template <int HD>
-__device__ __forceinline__ void attn_sub(const Dev& D, const RowInfo* ri, int g, int c0, int w, int layer,
-                                         const __nv_bfloat16* kbuf, const __nv_bfloat16* vbuf, const float* sq, float* out,
-                                         int lane) {
-  constexpr int LP = HD / 16, PI = 32 / LP, WIT = 16 / PI, HH = HD / 2;
-  const int pos = ri->pos, s = ri->seq, n_paged = ri->n_paged, n_anc = ri->n_anc;
-  const int sub = lane % LP, pg = lane / LP;
-  const int da = sub * 8, db = HH + sub * 8;                // this lane's two 8-dim pieces
+__device__ __forceinline__ void attn_tile(const Dev& D, AttnSmem<HD>* sm, uint32_t kbase, uint32_t vbase, int row0, int c, int t,
+                                          int p_lo, int p_hi, int lane) {
+  constexpr int KT = HD / 16, NT = HD / 8;
+  const int c0 = c * kChunk;
+  const int rq = lane >> 2, cq = (lane & 3) * 2;            // fragment row (pair) / column offset of this lane
+  // ---- S^T = Q . K^T over the head dim
+  // four independent accumulator chains per position half (q hi / lo planes x even / odd k-tiles), added in a
+  // fixed order afterwards: a dependent mma.sync costs ~35 cycles
+  float S[2][4], Sx[2][3][4];
+#pragma unroll
+  for (int j = 0; j < 2; ++j)
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+      S[j][e] = 0.f;
+      Sx[j][0][e] = Sx[j][1][e] = Sx[j][2][e] = 0.f;
+    }
+  const int krow = row0 + (lane & 7) + ((lane >> 4) << 3);   // ldmatrix row of this lane: matrices 0,1 -> rows 0-7, 2,3 -> 8-15
+  const int khalf = (lane >> 3) & 1;                           // matrices 1,3: second 16-byte piece of the k-tile
+#pragma unroll
+  for (int kt = 0; kt < KT; ++kt) {
+    uint32_t ah[4], al[4], b[4];
+    ah[0] = *reinterpret_cast<const uint32_t*>(&sm->qh[rq][kt * 16 + cq]);
+    ah[1] = *reinterpret_cast<const uint32_t*>(&sm->qh[rq + 8][kt * 16 + cq]);
+    ah[2] = *reinterpret_cast<const uint32_t*>(&sm->qh[rq][kt * 16 + 8 + cq]);
+    ah[3] = *reinterpret_cast<const uint32_t*>(&sm->qh[rq + 8][kt * 16 + 8 + cq]);
+    al[0] = *reinterpret_cast<const uint32_t*>(&sm->ql[rq][kt * 16 + cq]);
+    al[1] = *reinterpret_cast<const uint32_t*>(&sm->ql[rq + 8][kt * 16 + cq]);
+    al[2] = *reinterpret_cast<const uint32_t*>(&sm->ql[rq][kt * 16 + 8 + cq]);
+    al[3] = *reinterpret_cast<const uint32_t*>(&sm->ql[rq + 8][kt * 16 + 8 + cq]);
+    const int piece = (kt * 2 + khalf) ^ (krow & 7);
+    ldsm_x4(kbase + (krow * HD + piece * 8) * 2, b);           // b[0],b[1]: positions 0-7 of the tile; b[2],b[3]: 8-15
+    if (kt & 1) {
+      mma_bf16(Sx[0][1], ah, b[0], b[1]);
+      mma_bf16(Sx[0][2], al, b[0], b[1]);
+      mma_bf16(Sx[1][1], ah, b[2], b[3]);
+      mma_bf16(Sx[1][2], al, b[2], b[3]);
+    } else {
+      mma_bf16(S[0], ah, b[0], b[1]);
+      mma_bf16(Sx[0][0], al, b[0], b[1]);
+      mma_bf16(S[1], ah, b[2], b[3]);
+      mma_bf16(Sx[1][0], al, b[2], b[3]);
+    }
+  }
+#pragma unroll
+  for (int j = 0; j < 2; ++j)
+#pragma unroll
+    for (int e = 0; e < 4; ++e) S[j][e] = (S[j][e] + Sx[j][1][e]) + (Sx[j][0][e] + Sx[j][2][e]);
+  // ---- mask, scale, softmax over the tile's 16 positions (fragment rows rq and rq + 8)
   const float scale = 1.0f / sqrtf((float)HD);
-  float qf[16];
+  const int pos_a = (rq >= p_lo && rq < p_hi) ? sm->ppos[rq] : -1;
+  const int pos_b = (rq + 8 >= p_lo && rq + 8 < p_hi) ? sm->ppos[rq + 8] : -1;
+  float mx_a = -INFINITY, mx_b = -INFINITY;
 #pragma unroll
-  for (int e = 0; e < 8; ++e) {
-    qf[e] = sq[da + e];
-    qf[8 + e] = sq[db + e];
-  }
-  const int pl0 = 16 * w + pg;                               // + it * PI
-  const bool all_pool = c0 + 16 * w + 16 <= n_paged;        // warp-uniform fast path: every position committed
-  const size_t slot_g = (size_t)g * HD;
-  float sc[WIT];
+  for (int j = 0; j < 2; ++j)
 #pragma unroll
-  for (int it = 0; it < WIT; ++it) {
-    const int pl = pl0 + it * PI, pp = c0 + pl;
-    float kf[16];
-    if (all_pool || pp < n_paged) {
-      cvt_bf16x16(*reinterpret_cast<const uint4*>(kbuf + pl * HD + da), *reinterpret_cast<const uint4*>(kbuf + pl * HD + db), kf);
-    } else {
-      const int ai = pp - n_paged;
-      const int slot = (ai < n_anc) ? ri->anc[ai & (kMaxAnc - 1)] : ri->slot;   // pp > pos: any valid slot (masked below)
-      const __nv_bfloat16* kp = D.kslot + slot_off(D, s, slot, layer) + slot_g;
-      cvt_bf16x16(*reinterpret_cast<const uint4*>(kp + da), *reinterpret_cast<const uint4*>(kp + db), kf);
+    for (int e = 0; e < 4; ++e) {
+      const int pp = c0 + t * 16 + j * 8 + cq + (e & 1);
+      const int lim = (e < 2) ? pos_a : pos_b;
+      const float v = (pp <= lim) ? S[j][e] * scale : -INFINITY;
+      S[j][e] = v;
+      if (e < 2) mx_a = fmaxf(mx_a, v); else mx_b = fmaxf(mx_b, v);
     }
-    float acc = 0.f, acc2 = 0.f;
 #pragma unroll
-    for (int e = 0; e < 16; e += 2) {
-      acc = fmaf(qf[e], kf[e], acc);
-      acc2 = fmaf(qf[e + 1], kf[e + 1], acc2);
-    }
-    acc += acc2;
-#pragma unroll
-    for (int o = 1; o < LP; o <<= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
-    sc[it] = (pp <= pos) ? acc * scale : -INFINITY;
+  for (int o = 1; o < 4; o <<= 1) {
+    mx_a = fmaxf(mx_a, __shfl_xor_sync(0xffffffffu, mx_a, o));
+    mx_b = fmaxf(mx_b, __shfl_xor_sync(0xffffffffu, mx_b, o));
   }
-  float mx = sc[0];
+  float l_a = 0.f, l_b = 0.f;
+  uint32_t ph[4], pl[4];                                      // P as A fragments (hi / lo planes)
+  {
+    float p[2][4];
 #pragma unroll
-  for (int it = 1; it < WIT; ++it) mx = fmaxf(mx, sc[it]);
+    for (int j = 0; j < 2; ++j)
 #pragma unroll
-  for (int o = LP; o < 32; o <<= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
-  float lsum = 0.f;
+      for (int e = 0; e < 4; ++e) {
+        const float m = (e < 2) ? mx_a : mx_b;
+        const float v = (S[j][e] == -INFINITY) ? 0.f : expf(S[j][e] - m);
+        p[j][e] = v;
+        if (e < 2) l_a += v; else l_b += v;
+      }
 #pragma unroll
-  for (int it = 0; it < WIT; ++it) {
-    const float e = (sc[it] == -INFINITY) ? 0.f : expf(sc[it] - mx);   // mx = -inf only if every sc is -inf
-    sc[it] = e;
-    lsum += e;
-  }
-#pragma unroll
-  for (int o = LP; o < 32; o <<= 1) lsum += __shfl_xor_sync(0xffffffffu, lsum, o);
-  float of[16];
-#pragma unroll
-  for (int e = 0; e < 16; ++e) of[e] = 0.f;
-#pragma unroll
-  for (int it = 0; it < WIT; ++it) {
-    const int pl = pl0 + it * PI, pp = c0 + pl;
-    float vf[16];
-    if (all_pool || pp < n_paged) {
-      cvt_bf16x16(*reinterpret_cast<const uint4*>(vbuf + pl * HD + da), *reinterpret_cast<const uint4*>(vbuf + pl * HD + db), vf);
-    } else {
-      const int ai = pp - n_paged;
-      const int slot = (ai < n_anc) ? ri->anc[ai & (kMaxAnc - 1)] : ri->slot;
-      const __nv_bfloat16* vp = D.vslot + slot_off(D, s, slot, layer) + slot_g;
-      cvt_bf16x16(*reinterpret_cast<const uint4*>(vp + da), *reinterpret_cast<const uint4*>(vp + db), vf);
-    }
-    const float pr = sc[it];
-    if (pp <= pos) {
-#pragma unroll
-      for (int e = 0; e < 16; ++e) of[e] = fmaf(pr, vf[e], of[e]);
+    for (int j = 0; j < 2; ++j) {                             // a0a1 | a2a3 = positions 0-7 (rows rq | rq+8), a4a5 | a6a7 = 8-15
+      const float h0 = bf16_rt(p[j][0]), h1 = bf16_rt(p[j][1]), h2 = bf16_rt(p[j][2]), h3 = bf16_rt(p[j][3]);
+      ph[2 * j] = pack_bf16(h0, h1);
+      ph[2 * j + 1] = pack_bf16(h2, h3);
+      pl[2 * j] = pack_bf16(p[j][0] - h0, p[j][1] - h1);
+      pl[2 * j + 1] = pack_bf16(p[j][2] - h2, p[j][3] - h3);
     }
   }
 #pragma unroll
-  for (int e = 0; e < 16; ++e) {
-    float v = of[e];
-#pragma unroll
-    for (int o = LP; o < 32; o <<= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-    of[e] = v;
+  for (int o = 1; o < 4; o <<= 1) {
+    l_a += __shfl_xor_sync(0xffffffffu, l_a, o);
+    l_b += __shfl_xor_sync(0xffffffffu, l_b, o);
   }
-  if (pg == 0) {
+  // ---- O = P . V
+  float O[NT][4];
 #pragma unroll
-    for (int e = 0; e < 8; ++e) {
-      out[da + e] = of[e];
-      out[db + e] = of[8 + e];
-    }
+  for (int nt = 0; nt < NT; ++nt)
+#pragma unroll
+    for (int e = 0; e < 4; ++e) O[nt][e] = 0.f;
+  const int vrow = row0 + (lane & 7) + (((lane >> 3) & 1) << 3);   // matrices 0,2: positions 0-7; 1,3: 8-15
+  const int vsel = lane >> 4;                                        // matrices 2,3: the next 8-dim piece
+#pragma unroll
+  for (int nt = 0; nt < NT; nt += 2) {
+    uint32_t b[4];
+    const int piece = (nt + vsel) ^ (vrow & 7);
+    ldsm_x4_t(vbase + (vrow * HD + piece * 8) * 2, b);         // b[0],b[1]: dims nt*8..+8; b[2],b[3]: the next 8
+    mma_bf16(O[nt], ph, b[0], b[1]);
+    mma_bf16(O[nt], pl, b[0], b[1]);
+    mma_bf16(O[nt + 1], ph, b[2], b[3]);
+    mma_bf16(O[nt + 1], pl, b[2], b[3]);
   }
-  if (lane == 0) {
-    out[HD] = mx;
-    out[HD + 1] = lsum;
+  // ---- one (o, max, sum) sub-partial per pair: sub index = 4*c + t
+  const size_t sub = (size_t)(c * 4 + t) * (HD + 2);
+  if (pos_a >= c0 + t * 16) {                                 // the row sees this tile
+    float* dst = D.attn_part + ((size_t)sm->prow[rq] * D.nh + sm->phead[rq]) * (size_t)(D.max_chunks * 4) * (HD + 2) + sub;
+#pragma unroll
+    for (int nt = 0; nt < NT; ++nt) *reinterpret_cast<float2*>(dst + nt * 8 + cq) = make_float2(O[nt][0], O[nt][1]);
+    if ((lane & 3) == 0) { dst[HD] = mx_a; dst[HD + 1] = l_a; }
+  }
+  if (pos_b >= c0 + t * 16) {
+    float* dst = D.attn_part + ((size_t)sm->prow[rq + 8] * D.nh + sm->phead[rq + 8]) * (size_t)(D.max_chunks * 4) * (HD + 2) + sub;
+#pragma unroll
+    for (int nt = 0; nt < NT; ++nt) *reinterpret_cast<float2*>(dst + nt * 8 + cq) = make_float2(O[nt][2], O[nt][3]);
+    if ((lane & 3) == 0) { dst[HD] = mx_b; dst[HD + 1] = l_b; }
   }
 }
 
 template <int HD, int GT>
 __device__ void glue_attention(const RoundArgs& a, int j, int tid_e, int lane, int we, int cta, int G,
                                AttnSmem<HD>* sm, int n_live_ms) {
-  constexpr int kGlueWarps = GT / 32, kEpiThreads = GT;
   constexpr int CPR = HD / 8;                                // 16-byte pieces per K/V row
+  constexpr int kEpiThreads = GT;
   const Dev& D = a.D;
   const int n_msg = max(1, n_live_ms) * D.nkv;
   // chunks per task: one wave of tasks over the grid when a task then has <= 6 chunks (one-row rounds),
   // else fine-grained tasks of 3 chunks dealt round-robin (lattice rounds: many (stage, head) families)
+  // ranges of chunks per (stage, sequence, KV head): as many as fill the grid once.  With >= 2 ranges the LAST
+  // chunk (the one with the private positions, the per-row passes and usually the final merge) is a range of
+  // its own and the others share the rest; more families than CTAs: 3-chunk ranges dealt round-robin.
   const int nr_fit = G / n_msg;
-  const int cr_fit = nr_fit >= 1 ? (a.n_chunks + nr_fit - 1) / nr_fit : a.n_chunks;
-  const int CR = cr_fit <= 6 ? max(1, cr_fit) : 3;
-  const int n_ranges = (a.n_chunks + CR - 1) / CR;
-  const int team = we >> 2, quarter = we & 3;               // teams of four warps: team = pair, warp = position quarter
+  const bool tail_own = nr_fit >= 2 && a.n_chunks >= 2;
+  const int n_body = tail_own ? a.n_chunks - 1 : a.n_chunks;
+  const int nr_body = tail_own ? nr_fit - 1 : max(nr_fit, 1);
+  const int CR = nr_fit >= 1 ? max(1, (n_body + nr_body - 1) / nr_body) : 3;
+  const int n_ranges = (n_body + CR - 1) / CR + (tail_own ? 1 : 0);
   const int per_ms = D.nkv * n_ranges;
   const int n_tasks = D.N * D.max_seqs * per_ms;
   const int Gq = D.nh / D.nkv;
@@ -565,8 +627,9 @@ __device__ void glue_attention(const RoundArgs& a, int j, int tid_e, int lane, i
     const int g = rem / n_ranges, rg = rem - g * n_ranges;
     const SeqState st = D.seqs[s];
     if (!r_seq_live(st) || st.q < m || j >= a.dec.layer_len[m]) continue;
-    const int ca = rg * CR;
-    const int cb = min(min(ca + CR, a.n_chunks), (st.ctx_len + st.q) / kChunk + 1);   // no row lies beyond ctx_len + q
+    const bool is_tail = tail_own && rg == n_ranges - 1;
+    const int ca = is_tail ? n_body : rg * CR;
+    const int cb = min(is_tail ? a.n_chunks : min(ca + CR, n_body), (st.ctx_len + st.q) / kChunk + 1);   // no row lies beyond ctx_len + q
     if (ca >= cb) continue;
     const int cnt = r_stage_count(st.q, m);
     const int layer = a.dec.layer_lo[m] + j;
@@ -576,7 +639,6 @@ __device__ void glue_attention(const RoundArgs& a, int j, int tid_e, int lane, i
 
     for (int pb = 0; pb < n_pairs; pb += kAttnPairs) {
       const int np = min(kAttnPairs, n_pairs - pb);
-      // ---- chunks of the range: stage committed K/V (double buffered), every pair of the pass attends
       auto stage = [&](int c, int buf) {
         const int c0 = c * kChunk;
         const int n_rows = min(kChunk, n_paged - c0);        // committed rows of the chunk (one page: page_size % 64 == 0)
@@ -584,60 +646,94 @@ __device__ void glue_attention(const RoundArgs& a, int j, int tid_e, int lane, i
           const size_t base = page_off(D, s, layer, c0) + (size_t)g * HD;
           for (int id = tid_e; id < n_rows * CPR; id += kEpiThreads) {
             const int pl = id / CPR, cj = id - pl * CPR;
-            cp_async16(&sm->kv[buf][0][pl * HD + cj * 8], D.kpool + base + (size_t)pl * kv_stride + cj * 8);
-            cp_async16(&sm->kv[buf][1][pl * HD + cj * 8], D.vpool + base + (size_t)pl * kv_stride + cj * 8);
+            const int dj = (cj ^ (pl & 7)) * 8;
+            cp_async16(&sm->kv[buf][0][pl * HD + dj], D.kpool + base + (size_t)pl * kv_stride + cj * 8);
+            cp_async16(&sm->kv[buf][1][pl * HD + dj], D.vpool + base + (size_t)pl * kv_stride + cj * 8);
+          }
+        }
+        if (n_rows < kChunk) {                               // rows past the committed prefix: zeros (a masked position
+          const int z0 = max(n_rows, 0);                     // still enters the P.V MMA with weight 0: keep it finite)
+          for (int id = tid_e; id < (kChunk - z0) * CPR; id += kEpiThreads) {
+            const int pl = z0 + id / CPR, cj = id % CPR;
+            *reinterpret_cast<uint4*>(&sm->kv[buf][0][pl * HD + cj * 8]) = make_uint4(0u, 0u, 0u, 0u);
+            *reinterpret_cast<uint4*>(&sm->kv[buf][1][pl * HD + cj * 8]) = make_uint4(0u, 0u, 0u, 0u);
           }
         }
         cp_async_commit();
       };
       stage(ca, 0);
-      // ---- q of the pass's pairs (phase Q wrote it), in flight together with the first chunk
-      for (int id = tid_e; id < np * HD; id += kEpiThreads) {
+      // ---- q of the pass's pairs (phase Q wrote it) -> bf16 hi / lo planes, in flight together with the first chunk
+      for (int id = tid_e; id < kAttnPairs * HD; id += kEpiThreads) {
         const int pi = id / HD, t = id - pi * HD;
-        const int r = r0 + (pb + pi) / Gq, h = g * Gq + (pb + pi) % Gq;
-        sm->q[pi][t] = D.qbuf[((size_t)r * D.nh + h) * HD + t];
+        float v = 0.f;
+        if (pi < np) {
+          const int r = r0 + (pb + pi) / Gq, h = g * Gq + (pb + pi) % Gq;
+          v = D.qbuf[((size_t)r * D.nh + h) * HD + t];
+        }
+        const __nv_bfloat16 hi = __float2bfloat16_rn(v);
+        sm->qh[pi][t] = hi;
+        sm->ql[pi][t] = __float2bfloat16_rn(v - __bfloat162float(hi));
+      }
+      if (tid_e < kAttnPairs) {
+        const int pi = tid_e;
+        int pos = -1, r = 0, h = 0;
+        if (pi < np) {
+          r = r0 + (pb + pi) / Gq;
+          h = g * Gq + (pb + pi) % Gq;
+          pos = D.rows[r].pos;
+          if (pos < ca * kChunk) pos = -1;                   // the row ends before this range
+        }
+        sm->ppos[pi] = pos;
+        sm->prow[pi] = r;
+        sm->phead[pi] = h;
       }
       for (int c = ca; c < cb; ++c) {
         const int buf = (c - ca) & 1, c0 = c * kChunk;
         if (c + 1 < cb) stage(c + 1, buf ^ 1);
         else cp_async_commit();
         cp_async_wait<1>();
-        bar_epi<GT>();                                           // chunk c staged by all threads; q written
-        for (int pi = team; pi < np; pi += kGlueWarps / 4) {
-          const RowInfo* ri = &D.rows[r0 + (pb + pi) / Gq];
-          if (ri->pos < c0) continue;
-          attn_sub<HD>(D, ri, g, c0, quarter, layer, sm->kv[buf][0], sm->kv[buf][1], sm->q[pi], sm->xch[quarter][pi], lane);
-        }
-        bar_epi<GT>();                                           // sub-partials of all four warps written
-        for (int id = tid_e; id < np * HD; id += kEpiThreads) {
-          const int pi = id / HD, t = id - pi * HD;
-          const int r = r0 + (pb + pi) / Gq, h = g * Gq + (pb + pi) % Gq;
-          if (D.rows[r].pos < c0) continue;
-          float M = sm->xch[0][pi][HD];                      // finite: warp 0 holds position c0 <= pos
-#pragma unroll
-          for (int w = 1; w < 4; ++w) M = fmaxf(M, sm->xch[w][pi][HD]);
-          float num = 0.f, den = 0.f;
-#pragma unroll
-          for (int w = 0; w < 4; ++w) {                      // warp order (fixed: H3)
-            const float wgt = expf(sm->xch[w][pi][HD] - M);  // exp(-inf) = 0 for a warp without visible positions
-            num = fmaf(wgt, sm->xch[w][pi][t], num);
-            den = fmaf(wgt, sm->xch[w][pi][HD + 1], den);
+        bar_epi<GT>();                                         // chunk c staged by all threads; q planes written
+        {
+          const uint32_t kb = smem_u32(sm->kv[buf][0]), vb = smem_u32(sm->kv[buf][1]);
+          const int t_shared = max(0, min(4, (n_paged - c0) / 16));   // tiles whose 16 positions are all committed:
+          if (we < t_shared) attn_tile<HD>(D, sm, kb, vb, we * 16, c, we, 0, np, lane);   // every pair shares them
+          // tiles that hold private positions: warp t owns tile t of the staged chunk and takes the lattice rows one
+          // at a time, patching the row's ancestor / own K/V rows (from their slots) into the tile IN PLACE at their
+          // positions.  Rows above the row's own position keep finite data (zeros or an earlier row's patch): they
+          // are masked and enter the P.V MMA with weight 0.  No CTA-wide synchronisation: tiles are disjoint.
+          const int n_rl = (np + Gq - 1) / Gq;
+          if (we >= t_shared && we < 4) {
+            const int t = we, p0 = c0 + t * 16;
+            for (int rl = 0; rl < n_rl; ++rl) {
+              const int r = r0 + pb / Gq + rl;
+              const RowInfo* ri = &D.rows[r];
+              const int pos = ri->pos;
+              if (pos < p0) continue;                        // the row does not see this tile (warp-uniform)
+              const int i_lo = max(n_paged - p0, 0), i_hi = min(pos - p0, 15);
+              for (int id = lane; id < (i_hi - i_lo + 1) * CPR; id += 32) {
+                const int i = i_lo + id / CPR, cj = id % CPR, pl = t * 16 + i;
+                const int ai = p0 + i - n_paged;
+                const int slot = (ai < ri->n_anc) ? ri->anc[ai] : ri->slot;
+                const size_t so = slot_off(D, s, slot, layer) + (size_t)g * HD + cj * 8;
+                const int dj = (cj ^ (pl & 7)) * 8;
+                *reinterpret_cast<uint4*>(&sm->kv[buf][0][pl * HD + dj]) = *reinterpret_cast<const uint4*>(D.kslot + so);
+                *reinterpret_cast<uint4*>(&sm->kv[buf][1][pl * HD + dj]) = *reinterpret_cast<const uint4*>(D.vslot + so);
+              }
+              __syncwarp();
+              attn_tile<HD>(D, sm, kb, vb, t * 16, c, t, rl * Gq, min(np, (rl + 1) * Gq), lane);
+              __syncwarp();
+            }
           }
-          float* dst = D.attn_part + (((size_t)r * D.nh + h) * D.max_chunks + c) * (HD + 2);
-          dst[t] = num;
-          if (t == 0) {
-            dst[HD] = M;
-            dst[HD + 1] = den;
-          }
         }
-        bar_epi<GT>();                                           // kv buffer and xch free for the next chunk
+        bar_epi<GT>();                                         // kv buffer free for chunk c + 2
       }
-      // ---- all chunk partials of this pass are written: count them in; the last writer of (row, head) merges
+      // ---- all sub-partials of this pass are written: count the chunks in; the last writer of (row, head) merges
       __threadfence();
       bar_epi<GT>();
-      for (int pi = we; pi < np; pi += kGlueWarps) {
-        const int r = r0 + (pb + pi) / Gq, h = g * Gq + (pb + pi) % Gq;
-        const int pos = D.rows[r].pos;
+      for (int pi = we; pi < np; pi += GT / 32) {
+        const int pos = sm->ppos[pi];
+        if (pos < 0) continue;
+        const int r = sm->prow[pi], h = sm->phead[pi];
         const int mine = min(cb, pos / kChunk + 1) - ca;     // chunks of this range visible to the row
         if (mine <= 0) continue;
         const int nc = pos / kChunk + 1;
@@ -646,7 +742,7 @@ __device__ void glue_attention(const RoundArgs& a, int j, int tid_e, int lane, i
         old = __shfl_sync(0xffffffffu, old, 0);
         if (old + mine == nc) {
           __threadfence();
-          attn_merge<HD>(D, r, h, nc, lane);
+          attn_merge<HD>(D, r, h, pos / 16 + 1, lane);
           if (lane == 0) D.attn_cnt[r * D.nh + h] = 0;
         }
       }
