@@ -186,12 +186,12 @@ struct Walker {            // this CTA's items, in order
 };
 
 // ---------------------------------------------------------------- grid barrier (epilogue groups)
-// Every epilogue thread orders its generic-proxy global writes against later async-proxy (TMA) reads, the CTA
-// barrier collects them, and ONE thread publishes them gpu-wide (fence cumulativity, as in a cooperative-groups
-// grid sync), arrives, waits for all CTAs, and invalidates this SM's L1 (gpu-scope fence) before the group goes on.
+// Every glue thread orders its generic-proxy global writes against later async-proxy (TMA) reads; the CTA barrier
+// orders them before ONE thread's gpu-scope release (red.release: cumulative over what the barrier made visible to
+// it), which arrives on the counter; the same thread spins with gpu-scope acquire loads and the second CTA barrier
+// hands the acquired view to the group.  No separate fences: release / acquire + bar.sync compose in the PTX model.
 template <int GT>
 __device__ __forceinline__ void grid_bar(unsigned* gbar, unsigned target, int tid_e, volatile unsigned* s_seen, unsigned gb) {
-  __threadfence();
   fence_proxy_async();
   bar_epi<GT>();
   if (tid_e == 0) {
@@ -200,7 +200,6 @@ __device__ __forceinline__ void grid_bar(unsigned* gbar, unsigned target, int ti
     while (ld_acquire_u32(gbar) < target) {
       if (++spins > 400000000u) __trap();   // protocol bug: trap instead of hanging the box
     }
-    __threadfence();
     *s_seen = gb;                // the activation producer of this CTA learns of the barrier without polling L2
   }
   bar_epi<GT>();
