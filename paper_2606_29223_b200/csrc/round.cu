@@ -200,6 +200,7 @@ __device__ __forceinline__ void grid_bar(unsigned* gbar, unsigned target, int ti
     while (ld_acquire_u32(gbar) < target) {
       if (++spins > 400000000u) __trap();   // protocol bug: trap instead of hanging the box
     }
+    __threadfence_block();
     *s_seen = gb;                // the activation producer of this CTA learns of the barrier without polling L2
   }
   bar_epi<GT>();
@@ -727,8 +728,7 @@ __device__ void glue_attention(const RoundArgs& a, int j, int tid_e, int lane, i
         bar_epi<GT>();                                         // kv buffer free for chunk c + 2
       }
       // ---- all sub-partials of this pass are written: count the chunks in; the last writer of (row, head) merges
-      __threadfence();
-      bar_epi<GT>();
+      bar_epi<GT>();                                           // orders every warp's sub-partial stores before the counter's release
       for (int pi = we; pi < np; pi += GT / 32) {
         const int pos = sm->ppos[pi];
         if (pos < 0) continue;
@@ -737,11 +737,11 @@ __device__ void glue_attention(const RoundArgs& a, int j, int tid_e, int lane, i
         if (mine <= 0) continue;
         const int nc = pos / kChunk + 1;
         int old = 0;
-        if (lane == 0) old = atomicAdd(&D.attn_cnt[r * D.nh + h], mine);
+        if (lane == 0)                                         // release our sub-partials, acquire the other ranges'
+          asm volatile("atom.acq_rel.gpu.global.add.s32 %0, [%1], %2;\n" : "=r"(old) : "l"(&D.attn_cnt[r * D.nh + h]), "r"(mine) : "memory");
         old = __shfl_sync(0xffffffffu, old, 0);
         if (old + mine == nc) {
-          __threadfence();
-          attn_merge<HD>(D, r, h, pos / 16 + 1, lane);
+          attn_merge<HD>(D, r, h, pos / 16 + 1, lane);           // reads with ld.global.cg (L2)
           if (lane == 0) D.attn_cnt[r * D.nh + h] = 0;
         }
       }
@@ -854,7 +854,7 @@ __global__ void __launch_bounds__(kMaxThreads, 1) k_round(const __grid_constant_
             __nanosleep(32);
             if (++spins > 100000000u) __trap();
           }
-          __threadfence();
+          __threadfence_block();           // pairs with the cta-scope release before the flag store in grid_bar
           fence_proxy_async();
         }
         const int which = w.o.which;
