@@ -1,23 +1,23 @@
 // round.cu — k_round: ONE persistent kernel for the whole expand + exit part of a DEX round
 // (Alg. 1 lines 5-6): for every layer-step j all live stages run
-//   QKV GEMM -> RoPE + slot-KV write + lattice attention -> O GEMM + residual + RMSNorm ->
-//   gate/up GEMM -> SwiGLU -> down GEMM + residual + RMSNorm,
-// then the fused exit (final RMSNorm done by the last step, LM-head GEMM, DECS arg-max).
+//   QKV GEMM -> QKV finalize (scale, RoPE, slot-KV write) -> lattice attention -> O GEMM -> residual + norm operand ->
+//   gate/up GEMM -> SwiGLU -> down GEMM -> residual + norm operand,
+// then the fused exit (LM-head GEMM + DECS arg-max on the final-norm operand of every new row).
 //
 // Why one kernel: at <= 16 stacked rows every op is a pure HBM stream of its weights (5-30 us at
 // 7B), so launch boundaries and dependency bubbles, not bytes, set the speed.  Here one CTA per SM
-// stays resident; its TMA producer walks the round's whole (op, tile, K-split) item list and keeps
+// stays resident; its weight producer walks the round's whole (op, tile, K-split) item list and keeps
 // requesting weight tiles as far ahead as the shared-memory ring allows - weights do not depend on
 // activations - while the dependent part (activation boxes, MMAs, epilogue, glue) trails behind
 // grid-wide barriers.  The HBM stream therefore continues across op boundaries, glue phases and
 // the barrier latency itself.
 //
-//   warp 0      producer: weight tiles (always ahead) + activation boxes (after the op's inputs
-//               are published by a grid barrier)
-//   warp 1      tcgen05.mma issuer (one lane), owns TMEM (two accumulator stages)
-//   warps 2..5  epilogue group: TMEM -> split-K partials / exit arg-max, then the glue phase of
-//               the step (attention, combine, add+norm, SwiGLU) spread over all CTAs, then the
-//               grid barrier that publishes the next op's operand
+//   warp 0      weight producer (TMA, always ahead)
+//   warp 6      activation producer (TMA, after the grid barrier that publishes the op's operand)
+//   warp 1      tcgen05.mma issuer (one elected lane), owns TMEM (two accumulator stages)
+//   warps 2..5  GEMM epilogue: TMEM -> split-K partials / exit arg-max; then part of the glue group
+//   warps 2..5, 7..10  glue group: the step's glue phases (QKV finalize, attention, add+norm, SwiGLU) spread
+//               over all CTAs, each followed by the grid barrier that publishes the next op's operand
 //
 // Items are dealt round-robin to CTAs continuing across ops, so the per-op remainder rotates and
 // every CTA streams the same bytes per round to within one item.  The K split is fixed per

@@ -163,3 +163,40 @@ def test_fullsize_dex_equals_ar_counts_and_gemm(P, key, T):
     g.close()
     del wd
     torch.cuda.empty_cache()
+
+
+def test_c2_dex_short_run_against_fp32_oracle(P, c2):
+    """The lattice itself at the 7B shape against the oracle's Alg. 1 trace (8-token prompt, 2 commits): every new
+    node's stage-boundary hidden state (tolerance R16), its candidate token (a flip only at an oracle top-2
+    margin < 1e-2 of that node, R17), rows per stage / layer evaluations (bit-exact), the commit."""
+    import dex_synth
+    from oracle import OracleModel, dex_decode
+    wl, w = c2
+    om = OracleModel(wl.shape, w, dtype=np.float32, kv_round="bf16")
+    p = dex_synth.make_prompt(wl.shape.vocab, 8, 11)
+    T = 2
+    od = dex_decode(om, p, T, wl.depths, decs=True, trace=True)
+    g = P.Dex(wl.shape, w, wl.depths, max_ctx=128, debug_taps=1, use_graph=0)
+    g.prefill(0, p)
+    worst = 0.0
+    for ri, orec in enumerate(od["rounds"]):
+        r = g.step(0)[0]
+        assert r.q_before == orec["q"] and r.layer_evals == orec["layer_evals"]
+        assert list(r.rows_per_stage)[:len(wl.depths)] == orec["rows_per_stage"]
+        B = g.tap_B()
+        flipped = False
+        for node in orec["nodes"]:
+            h = g.tap_hidden(node)
+            o = orec["h_out"][node]
+            worst = max(worst, float(np.abs(h[-1] - o).max() / np.abs(o).max()))
+            if B[node] != orec["u"][node]:
+                assert orec["u_margin"][node] < 1e-2, (ri, node, orec["u_margin"][node])
+                flipped = True
+        if flipped:
+            break                                              # the lattices explore different candidates from here on
+        if orec["committed"]:
+            assert r.token == orec["token"] and r.match_k == orec["match_k"]
+            assert abs(r.ref_top1 - orec["ref_top1"]) < 5e-2
+            g.collapse(0, r.match_k, r.token)
+    assert worst < 2e-2, worst
+    g.close()
