@@ -194,6 +194,8 @@ def bench_dex(args):
     T = args.gen_len or wl.gen_len
     n_prompt = args.prompt_len or wl.prompt_len
     shape, X = wl.shape, wl.depths
+    if args.depths:                      # exploration-set sweep (resolution / single-exit ablation)
+        X = tuple(int(x) for x in args.depths.split(","))
     N, L = len(X), shape.n_layers
     w_host = dex_synth.make_weights(shape, wl.weight_seed, threads=16)
     w_dev = {k: v.to(device=dev, dtype=(torch.float32 if k.startswith("norm") else torch.bfloat16)).contiguous()
@@ -419,6 +421,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="dex", choices=["dex", "reference"])
     ap.add_argument("--workload", default="c2")
+    ap.add_argument("--depths", default="", help="comma-separated exploration set X (last = L); default: the workload's")
     ap.add_argument("--gen-len", type=int, default=0)
     ap.add_argument("--prompt-len", type=int, default=0)
     ap.add_argument("--act-planes", type=int, default=2)
