@@ -20,9 +20,11 @@ Parity pins (tests/test_oracle_*.py, all ``-m "not gpu"``):
   dex.py     Alg. 1, 2     node hidden == from-scratch forward of its own prefix;
                            losslessness; y == final-depth argmax
                            (PAPER.md:204); closed-form round / layer-eval counts
+  gumbel.py  Alg. 2 l.10-15  Gumbel-Max frequencies == softmax(l/tau) (chi-square), moments of the rows,
+                           sampled DEX stream == sampled AR stream for every X
 Nothing is "parity unpinned".
 """
 from .model import OracleModel, rmsnorm, bf16_round  # noqa: F401
-from .ar import ar_greedy  # noqa: F401
+from .ar import ar_greedy, ar_sample  # noqa: F401
 from .dex import dex_decode  # noqa: F401
-from . import ead, lattice  # noqa: F401
+from . import ead, gumbel, lattice  # noqa: F401

@@ -5,6 +5,7 @@ first input, so all T tokens come out of the same one-token loop (as they do for
 """
 import numpy as np
 
+from .gumbel import gumbel_row, perturbed
 from .model import argmax_lowest
 
 
@@ -55,4 +56,30 @@ def ar_greedy(model, prompt, T, keep_hidden=False, keep_logits=False, state=None
     out["tokens"] = np.array(out["tokens"], dtype=np.int64)
     out["exit_tokens"] = np.array(out["exit_tokens"], dtype=np.int64)
     out["state"] = (ck, cv)
+    return out
+
+
+def ar_sample(model, prompt, T, tau, seed, seq=0, state=None):
+    """Autoregressive SAMPLING with the Gumbel-Max rule and the shared counter-based noise of oracle/gumbel.py:
+    y_t = argmax_v (logits_L / tau + G[pos of y_t]).  Returns tokens [T] and the top-2 of the perturbed logits."""
+    prompt = list(int(t) for t in prompt)
+    ck, cv = state if state is not None else prefill(model, prompt)
+    toks = list(prompt)
+    out = dict(tokens=[], top1=[], top2=[])
+    V = model.lm_head.shape[0]
+    for _ in range(T):
+        pos = len(toks) - 1
+        x = model.embed_tok(toks[-1])
+        for l in range(model.L):
+            x, k, v = model.layer(l, x, pos, ck[l], cv[l])
+            ck[l].append(k)
+            cv[l].append(v)
+        z = perturbed(model.exit_logits(x), tau, gumbel_row(seed, seq, pos + 1, V))
+        y = argmax_lowest(z)
+        srt = np.sort(z)
+        out["tokens"].append(y)
+        out["top1"].append(float(srt[-1]))
+        out["top2"].append(float(srt[-2]))
+        toks.append(y)
+    out["tokens"] = np.array(out["tokens"], dtype=np.int64)
     return out

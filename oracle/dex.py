@@ -13,14 +13,16 @@ import numpy as np
 from . import lattice as lt
 from .ar import prefill
 from .ead import check_X
+from .gumbel import gumbel_row, perturbed
 from .model import argmax_lowest
 
 
-def dex_decode(model, prompt, T, X, decs=True, trace=False, state=None, force_tokens=None):
+def dex_decode(model, prompt, T, X, decs=True, trace=False, state=None, force_tokens=None, sample=None):
     """Returns dict with tokens [T], match_k [T] (anchor index b_k selected at each commit),
     rounds (list of per-round records) and totals.  `force_tokens` (optional [T]) replaces the
     committed token y (teacher forcing used by the GPU parity harness, R17) - never set when
-    checking losslessness."""
+    checking losslessness.  `sample` = (tau, seed, seq): sampling-mode DECS (Alg. 2 lines 10-15) with the
+    shared Gumbel rows of oracle/gumbel.py (reading R24); None: greedy."""
     X = check_X(X, model.L)
     N = len(X)
     lo = [0] + X[:-1]                          # d_{k-1}, with d_{-1}=0
@@ -66,6 +68,9 @@ def dex_decode(model, prompt, T, X, decs=True, trace=False, state=None, force_to
         logits_ref = None
         for i in new_nodes:
             logits = model.exit_logits(new_h[i])
+            if sample is not None:             # Alg. 2 line 13: l / tau + G of the slot (position being decoded)
+                tau, seed, sseq = sample
+                logits = perturbed(logits, tau, gumbel_row(seed, sseq, n + lt.pos_offset(i), logits.shape[0]))
             masked = set()
             if decs and i != ref_node:         # Alg. 2 lines 1-4: reference node never masked
                 masked = {u[a] if a in u else new_u[a] for a in lt.slot_chain_prior(i)}
