@@ -207,8 +207,10 @@ def bench_dex(args):
     prompt[:] = dex_synth.make_prompt(shape.vocab, n_prompt, wl.prompt_seed, seq=replica_prompt_seq(rank))
     max_ctx = n_prompt + T + 8
     FL = P.DEX_STEP_AUTOCOLLAPSE
-    g = P.Dex(shape, w_dev, X, max_ctx=max_ctx, device=dev, act_planes=args.act_planes)
-    a = P.Dex(shape, w_dev, (L,), max_ctx=max_ctx, device=dev, act_planes=args.act_planes)
+    mode = dict(decs=args.decs, sample=1 if args.temperature > 0 else 0, temperature=max(args.temperature, 1e-6),
+                sample_seed=args.sample_seed)
+    g = P.Dex(shape, w_dev, X, max_ctx=max_ctx, device=dev, act_planes=args.act_planes, **mode)
+    a = P.Dex(shape, w_dev, (L,), max_ctx=max_ctx, device=dev, act_planes=args.act_planes, **mode)
     g.prefill(0, prompt)
     a.prefill(0, prompt)
 
@@ -326,7 +328,7 @@ def bench_dex(args):
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "bf16", "data": "synthetic",
             "config": {"workload": f"{wl.key}: {shape.name} L={L} d={shape.d_model} X={list(X)} prompt={n_prompt} "
-                                   f"gen={T} bs=1 greedy decs=1",
+                                   f"gen={T} bs=1 {'greedy' if args.temperature <= 0 else 'sample T=%g' % args.temperature} decs={args.decs}",
                        "parallelism": "replicas only" if world > 1 else "single GPU",
                        "act_planes": args.act_planes,
                        "l2": "inputs larger than L2 (13.5 GB of weights streamed per pass vs 126 MB L2)",
@@ -422,6 +424,9 @@ def main():
     ap.add_argument("--impl", default="dex", choices=["dex", "reference"])
     ap.add_argument("--workload", default="c2")
     ap.add_argument("--depths", default="", help="comma-separated exploration set X (last = L); default: the workload's")
+    ap.add_argument("--decs", type=int, default=1, help="1: DECS masking (Alg. 2), 0: vanilla decoding of the exits")
+    ap.add_argument("--temperature", type=float, default=0.0, help="> 0: sampling-mode DECS (Alg. 2 lines 10-15)")
+    ap.add_argument("--sample-seed", type=int, default=2024)
     ap.add_argument("--gen-len", type=int, default=0)
     ap.add_argument("--prompt-len", type=int, default=0)
     ap.add_argument("--act-planes", type=int, default=2)

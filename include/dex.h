@@ -62,6 +62,12 @@ typedef struct dex_config {
   int32_t act_planes;    /* 1: activations enter the MMAs as bf16; 2: as bf16 hi+lo pair  */
   int32_t use_graph;     /* 1: replay the step as a CUDA graph                            */
   int32_t round_kernel;  /* 1: one persistent kernel per round (k_round); 0: one launch per op */
+  int32_t sample;        /* 0: greedy (Alg. 2 line 9); 1: sampling-mode DECS (Alg. 2 lines 10-15):
+                            y = argmax_v (l_v / temperature + G_v) with a Gumbel(0,1) row shared by every depth of a
+                            slot chain, drawn by a counter-based generator from (sample_seed, sequence, absolute
+                            position of the decoded token) - reading R24 in DESIGN.md.  Needs round_kernel = 1 */
+  float   temperature;   /* tau > 0 (sample = 1)                                           */
+  int32_t sample_seed;
 } dex_config;
 
 /* Device pointers to the packed tensors (row-major, "out x in"; layout = dex_synth/gen.py):

@@ -24,7 +24,8 @@ class DexConfig(C.Structure):
     _fields_ = [(n, C.c_int32) for n in ("n_layers", "d_model", "n_heads", "n_kv_heads", "head_dim", "d_ffn", "vocab")] + \
                [("rms_eps", C.c_float), ("rope_theta", C.c_float)] + \
                [(n, C.c_int32) for n in ("max_seqs", "max_ctx", "page_size", "decs", "eos_id", "debug_taps",
-                                         "act_planes", "use_graph", "round_kernel")]
+                                         "act_planes", "use_graph", "round_kernel", "sample")] + \
+               [("temperature", C.c_float), ("sample_seed", C.c_int32)]
 
 
 class DexWeights(C.Structure):
@@ -161,7 +162,8 @@ class Dex:
     """Convenience owner of the device memory a context borrows (weights, workspace, stream)."""
 
     def __init__(self, shape, weights, depths, max_seqs=1, max_ctx=1024, page_size=128, decs=1, eos_id=-1,
-                 debug_taps=0, act_planes=2, use_graph=1, round_kernel=1, device="cuda:0", stream=None):
+                 debug_taps=0, act_planes=2, use_graph=1, round_kernel=1, sample=0, temperature=1.0, sample_seed=0,
+                 device="cuda:0", stream=None):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2606_29223_b200 needs a CUDA device (no CPU fallback)")
@@ -170,7 +172,8 @@ class Dex:
         self.shape, self.depths = shape, tuple(int(d) for d in depths)
         self.cfg = DexConfig(shape.n_layers, shape.d_model, shape.n_heads, shape.n_kv_heads, shape.head_dim,
                              shape.d_ffn, shape.vocab, shape.rms_eps, shape.rope_theta, max_seqs, max_ctx, page_size,
-                             decs, eos_id, debug_taps, act_planes, use_graph, round_kernel)
+                             decs, eos_id, debug_taps, act_planes, use_graph, round_kernel, sample, temperature,
+                             sample_seed)
         with torch.cuda.device(self.device):
             self.w = {}
             for k, v in weights.items():

@@ -129,6 +129,9 @@ int validate(const dex_config* cfg, const int32_t* depths, int32_t n) {
   if (cfg->max_seqs < 1 || cfg->max_seqs > 8) return fail(nullptr, DEX_EINVAL, "max_seqs must be in [1,8]");
   if (cfg->max_ctx < 2) return fail(nullptr, DEX_EINVAL, "max_ctx too small");
   if (cfg->round_kernel != 0 && cfg->round_kernel != 1) return fail(nullptr, DEX_EINVAL, "round_kernel must be 0 or 1");
+  if (cfg->sample != 0 && cfg->sample != 1) return fail(nullptr, DEX_EINVAL, "sample must be 0 or 1");
+  if (cfg->sample && !(cfg->temperature > 0.f)) return fail(nullptr, DEX_EINVAL, "temperature must be > 0");
+  if (cfg->sample && !cfg->round_kernel) return fail(nullptr, DEX_EINVAL, "sampling mode needs round_kernel = 1");
   if (cfg->act_planes != 1 && cfg->act_planes != 2) return fail(nullptr, DEX_EINVAL, "act_planes must be 1 or 2");
   if (cfg->vocab < 2) return fail(nullptr, DEX_EINVAL, "vocab too small");
   if (cfg->d_model > 8192) return fail(nullptr, DEX_ECAPACITY, "d_model > 8192 not supported");
@@ -428,7 +431,7 @@ int enqueue_step(dex_ctx* c, uint32_t flags, int n_chunks) {
   CU(c, launch_gather_norm(D, c->dec_plan, D.R_dec, c->stream));
   ph_end(c, PH_BOOK);
   int rc;
-  if (c->cfg.round_kernel && c->round_ok && !c->phase_split) {
+  if (c->cfg.round_kernel && c->round_ok && (!c->phase_split || c->cfg.sample)) {
     rc = enqueue_round(c, n_chunks);
     if (rc) return rc;
   } else {
@@ -490,7 +493,7 @@ void account_round(dex_ctx* c) {
     (void)any;
     gemm_launches += 4;
   }
-  const bool mega = c->cfg.round_kernel && c->round_ok && !c->phase_split;
+  const bool mega = c->cfg.round_kernel && c->round_ok && (!c->phase_split || c->cfg.sample);
   c->counters[0] += 1;
   c->counters[1] += mega ? 7.0 : 2 + 10.0 * D.max_len + 1 + 1 + 3;
   c->counters[2] += mega ? 1 : gemm_launches;
@@ -580,6 +583,7 @@ int32_t dex_init(dex_ctx** out, const dex_config* cfg, const dex_weights* w, con
   D.max_seqs = cfg->max_seqs; D.max_ctx = cfg->max_ctx; D.page_size = cfg->page_size;
   D.pages_per_seq = L.pages_per_seq; D.n_pages = L.n_pages; D.n_slots = L.n_slots; D.n_nodes = L.n_nodes;
   D.R_cap = L.R_cap; D.R_dec = L.R_dec; D.exit_chunk = L.exit_chunk; D.decs = cfg->decs; D.planes = cfg->act_planes; D.taps = cfg->debug_taps;
+  D.sample = cfg->sample; D.inv_tau = cfg->sample ? 1.0f / cfg->temperature : 1.0f; D.sample_seed = (unsigned)cfg->sample_seed;
   D.max_len = L.max_len; D.max_chunks = L.max_chunks; D.ref_tiles = L.ref_tiles;
   D.embed = static_cast<const __nv_bfloat16*>(w->embed);
   D.lm_head = static_cast<const __nv_bfloat16*>(w->lm_head);
@@ -616,6 +620,10 @@ int32_t dex_init(dex_ctx** out, const dex_config* cfg, const dex_weights* w, con
     const size_t attn = (round_attn_smem(cfg->head_dim) + 1023) / 1024 * 1024;
     const size_t budget = 222 * 1024 - attn - 2048;
     c->round_ok = budget / stage >= 3;                    // too few ring stages (very wide stages): per-op path
+    if (cfg->sample && !c->round_ok) {
+      delete c;
+      return fail(nullptr, DEX_ECAPACITY, "sampling mode needs the round kernel, whose ring does not fit this stage width");
+    }
     c->round_ring.n_stages = (int)std::max<size_t>(2, std::min<size_t>(12, budget / stage));
     c->round_attn_off = (int)((c->round_ring.n_stages * stage + 1023 + 512) / 1024 * 1024);
     c->round_ring.smem = c->round_attn_off + attn + 1024;

@@ -82,6 +82,9 @@ struct Dev {
   int R_dec;               // rows used by the decode plan
   int exit_chunk;          // rows per exit-head group (= largest decode group, rounded to 16: the exit shares the ring)
   int decs, planes, taps;
+  int sample;              // sampling-mode DECS (Alg. 2 lines 10-15)
+  float inv_tau;           // 1 / temperature
+  unsigned sample_seed;
   int max_len;             // max_m |Pi_m|
   // weights
   const __nv_bfloat16 *embed, *lm_head;
@@ -151,6 +154,19 @@ __device__ __forceinline__ float inv_rms(const Dev& D, int r) {
 #pragma unroll
   for (int i = 0; i < kSsSeg / 4; ++i) ss += (v[i].x + v[i].y) + (v[i].z + v[i].w);   // fixed order
   return 1.0f / sqrtf(ss / (float)D.d + D.eps);
+}
+
+// Gumbel(0,1) noise of (seed, sequence, absolute position of the decoded token, vocabulary id): splitmix64 finaliser
+// of a counter, 24-bit uniform, G = -log(-log u).  The CPU checker implements the same generator on its own (R24).
+__device__ __forceinline__ float gumbel_noise(unsigned seed, int seq, int pos, int v) {
+  const unsigned long long key = (unsigned long long)seed ^ ((unsigned long long)seq << 56);
+  const unsigned long long ctr = ((unsigned long long)(unsigned)pos << 32) + (unsigned long long)(unsigned)v + 1ull;
+  unsigned long long z = key + 0x9E3779B97F4A7C15ull * ctr;
+  z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
+  z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
+  z = z ^ (z >> 31);
+  const float u = ((float)(unsigned)(z >> 41) + 0.5f) * 1.1920928955078125e-07f;   // 2^-23: exact in fp32
+  return -logf(-logf(u));
 }
 
 // fp32 -> bf16 hi (+ lo residual) planes.

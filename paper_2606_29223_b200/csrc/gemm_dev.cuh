@@ -20,6 +20,7 @@ struct EpiCtx {
   unsigned long long* best_key;
   float2* ref_tile;
   int ref_tiles;
+  const Dev* dev;          // sampling mode only (k_round): deferred norm scale, temperature, seed
 };
 
 // One ring stage: (kTileK/16) MMAs of M=128, K=16 into d_tmem.  Activation planes (bf16 hi / lo, R23):
@@ -72,12 +73,19 @@ __device__ __forceinline__ void epilogue_item(const EpiCtx& e, uint32_t t_addr, 
           dst[(size_t)i * e.part_ld] = __uint_as_float(v[i]);
       }
     } else {
+      // sampling mode (Alg. 2 line 13): the logit needs its deferred RMSNorm scale before the noise is added;
+      // lane i computes the scale of row c0 + i once per block of 16 rows
+      float inv_lane = 1.f;
+      const bool sampling = e.dev != nullptr && e.dev->sample;
+      if (sampling && lane < 16 && row0 + c0 + lane < row_end) inv_lane = inv_rms(*e.dev, row0 + c0 + lane) * e.dev->inv_tau;
 #pragma unroll
       for (int i = 0; i < 16; ++i) {
         const int rr = row0 + c0 + i;
+        const float inv_i = __shfl_sync(0xffffffffu, inv_lane, i);
         if (rr >= row_end || !((e.s_valid[rr >> 5] >> (rr & 31)) & 1u)) continue;   // warp-uniform
         const RowInfo* ri = &e.rows[rr];
         float val = __uint_as_float(v[i]);
+        if (sampling) val = val * inv_i + gumbel_noise(e.dev->sample_seed, ri->seq, ri->pos + 1, col);
         bool dead = col >= e.vocab;
         const int nm = ri->n_mask;                      // Alg. 2 lines 5-7: mask prior proposals
         for (int t = 0; t < nm; ++t) dead |= (ri->mask_tok[t] == col);

@@ -607,9 +607,11 @@ __global__ void k_decide(Dev D, Plan plan, int auto_collapse) {
       t1 = hi;
     }
     // the exit head saw x*w_final: apply the deferred RMSNorm scale of the anchor row
-    const float inv = inv_rms(D, plan.row_base[N - 1] + s * cap_of(N, N - 1));
-    t1 *= inv;
-    t2 *= inv;
+    if (!D.sample) {                                    // sampling mode reports the perturbed values (already scaled)
+      const float inv = inv_rms(D, plan.row_base[N - 1] + s * cap_of(N, N - 1));
+      t1 *= inv;
+      t2 *= inv;
+    }
   }
   if (lane != 0) return;
   res->active = 1;

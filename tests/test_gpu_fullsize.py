@@ -200,3 +200,21 @@ def test_c2_dex_short_run_against_fp32_oracle(P, c2):
             g.collapse(0, r.match_k, r.token)
     assert worst < 2e-2, worst
     g.close()
+
+
+def test_c2_sampling_dex_equals_ar(P, c2):
+    """Sampling-mode DECS at the 7B shape: GPU DEX stream == GPU AR stream (same Gumbel rows), differs from greedy."""
+    import dex_synth
+    wl, w = c2
+    p = dex_synth.make_prompt(wl.shape.vocab, 64, wl.prompt_seed)
+    T = 32
+    out = {}
+    for name, X, kw in (("ar", (wl.shape.n_layers,), dict(sample=1, temperature=1.0, sample_seed=5)),
+                        ("dex", wl.depths, dict(sample=1, temperature=1.0, sample_seed=5)),
+                        ("greedy", wl.depths, dict())):
+        d = P.Dex(wl.shape, w, X, max_ctx=128, **kw)
+        d.prefill(0, p)
+        out[name], _ = d.generate(T)
+        d.close()
+    assert np.array_equal(out["dex"], out["ar"])
+    assert not np.array_equal(out["dex"], out["greedy"])
