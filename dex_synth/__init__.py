@@ -8,4 +8,4 @@ stand in for the paper's checkpoints and GSM8K / HumanEval / XSum prompts
 (Sec. 4), none of which exist in this environment.
 """
 from .configs import ModelShape, Workload, WORKLOADS, workload  # noqa: F401
-from .gen import make_weights, make_prompt, bf16_round_f32  # noqa: F401
+from .gen import make_weights, make_adapters, make_prompt, bf16_round_f32  # noqa: F401

@@ -81,3 +81,20 @@ def make_prompt(vocab: int, n: int, seed: int = 4321, seq: int = 0) -> np.ndarra
     """n tokens ~ U[0, vocab) (BASELINE.json:configs "uniform over vocab")."""
     rg = np.random.Generator(np.random.Philox(key=_subseed(seed, "prompt", seq)))
     return rg.integers(0, vocab, size=n, dtype=np.int64).astype(np.int32)
+
+
+def make_adapters(shape: ModelShape, n_ad: int, seed: int = 1234, alpha: float = 1e-3, m: int = 0, std: float = 0.02):
+    """Random-init inducing adapters for the n_ad non-final exit depths: w1 [n,m,h] and
+    w2 [n,h,m] bf16-representable N(0, std); biases N(0, std) fp32; RMSNorm scale ones; gate alpha (the paper
+    initialises it to 1e-3; tests use larger values so that the adapter changes proposals).  m = 2h by default."""
+    h = shape.d_model
+    m = m or 2 * h
+    out = {
+        "w1": torch.stack([_normal((m, h), seed, "ad_w1", k, std) for k in range(n_ad)]).to(torch.bfloat16),
+        "w2": torch.stack([_normal((h, m), seed, "ad_w2", k, std) for k in range(n_ad)]).to(torch.bfloat16),
+        "b1": torch.stack([_normal((m,), seed, "ad_b1", k, std) for k in range(n_ad)]),
+        "b2": torch.stack([_normal((h,), seed, "ad_b2", k, std) for k in range(n_ad)]),
+        "norm": torch.ones((n_ad, h), dtype=torch.float32),
+        "alpha": torch.full((n_ad,), float(alpha), dtype=torch.float32),
+    }
+    return out

@@ -67,7 +67,7 @@ def dex_decode(model, prompt, T, X, decs=True, trace=False, state=None, force_to
         ref_node = lt.anchor(N - 1)
         logits_ref = None
         for i in new_nodes:
-            logits = model.exit_logits(new_h[i])
+            logits = model.exit_logits_at(new_h[i], lt.stage(i), N)   # adapters (if any) at non-final depths
             if sample is not None:             # Alg. 2 line 13: l / tau + G of the slot (position being decoded)
                 tau, seed, sseq = sample
                 logits = perturbed(logits, tau, gumbel_row(seed, sseq, n + lt.pos_offset(i), logits.shape[0]))

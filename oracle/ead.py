@@ -73,3 +73,9 @@ def first_match_depth(omega_row, X):
     """Vanilla DEX commit rule (reading R7): shallowest explored depth whose
     candidate equals the final-depth token (plain equality, not stable)."""
     return min(d for d in X if omega_row[d - 1] == 1)
+
+
+def adapter_params(h, m=None):
+    """P_ad = hm + mh + m + 2h + 1; m = 2h by default -> 4h^2 + 4h + 1."""
+    m = 2 * h if m is None else m
+    return h * m + m * h + m + 2 * h + 1

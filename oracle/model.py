@@ -44,7 +44,7 @@ def silu(x):
 class OracleModel:
     """Holds the tensors of dex_synth.make_weights upcast to `dtype` (exact for bf16)."""
 
-    def __init__(self, shape, weights, dtype=np.float64, kv_round=None):
+    def __init__(self, shape, weights, dtype=np.float64, kv_round=None, adapters=None):
         self.shape = shape
         self.dtype = dtype
         self.kv_round = kv_round
@@ -64,6 +64,9 @@ class OracleModel:
         self.norm_attn = cv(weights["norm_attn"])
         self.norm_ffn = cv(weights["norm_ffn"])
         self.norm_final = cv(weights["norm_final"])
+        # inducing adapters of the non-final exit depths (App. C.2), optional:
+        # dict of w1 [n,m,h], b1 [n,m], w2 [n,h,m], b2 [n,h], norm [n,h], alpha [n]
+        self.adapters = None if adapters is None else {k: cv(v) for k, v in adapters.items()}
 
     # ---- one layer, one position -------------------------------------------------------
     def qkv(self, l, x, pos):
@@ -108,6 +111,23 @@ class OracleModel:
     def exit_logits(self, h):
         """Shared exit: final RMSNorm + LM head at any depth."""
         return self.lm_head @ rmsnorm(h, self.norm_final, self.eps)
+
+    def adapter_delta(self, h, k):
+        """Delta h = alpha_k W2_k sigma(W1_k RMSNorm(h) + b1_k) + b2_k scaled by alpha_k (the parameter
+        count P_ad = hm + mh + m + 2h + 1 fixes two biased linears, an RMSNorm scale and the scalar gate,
+        PAPER.md:498-500); sigma = the backbone activation (SiLU)."""
+        A = self.adapters
+        a = rmsnorm(h, A["norm"][k], self.eps)
+        z = silu(A["w1"][k] @ a + A["b1"][k])
+        return A["alpha"][k] * (A["w2"][k] @ z + A["b2"][k])
+
+    def exit_logits_at(self, h, k, n_depths):
+        """Exit at candidate depth index k of n_depths: non-final depths decode the induced representation
+        h~ = h + Delta h "by the same final normalization and LM head as the backbone"; the
+        final depth uses the original hidden state without an adapter."""
+        if self.adapters is not None and k < n_depths - 1:
+            h = h + self.adapter_delta(h, k)
+        return self.exit_logits(h)
 
     def embed_tok(self, tok):
         return self.embed[int(tok)].copy()
