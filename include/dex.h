@@ -68,12 +68,20 @@ typedef struct dex_config {
                             position of the decoded token) - reading R24 in DESIGN.md.  Needs round_kernel = 1 */
   float   temperature;   /* tau > 0 (sample = 1)                                           */
   int32_t sample_seed;
+  int32_t adapter_dim;   /* m > 0: inducing-adapter exits (App. C.2): a row leaving the NON-final
+                            depth d_k (k < N-1) is decoded from h~ = h + alpha_k (W2_k SiLU(W1_k RMSNorm(h; norm_k) + b1_k)
+                            + b2_k) by the shared final norm + LM head; the hidden handed to deeper stages stays h
+                            (lossless).  m is the adapter width (paper: 2 d_model), a multiple of 64,
+                            <= d_ffn.  Needs round_kernel = 1, N >= 2 and the ad_* tensors of dex_weights.  0: off */
 } dex_config;
 
 /* Device pointers to the packed tensors (row-major, "out x in"; layout = dex_synth/gen.py):
  *   embed [V,d] bf16, lm_head [V,d] bf16, wqkv [L,(nh+2nkv)*hd,d] bf16 (q heads, k heads, v heads),
  *   wo [L,d,nh*hd] bf16, wgu [L,2,ffn,d] bf16 (gate, up), wdn [L,d,ffn] bf16,
- *   norm_attn [L,d] f32, norm_ffn [L,d] f32, norm_final [d] f32. */
+ *   norm_attn [L,d] f32, norm_ffn [L,d] f32, norm_final [d] f32;
+ *   adapters (adapter_dim = m > 0 only, else ignored; one per non-final depth, k = 0..N-2):
+ *   ad_w1 [N-1,m,d] bf16, ad_w2 [N-1,d,m] bf16, ad_b1 [N-1,m] f32, ad_b2 [N-1,d] f32, ad_norm [N-1,d] f32,
+ *   ad_alpha [N-1] f32. */
 typedef struct dex_weights {
   const void*  embed;
   const void*  lm_head;
@@ -84,6 +92,12 @@ typedef struct dex_weights {
   const float* norm_attn;
   const float* norm_ffn;
   const float* norm_final;
+  const void*  ad_w1;
+  const void*  ad_w2;
+  const float* ad_b1;
+  const float* ad_b2;
+  const float* ad_norm;
+  const float* ad_alpha;
 } dex_weights;
 
 /* Per-sequence record of one round of Alg. 1 (host memory). */

@@ -25,12 +25,13 @@ class DexConfig(C.Structure):
                [("rms_eps", C.c_float), ("rope_theta", C.c_float)] + \
                [(n, C.c_int32) for n in ("max_seqs", "max_ctx", "page_size", "decs", "eos_id", "debug_taps",
                                          "act_planes", "use_graph", "round_kernel", "sample")] + \
-               [("temperature", C.c_float), ("sample_seed", C.c_int32)]
+               [("temperature", C.c_float), ("sample_seed", C.c_int32), ("adapter_dim", C.c_int32)]
 
 
 class DexWeights(C.Structure):
     _fields_ = [(n, C.c_void_p) for n in ("embed", "lm_head", "wqkv", "wo", "wgu", "wdn",
-                                          "norm_attn", "norm_ffn", "norm_final")]
+                                          "norm_attn", "norm_ffn", "norm_final",
+                                          "ad_w1", "ad_w2", "ad_b1", "ad_b2", "ad_norm", "ad_alpha")]
 
 
 class DexStepResult(C.Structure):
@@ -163,24 +164,37 @@ class Dex:
 
     def __init__(self, shape, weights, depths, max_seqs=1, max_ctx=1024, page_size=128, decs=1, eos_id=-1,
                  debug_taps=0, act_planes=2, use_graph=1, round_kernel=1, sample=0, temperature=1.0, sample_seed=0,
-                 device="cuda:0", stream=None):
+                 adapters=None, device="cuda:0", stream=None):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2606_29223_b200 needs a CUDA device (no CPU fallback)")
         self.torch = torch
         self.device = torch.device(device)
         self.shape, self.depths = shape, tuple(int(d) for d in depths)
+        adapter_dim = 0
+        if adapters is not None:            # dex_synth.make_adapters layout: one adapter per non-final depth
+            if adapters["w1"].shape[0] != len(self.depths) - 1:
+                raise ValueError("need one inducing adapter per non-final depth (N - 1)")
+            adapter_dim = int(adapters["w1"].shape[1])
         self.cfg = DexConfig(shape.n_layers, shape.d_model, shape.n_heads, shape.n_kv_heads, shape.head_dim,
                              shape.d_ffn, shape.vocab, shape.rms_eps, shape.rope_theta, max_seqs, max_ctx, page_size,
                              decs, eos_id, debug_taps, act_planes, use_graph, round_kernel, sample, temperature,
-                             sample_seed)
+                             sample_seed, adapter_dim)
         with torch.cuda.device(self.device):
             self.w = {}
             for k, v in weights.items():
                 dt = torch.float32 if k.startswith("norm") else torch.bfloat16
                 self.w[k] = v.to(device=self.device, dtype=dt).contiguous()
-            self.wstruct = DexWeights(*[self.w[k].data_ptr() for k in ("embed", "lm_head", "wqkv", "wo", "wgu", "wdn",
-                                                                       "norm_attn", "norm_ffn", "norm_final")])
+            ptrs = [self.w[k].data_ptr() for k in ("embed", "lm_head", "wqkv", "wo", "wgu", "wdn",
+                                                   "norm_attn", "norm_ffn", "norm_final")]
+            if adapters is not None:
+                for k in ("w1", "w2", "b1", "b2", "norm", "alpha"):
+                    dt = torch.bfloat16 if k in ("w1", "w2") else torch.float32
+                    self.w["ad_" + k] = adapters[k].to(device=self.device, dtype=dt).contiguous()
+                    ptrs.append(self.w["ad_" + k].data_ptr())
+            else:
+                ptrs += [None] * 6
+            self.wstruct = DexWeights(*ptrs)
             self.ws_bytes = dex_workspace_bytes(self.cfg, self.depths)
             self.workspace = torch.empty(self.ws_bytes + 1024, dtype=torch.uint8, device=self.device)
             ptr = (self.workspace.data_ptr() + 1023) // 1024 * 1024

@@ -67,7 +67,7 @@ struct dex_ctx {
   Dev D;
   Plan dec_plan, pre_plan, exit_plan;
   RingCfg dec_ring, pre_ring, exit_ring;
-  OpCfg op[5];                        // qkv, o, gate/up, down, lm_head
+  OpCfg op[7];                        // qkv, o, gate/up, down, lm_head, adapter W1, adapter W2
   CUtensorMap tmX[4];                 // act_a, act_o, act_f, act_e
   cudaStream_t stream;
   int n_sms;
@@ -81,6 +81,7 @@ struct dex_ctx {
   RingCfg round_ring;
   int round_attn_off;
   bool round_ok;                      // the round kernel's ring + attention scratch fit shared memory
+  bool has_ad;                        // inducing-adapter exits (cfg.adapter_dim > 0, N >= 2): round kernel only
   std::map<long long, cudaGraphExec_t> graphs;
   std::string err;
   // phase timing (taps only)
@@ -134,6 +135,10 @@ int validate(const dex_config* cfg, const int32_t* depths, int32_t n) {
   if (cfg->sample && !cfg->round_kernel) return fail(nullptr, DEX_EINVAL, "sampling mode needs round_kernel = 1");
   if (cfg->act_planes != 1 && cfg->act_planes != 2) return fail(nullptr, DEX_EINVAL, "act_planes must be 1 or 2");
   if (cfg->vocab < 2) return fail(nullptr, DEX_EINVAL, "vocab too small");
+  if (cfg->adapter_dim < 0 || cfg->adapter_dim % 64 || cfg->adapter_dim > cfg->d_ffn)
+    return fail(nullptr, DEX_EINVAL, "adapter_dim must be a multiple of 64 in [0, d_ffn]");
+  if (cfg->adapter_dim && !cfg->round_kernel) return fail(nullptr, DEX_EINVAL, "inducing adapters need round_kernel = 1");
+  if (cfg->adapter_dim && n < 2) return fail(nullptr, DEX_EINVAL, "inducing adapters need a non-final depth (N >= 2)");
   if (cfg->d_model > 8192) return fail(nullptr, DEX_ECAPACITY, "d_model > 8192 not supported");
   if (cfg->max_seqs * cap_of(n, 0) > 256) return fail(nullptr, DEX_ECAPACITY, "max_seqs * 2^(N-2) rows exceed 256 per stage");
   return DEX_OK;
@@ -166,7 +171,7 @@ void split_fine(OpDesc& o, bool allow_split) {
 struct Layout {
   int N, R_dec, R_cap, exit_chunk, max_chunks, n_slots, n_nodes, pages_per_seq, n_pages, max_len, ref_tiles;
   Plan dec, pre, ext;
-  OpCfg op[5];
+  OpCfg op[7];
   size_t part_floats;
   size_t off[40];
   size_t total;
@@ -222,6 +227,15 @@ void make_layout(const dex_config& c, const int32_t* depths, int n, Layout& L) {
     if (i != 4) {
       L.part_floats = std::max(L.part_floats, (size_t)L.op[i].dec.ksplit * L.op[i].dec.split_stride);
       L.part_floats = std::max(L.part_floats, (size_t)L.op[i].pre.ksplit * L.op[i].pre.split_stride);
+    }
+  }
+  if (c.adapter_dim > 0) {   // adapter projections: decode rounds only
+    const int ao[2] = {c.adapter_dim, c.d_model}, ak[2] = {c.d_model, c.adapter_dim};
+    for (int i = 0; i < 2; ++i) {
+      fill_desc(L.op[5 + i].dec, ao[i], ak[i], L.R_cap);
+      split_fine(L.op[5 + i].dec, true);
+      L.op[5 + i].pre = L.op[5 + i].dec;
+      L.part_floats = std::max(L.part_floats, (size_t)L.op[5 + i].dec.ksplit * L.op[5 + i].dec.split_stride);
     }
   }
   L.max_chunks = (c.max_ctx + n) / kChunk + 1;
@@ -404,7 +418,7 @@ int enqueue_round(dex_ctx* c, int n_chunks) {
   a.D = c->D;
   a.dec = c->dec_plan;
   a.ext = c->exit_plan;
-  for (int i = 0; i < 5; ++i) a.op[i] = c->op[i].dec;
+  for (int i = 0; i < 7; ++i) a.op[i] = c->op[i].dec;
   a.x_cap = c->round_ring.x_cap;
   a.n_stages = c->round_ring.n_stages;
   a.acc_cols = c->round_ring.acc_cols;
@@ -431,7 +445,7 @@ int enqueue_step(dex_ctx* c, uint32_t flags, int n_chunks) {
   CU(c, launch_gather_norm(D, c->dec_plan, D.R_dec, c->stream));
   ph_end(c, PH_BOOK);
   int rc;
-  if (c->cfg.round_kernel && c->round_ok && (!c->phase_split || c->cfg.sample)) {
+  if (c->cfg.round_kernel && c->round_ok && (!c->phase_split || c->cfg.sample || c->has_ad)) {
     rc = enqueue_round(c, n_chunks);
     if (rc) return rc;
   } else {
@@ -493,7 +507,10 @@ void account_round(dex_ctx* c) {
     (void)any;
     gemm_launches += 4;
   }
-  const bool mega = c->cfg.round_kernel && c->round_ok && (!c->phase_split || c->cfg.sample);
+  if (c->has_ad)   // every live non-final stage streams its adapter once per round
+    for (int m = 0; m + 1 < D.N; ++m)
+      if (live[m]) wbytes += 2.0 * (c->op[5].dec.out_dim * (double)c->op[5].dec.k_dim + c->op[6].dec.out_dim * (double)c->op[6].dec.k_dim);
+  const bool mega = c->cfg.round_kernel && c->round_ok && (!c->phase_split || c->cfg.sample || c->has_ad);
   c->counters[0] += 1;
   c->counters[1] += mega ? 7.0 : 2 + 10.0 * D.max_len + 1 + 1 + 3;
   c->counters[2] += mega ? 1 : gemm_launches;
@@ -549,6 +566,8 @@ int32_t dex_init(dex_ctx** out, const dex_config* cfg, const dex_weights* w, con
   if (!w || !w->embed || !w->lm_head || !w->wqkv || !w->wo || !w->wgu || !w->wdn || !w->norm_attn || !w->norm_ffn ||
       !w->norm_final)
     return fail(nullptr, DEX_EINVAL, "null weight pointer");
+  if (cfg->adapter_dim && (!w->ad_w1 || !w->ad_w2 || !w->ad_b1 || !w->ad_b2 || !w->ad_norm || !w->ad_alpha))
+    return fail(nullptr, DEX_EINVAL, "adapter_dim > 0 but an adapter tensor is null");
   if (!workspace || (reinterpret_cast<uintptr_t>(workspace) & 1023)) return fail(nullptr, DEX_EINVAL, "workspace must be 1024-byte aligned");
   std::unique_ptr<Layout> Lp(new Layout);
   Layout& L = *Lp;
@@ -585,6 +604,9 @@ int32_t dex_init(dex_ctx** out, const dex_config* cfg, const dex_weights* w, con
   D.R_cap = L.R_cap; D.R_dec = L.R_dec; D.exit_chunk = L.exit_chunk; D.decs = cfg->decs; D.planes = cfg->act_planes; D.taps = cfg->debug_taps;
   D.sample = cfg->sample; D.inv_tau = cfg->sample ? 1.0f / cfg->temperature : 1.0f; D.sample_seed = (unsigned)cfg->sample_seed;
   D.max_len = L.max_len; D.max_chunks = L.max_chunks; D.ref_tiles = L.ref_tiles;
+  c->has_ad = cfg->adapter_dim > 0;
+  D.ad_m = cfg->adapter_dim;
+  if (c->has_ad) { D.ad_b1 = w->ad_b1; D.ad_b2 = w->ad_b2; D.ad_norm = w->ad_norm; D.ad_alpha = w->ad_alpha; }
   D.embed = static_cast<const __nv_bfloat16*>(w->embed);
   D.lm_head = static_cast<const __nv_bfloat16*>(w->lm_head);
   D.norm_attn = w->norm_attn; D.norm_ffn = w->norm_ffn; D.norm_final = w->norm_final;
@@ -606,7 +628,7 @@ int32_t dex_init(dex_ctx** out, const dex_config* cfg, const dex_weights* w, con
   c->dbg_stage = cfg->debug_taps ? WSP(float, B_DBG) : nullptr;
   c->dbg_floats = L.dbg_floats;
 #undef WSP
-  for (int i = 0; i < 5; ++i) c->op[i] = L.op[i];
+  for (int i = 0; i < 7; ++i) c->op[i] = L.op[i];
   c->dec_ring = make_ring(c->dec_plan, cfg->act_planes);
   c->pre_ring = make_ring(c->pre_plan, cfg->act_planes);
   c->exit_ring = make_ring(c->exit_plan, cfg->act_planes);
@@ -620,9 +642,9 @@ int32_t dex_init(dex_ctx** out, const dex_config* cfg, const dex_weights* w, con
     const size_t attn = (round_attn_smem(cfg->head_dim) + 1023) / 1024 * 1024;
     const size_t budget = 222 * 1024 - attn - 2048;
     c->round_ok = budget / stage >= 3;                    // too few ring stages (very wide stages): per-op path
-    if (cfg->sample && !c->round_ok) {
+    if ((cfg->sample || c->has_ad) && !c->round_ok) {
       delete c;
-      return fail(nullptr, DEX_ECAPACITY, "sampling mode needs the round kernel, whose ring does not fit this stage width");
+      return fail(nullptr, DEX_ECAPACITY, "sampling mode / inducing adapters need the round kernel, whose ring does not fit this stage width");
     }
     c->round_ring.n_stages = (int)std::max<size_t>(2, std::min<size_t>(12, budget / stage));
     c->round_attn_off = (int)((c->round_ring.n_stages * stage + 1023 + 512) / 1024 * 1024);
@@ -665,7 +687,13 @@ int32_t dex_init(dex_ctx** out, const dex_config* cfg, const dex_weights* w, con
   const int xk[4] = {D.d, D.nh * D.hd, D.ffn, D.d};
   for (int i = 0; i < 4; ++i)
     INIT_FAIL(encode_3d(c, enc, &c->tmX[i], xptr[i], xk[i], D.R_cap, cfg->act_planes, kBoxRows, all_stacked ? 2 : 1));
-  for (int i = 0; i < 5; ++i) c->tms.w[i] = c->op[i].tmW;
+  memset(&c->tms, 0, sizeof c->tms);
+  if (c->has_ad) {
+    const void* aptr[2] = {w->ad_w1, w->ad_w2};
+    for (int i = 0; i < 2; ++i)
+      INIT_FAIL(encode_3d(c, enc, &c->op[5 + i].tmW, aptr[i], c->op[5 + i].dec.k_dim, c->op[5 + i].dec.out_dim, n_depths - 1, kTileM));
+  }
+  for (int i = 0; i < (c->has_ad ? 7 : 5); ++i) c->tms.w[i] = c->op[i].tmW;
   for (int i = 0; i < 4; ++i) c->tms.x[i] = c->tmX[i];
 
   // state: FSM zeroed, free pages, result buffer, RoPE table

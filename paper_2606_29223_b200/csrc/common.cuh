@@ -86,6 +86,8 @@ struct Dev {
   float inv_tau;           // 1 / temperature
   unsigned sample_seed;
   int max_len;             // max_m |Pi_m|
+  int ad_m;                // inducing-adapter width m (0: exits decode h directly); adapter k serves stage k < N-1
+  const float *ad_b1, *ad_b2, *ad_norm, *ad_alpha;   // [N-1][m], [N-1][d], [N-1][d], [N-1]
   // weights
   const __nv_bfloat16 *embed, *lm_head;
   const float *norm_attn, *norm_ffn, *norm_final;
@@ -234,15 +236,15 @@ struct OpDesc {
   size_t split_stride;     // R_cap * part_ld
 };
 
-struct TmSet {             // TMA descriptors of the round kernel: weights qkv,o,gu,dn,lm_head; operands a,o,f,e
-  CUtensorMap w[5];
+struct TmSet {             // TMA descriptors of the round kernel: weights qkv,o,gu,dn,lm_head,ad_w1,ad_w2; operands a,o,f,e
+  CUtensorMap w[7];
   CUtensorMap x[4];
 };
 
 struct RoundArgs {
   Dev D;
   Plan dec, ext;
-  OpDesc op[5];
+  OpDesc op[7];                    // qkv, o, gate/up, down, lm_head, adapter W1, adapter W2
   int x_cap, n_stages, acc_cols, stacked;   // shared-memory ring / TMEM geometry
   int n_chunks;                    // attention chunks that can hold a live position (host upper bound)
   int attn_smem_off;               // byte offset of the attention scratch (AttnSmem) in dynamic shared memory

@@ -102,7 +102,8 @@ __device__ __forceinline__ bool r_seq_live(const SeqState& s) { return s.active 
 __device__ __forceinline__ int r_stage_count(int q, int m) { return m > q ? 0 : (m == q ? 1 : (1 << (q - 1 - m))); }
 
 // ---------------------------------------------------------------- the round's op / item sequence
-// op t < 4*n_steps: step j = t/4, kind t%4 (qkv, o, gate/up, down); op 4*n_steps: the exit head.
+// op t < 4*n_steps: step j = t/4, kind t%4 (qkv, o, gate/up, down); then, with inducing adapters,
+// the two adapter projections W1 (kind 5) and W2 (kind 6) of every live non-final stage; last op: the exit head (kind 4).
 struct OpI {
   int which, j, ext;
   unsigned mask;           // live groups of the op's plan
@@ -115,14 +116,21 @@ struct ItemI {
 struct Seq {               // shared by all roles: same deterministic walk
   const RoundArgs* a;
   const int* s_nb;         // [16] shared: decode group extents 0..7, exit chunk extents 8..15
-  int n_steps, n_ops, G, cta;
+  int n_steps, n_ops, n_ad_ops, G, cta;
 
+  __device__ __forceinline__ int which_of(int t) const {
+    return t < 4 * n_steps ? (t & 3) : (t < 4 * n_steps + n_ad_ops ? 5 + t - 4 * n_steps : 4);
+  }
   __device__ __forceinline__ void op_info(int t, OpI& o) const {
     unsigned mask = 0;
     if (t < 4 * n_steps) {
       o.j = t >> 2; o.which = t & 3; o.ext = 0;
       for (int g = 0; g < a->dec.n_grp; ++g)
         if (s_nb[g] > 0 && o.j < a->dec.layer_len[g]) mask |= 1u << g;
+    } else if (t < 4 * n_steps + n_ad_ops) {
+      o.j = 0; o.which = 5 + t - 4 * n_steps; o.ext = 0;
+      for (int g = 0; g + 1 < a->dec.n_grp; ++g)             // adapter g serves the rows leaving depth d_g, g < N-1
+        if (s_nb[g] > 0) mask |= 1u << g;
     } else {
       o.j = 0; o.which = 4; o.ext = 1;
       for (int g = 0; g < a->ext.n_grp; ++g)
@@ -141,16 +149,16 @@ struct Seq {               // shared by all roles: same deterministic walk
     it.nb = s_nb[(o.ext ? 8 : 0) + it.g];
     it.tile = rem / o.ksplit;
     it.split = rem - it.tile * o.ksplit;
-    it.layer = o.ext ? 0 : p.layer_lo[it.g] + o.j;
+    it.layer = o.ext ? 0 : (o.which >= 5 ? it.g : p.layer_lo[it.g] + o.j);
     it.kb0 = it.split * o.kbps;
     it.kb1 = min(it.kb0 + o.kbps, o.kb_total);
     it.row0 = p.row_base[it.g];
     it.row_end = it.row0 + p.rows_cap[it.g];
   }
   // grid barriers that must have completed before op t's operand may be read (9 per step: one after
-  // every GEMM's epilogue, one after every glue phase; the QKV output takes two glue phases)
+  // every GEMM's epilogue, one after every glue phase; the QKV output takes two glue phases; an adapter op two)
   __device__ __forceinline__ unsigned dep(int t) const {
-    if (t >= 4 * n_steps) return 9u * n_steps;
+    if (t >= 4 * n_steps) return 9u * n_steps + 2u * min(t - 4 * n_steps, n_ad_ops);
     const int k = t & 3;
     return 9u * (t >> 2) + (k == 0 ? 0u : 2u * k + 1u);
   }
@@ -244,6 +252,8 @@ __device__ void glue_add_norm(const RoundArgs& a, int j, int mode, const OpDesc&
         w = D.norm_ffn + (size_t)layer * D.d;
       } else if (j + 1 < a.dec.layer_len[grp]) {
         w = D.norm_attn + (size_t)(layer + 1) * D.d;
+      } else if (D.ad_m > 0 && grp + 1 < D.N) {
+        w = D.ad_norm + (size_t)grp * D.d;       // adapter input RMSNorm(h; norm_k): same row, same deferred scale
       } else {
         w = D.norm_final;
         dst = D.act_e;
@@ -290,6 +300,66 @@ __device__ void glue_silu(const RoundArgs& a, int j, const OpDesc& op, int gw, i
     o.z = g.z / (1.0f + expf(-g.z)) * up.z;
     o.w = g.w / (1.0f + expf(-g.w)) * up.w;
     r_split_store4(D.act_f, ps, (size_t)r * D.ffn + i, o, D.planes);
+  }
+}
+
+// Inducing adapter of the non-final exits (reading R25), first half:
+// act_f[:, 0..m) <- SiLU(inv_rms * (W1_k . (h * norm_k)) + b1_k).  Warp unit = (row, 128 elements of m).
+__device__ void glue_ad1(const RoundArgs& a, const OpDesc& op, int gw, int n_gw, int lane) {
+  const Dev& D = a.D;
+  const int m = D.ad_m, nblk = (m + 127) / 128;
+  const size_t ps = (size_t)D.R_cap * D.ffn;
+  for (int u = gw; u < D.R_dec * nblk; u += n_gw) {
+    const int r = u / nblk, b = u - r * nblk;
+    const int i = b * 128 + lane * 4;
+    if (i >= m) continue;
+    const RowInfo* ri = &D.rows[r];
+    const int valid = ri->valid, grp = ri->grp;
+    const float* const pp[1] = {D.part + (size_t)r * op.part_ld + i};
+    float4 sv[1];
+    r_sum4_batch<1, 8>(pp, op.ksplit, op.split_stride, sv);
+    const float inv = inv_rms(D, r);
+    if (!valid || grp + 1 >= D.N) continue;
+    const float4 bv = r_ld4(D.ad_b1 + (size_t)grp * m + i);
+    float4 t = make_float4(sv[0].x * inv + bv.x, sv[0].y * inv + bv.y, sv[0].z * inv + bv.z, sv[0].w * inv + bv.w);
+    float4 o;
+    o.x = t.x / (1.0f + expf(-t.x));
+    o.y = t.y / (1.0f + expf(-t.y));
+    o.z = t.z / (1.0f + expf(-t.z));
+    o.w = t.w / (1.0f + expf(-t.w));
+    r_split_store4(D.act_f, ps, (size_t)r * D.ffn + i, o, D.planes);
+  }
+}
+
+// Second half: h~ = h + alpha_k (W2_k . act + b2_k); exit operand act_e <- h~ * norm_final with the deferred scale of
+// h~ (ss_part rewritten).  x_cur keeps h: deeper stages continue from the un-induced hidden.
+__device__ void glue_ad2(const RoundArgs& a, const OpDesc& op, int gw, int n_gw, int lane) {
+  const Dev& D = a.D;
+  const int n_seg = (D.d + 127) / 128;
+  for (int u = gw; u < D.R_dec * n_seg; u += n_gw) {
+    const int r = u / n_seg, seg = u - r * n_seg;
+    const RowInfo* ri = &D.rows[r];
+    const int valid = ri->valid, grp = ri->grp;
+    const int i = seg * 128 + lane * 4;
+    const bool in = i < D.d;
+    const float4 xv = r_ld4(D.x_cur + (size_t)r * D.d + (in ? i : 0));
+    const float* const pp[1] = {D.part + (size_t)r * op.part_ld + (in ? i : 0)};
+    float4 sv[1];
+    r_sum4_batch<1, 16>(pp, op.ksplit, op.split_stride, sv);
+    if (!valid || grp + 1 >= D.N) continue;
+    float ss = 0.f;
+    if (in) {
+      const float al = D.ad_alpha[grp];
+      const float4 bv = r_ld4(D.ad_b2 + (size_t)grp * D.d + i);
+      const float4 wv = r_ld4(D.norm_final + i);
+      const float4 v = make_float4(xv.x + al * (sv[0].x + bv.x), xv.y + al * (sv[0].y + bv.y), xv.z + al * (sv[0].z + bv.z),
+                                   xv.w + al * (sv[0].w + bv.w));
+      ss = v.x * v.x + v.y * v.y + v.z * v.z + v.w * v.w;
+      r_split_store4(D.act_e, (size_t)D.R_cap * D.d, (size_t)r * D.d + i, make_float4(v.x * wv.x, v.y * wv.y, v.z * wv.z, v.w * wv.w),
+                     D.planes);
+    }
+    ss = r_warp_sum(ss);
+    if (lane == 0) D.ss_part[(size_t)r * kSsSeg + seg] = ss;
   }
 }
 
@@ -802,7 +872,7 @@ __global__ void __launch_bounds__(kMaxThreads, 1) k_round(const __grid_constant_
       mbar_init(&tempty[i], 4);
     }
     fence_mbar_init();
-    for (int i = 0; i < 5; ++i) tma_prefetch_desc(&tm.w[i]);
+    for (int i = 0; i < (D.ad_m > 0 ? 7 : 5); ++i) tma_prefetch_desc(&tm.w[i]);
     for (int i = 0; i < 4; ++i) tma_prefetch_desc(&tm.x[i]);
   }
   if (warp == 1) {
@@ -815,7 +885,8 @@ __global__ void __launch_bounds__(kMaxThreads, 1) k_round(const __grid_constant_
   const uint32_t tmem_base = *tmem_slot;
 
   Seq sq;
-  sq.a = &a; sq.s_nb = s_nb; sq.n_steps = s_steps; sq.n_ops = 4 * s_steps + 1; sq.G = gridDim.x; sq.cta = blockIdx.x;
+  sq.a = &a; sq.s_nb = s_nb; sq.n_steps = s_steps; sq.n_ad_ops = (D.ad_m > 0 && D.N >= 2) ? 2 : 0;
+  sq.n_ops = 4 * s_steps + sq.n_ad_ops + 1; sq.G = gridDim.x; sq.cta = blockIdx.x;
   const unsigned G = gridDim.x;
 
   if (s_steps > 0) {
@@ -858,7 +929,8 @@ __global__ void __launch_bounds__(kMaxThreads, 1) k_round(const __grid_constant_
           fence_proxy_async();
         }
         const int which = w.o.which;
-        const CUtensorMap* desc = &tm.x[which == 0 ? 0 : (which == 1 ? 1 : (which == 2 ? 0 : (which == 3 ? 2 : 3)))];
+        // operand of the op: act_a (qkv, gate/up, adapter W1), act_o (o), act_f (down, adapter W2), act_e (exit)
+        const CUtensorMap* desc = &tm.x[(which == 0 || which == 2 || which == 5) ? 0 : (which == 1 ? 1 : (which == 4 ? 3 : 2))];
         const int row0 = w.it.row0, nb = w.it.nb;
         for (int kb = w.it.kb0; kb < w.it.kb1; ++kb) {
           // slot free (its previous tile consumed) => full[st] is in this tile's phase; the bytes may
@@ -929,8 +1001,9 @@ __global__ void __launch_bounds__(kMaxThreads, 1) k_round(const __grid_constant_
       };
       stamp();
       auto run_items = [&](int t) {
-        const OpDesc& od = a.op[t < 4 * sq.n_steps ? (t & 3) : 4];
-        ec.mode = (t < 4 * sq.n_steps) ? 0 : 1;
+        const int which = sq.which_of(t);
+        const OpDesc& od = a.op[which];
+        ec.mode = which == 4 ? 1 : 0;
         ec.part_ld = od.part_ld; ec.split_stride = od.split_stride; ec.out_dim = od.out_dim;
         if (we >= 4) return;                                 // TMEM lane quarters belong to warps 2-5
         for (; w.valid && w.t == t; w.next(sq), ++n_it) {
@@ -973,7 +1046,21 @@ __global__ void __launch_bounds__(kMaxThreads, 1) k_round(const __grid_constant_
         stamp();
         ++gb; grid_bar<GT>(D.gbar, gb * G, tid_e, &s_seen, gb); stamp();
       }
-      run_items(4 * sq.n_steps); stamp();
+      int t_exit = 4 * sq.n_steps;
+      if (sq.n_ad_ops) {                                     // inducing adapters of the non-final exits
+        run_items(t_exit); stamp();
+        ++gb; grid_bar<GT>(D.gbar, gb * G, tid_e, &s_seen, gb); stamp();
+        glue_ad1(a, a.op[5], gw, n_gw, lane);
+        stamp();
+        ++gb; grid_bar<GT>(D.gbar, gb * G, tid_e, &s_seen, gb); stamp();
+        run_items(t_exit + 1); stamp();
+        ++gb; grid_bar<GT>(D.gbar, gb * G, tid_e, &s_seen, gb); stamp();
+        glue_ad2(a, a.op[6], gw, n_gw, lane);
+        stamp();
+        ++gb; grid_bar<GT>(D.gbar, gb * G, tid_e, &s_seen, gb); stamp();
+        t_exit += 2;
+      }
+      run_items(t_exit); stamp();
     }
   }
 

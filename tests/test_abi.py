@@ -34,15 +34,15 @@ def test_every_declared_symbol_is_exported(P):
 
 def test_struct_layout_matches_header(P):
     assert ctypes.sizeof(P.DexStepResult) == 120
-    assert ctypes.sizeof(P.DexConfig) == 21 * 4
-    assert ctypes.sizeof(P.DexWeights) == 9 * 8
+    assert ctypes.sizeof(P.DexConfig) == 22 * 4
+    assert ctypes.sizeof(P.DexWeights) == 15 * ctypes.sizeof(ctypes.c_void_p)
     assert P.DexStepResult.layer_evals.offset == 32
 
 
 def _cfg(P, **kw):
     base = dict(n_layers=8, d_model=256, n_heads=4, n_kv_heads=4, head_dim=64, d_ffn=688, vocab=1024, rms_eps=1e-5,
                 rope_theta=1e4, max_seqs=1, max_ctx=256, page_size=128, decs=1, eos_id=-1, debug_taps=0, act_planes=2,
-                use_graph=1, round_kernel=1, sample=0, temperature=1.0, sample_seed=0)
+                use_graph=1, round_kernel=1, sample=0, temperature=1.0, sample_seed=0, adapter_dim=0)
     base.update(kw)
     return P.DexConfig(*[base[n] for n, _ in P.DexConfig._fields_])
 
@@ -57,9 +57,12 @@ def test_exploration_set_validation(P):
             P.dex_workspace_bytes(cfg, bad)
         assert e.value.code == P.DEX_EINVAL
     for kw in [dict(head_dim=96), dict(n_kv_heads=3), dict(page_size=100), dict(max_seqs=0), dict(act_planes=3),
-               dict(d_model=250)]:
+               dict(d_model=250), dict(adapter_dim=96), dict(adapter_dim=704), dict(adapter_dim=512, round_kernel=0)]:
         with pytest.raises(P.DexError):
             P.dex_workspace_bytes(_cfg(P, **kw), (2, 4, 6, 8))
+    with pytest.raises(P.DexError):           # adapters need a non-final depth
+        P.dex_workspace_bytes(_cfg(P, adapter_dim=512), (8,))
+    assert P.dex_workspace_bytes(_cfg(P, adapter_dim=512), (2, 4, 6, 8)) >= P.dex_workspace_bytes(cfg, (2, 4, 6, 8))
     with pytest.raises(P.DexError) as e:      # 8 seqs x 64 stage-0 rows > 256
         P.dex_workspace_bytes(_cfg(P, max_seqs=8), tuple(range(1, 9)))
     assert e.value.code == P.DEX_ECAPACITY

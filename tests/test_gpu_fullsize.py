@@ -165,18 +165,21 @@ def test_fullsize_dex_equals_ar_counts_and_gemm(P, key, T):
     torch.cuda.empty_cache()
 
 
-def test_c2_dex_short_run_against_fp32_oracle(P, c2):
+@pytest.mark.parametrize("with_ad", [False, True])
+def test_c2_dex_short_run_against_fp32_oracle(P, c2, with_ad):
     """The lattice itself at the 7B shape against the oracle's Alg. 1 trace (8-token prompt, 2 commits): every new
     node's stage-boundary hidden state (tolerance R16), its candidate token (a flip only at an oracle top-2
-    margin < 1e-2 of that node, R17), rows per stage / layer evaluations (bit-exact), the commit."""
+    margin < 1e-2 of that node, R17), rows per stage / layer evaluations (bit-exact), the commit.  with_ad: the
+    non-final exits go through inducing adapters of the paper's width m = 2 d_model."""
     import dex_synth
     from oracle import OracleModel, dex_decode
     wl, w = c2
-    om = OracleModel(wl.shape, w, dtype=np.float32, kv_round="bf16")
+    ad = dex_synth.make_adapters(wl.shape, len(wl.depths) - 1, seed=7, alpha=0.5) if with_ad else None
+    om = OracleModel(wl.shape, w, dtype=np.float32, kv_round="bf16", adapters=ad)
     p = dex_synth.make_prompt(wl.shape.vocab, 8, 11)
     T = 2
     od = dex_decode(om, p, T, wl.depths, decs=True, trace=True)
-    g = P.Dex(wl.shape, w, wl.depths, max_ctx=128, debug_taps=1, use_graph=0)
+    g = P.Dex(wl.shape, w, wl.depths, max_ctx=128, debug_taps=1, use_graph=0, adapters=ad)
     g.prefill(0, p)
     worst = 0.0
     for ri, orec in enumerate(od["rounds"]):
@@ -218,3 +221,22 @@ def test_c2_sampling_dex_equals_ar(P, c2):
         d.close()
     assert np.array_equal(out["dex"], out["ar"])
     assert not np.array_equal(out["dex"], out["greedy"])
+
+
+def test_c2_adapter_dex_equals_ar(P, c2):
+    """Inducing-adapter exits at the 7B shape in the launch configuration bench.py times: the committed stream is the
+    GPU AR stream whatever the adapters propose; strong random adapters change the round count."""
+    import dex_synth
+    wl, w = c2
+    p = dex_synth.make_prompt(wl.shape.vocab, 64, wl.prompt_seed)
+    T = 32
+    ad = dex_synth.make_adapters(wl.shape, len(wl.depths) - 1, seed=7, alpha=0.5)
+    out = {}
+    for name, X, adapters in (("ar", (wl.shape.n_layers,), None), ("plain", wl.depths, None), ("ad", wl.depths, ad)):
+        d = P.Dex(wl.shape, w, X, max_ctx=128, adapters=adapters)
+        d.prefill(0, p)
+        toks, recs = d.generate(T)
+        out[name] = (toks, len(recs))
+        d.close()
+    assert np.array_equal(out["ad"][0], out["ar"][0]) and np.array_equal(out["plain"][0], out["ar"][0])
+    assert out["ad"][1] != out["plain"][1]
