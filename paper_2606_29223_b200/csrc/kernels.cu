@@ -396,9 +396,10 @@ __global__ void __launch_bounds__(256) k_silu_mul(Dev D, Plan plan, int step, in
 // branch-private suffix: K/V of its ancestor slots and its own slot, picked per row from the
 // ancestry list (the "ancestry bitmask" of north_star (b), stored as a slot list).  A position's
 // arithmetic is identical wherever its K/V lives, so a row gives the same bits before and after
-// its ancestors are committed.
+// its ancestors are committed.  row_split > 1 (prefill: 128 causal rows per (chunk, head)) deals the rows of a
+// (stage, sequence) to that many CTAs, each staging the chunk for itself: the per-row arithmetic is unchanged.
 template <int HD>
-__global__ void __launch_bounds__(128) k_attn(Dev D, Plan plan, int step, int kv_static) {
+__global__ void __launch_bounds__(128) k_attn(Dev D, Plan plan, int step, int kv_static, int row_split) {
   constexpr int CPR = HD / 8;                       // 16-byte chunks per K/V row
   __shared__ __align__(16) __nv_bfloat16 sK[kChunk * HD];
   __shared__ __align__(16) __nv_bfloat16 sV[kChunk * HD];
@@ -409,10 +410,13 @@ __global__ void __launch_bounds__(128) k_attn(Dev D, Plan plan, int step, int kv
 
   pdl_trigger();
   const int c = blockIdx.x, g = blockIdx.y;
-  const int m = blockIdx.z / D.max_seqs, s = blockIdx.z % D.max_seqs;
+  const int sub = blockIdx.z % row_split, zz = blockIdx.z / row_split;
+  const int m = zz / D.max_seqs, s = zz % D.max_seqs;
   if (m >= plan.n_grp || step >= plan.layer_len[m]) return;
   const int nb = D.grp_nb[m];
   if (nb == 0) return;
+  const int per = (nb + row_split - 1) / row_split;
+  const int r_lo = plan.row_base[m] + sub * per, r_hi = min(r_lo + per, plan.row_base[m] + nb);
   const int layer = plan.layer_lo[m] + step;
   const int c0 = c * kChunk;
 
@@ -422,7 +426,7 @@ __global__ void __launch_bounds__(128) k_attn(Dev D, Plan plan, int step, int kv
     n_paged_s = 0;
   }
   __syncthreads();
-  for (int r = plan.row_base[m] + threadIdx.x; r < plan.row_base[m] + nb; r += blockDim.x) {
+  for (int r = r_lo + threadIdx.x; r < r_hi; r += blockDim.x) {
     const RowInfo* ri = &D.rows[r];
     if (ri->valid && ri->grp == m && ri->seq == s && ri->pos >= c0) {
       int k = atomicAdd(&n_rows_s, 1);
@@ -890,15 +894,16 @@ cudaError_t launch_silu_mul(const Dev& D, const Plan& p, int rows, int step, con
   return launch_pdl(k_silu_mul, dim3(rows, (D.ffn / 4 + 255) / 256), dim3(256), st, D, p, step, o.ksplit, o.split_stride, o.part_ld);
 }
 cudaError_t launch_attn(const Dev& D, const Plan& p, int rows, int step, int n_chunks, int kv_static, cudaStream_t st) {
-  dim3 g(n_chunks, D.nkv, p.n_grp * D.max_seqs);
+  const int row_split = kv_static ? 1 : 8;      // prefill: up to 128 rows per (chunk, head) -> 16 per CTA
+  dim3 g(n_chunks, D.nkv, p.n_grp * D.max_seqs * row_split);
   dim3 gc(rows, D.nh);
   cudaError_t e;
   if (D.hd == 128) {
-    e = launch_pdl(k_attn<128>, g, dim3(128), st, D, p, step, kv_static);
+    e = launch_pdl(k_attn<128>, g, dim3(128), st, D, p, step, kv_static, row_split);
     if (e != cudaSuccess) return e;
     return launch_pdl(k_attn_combine<128>, gc, dim3(128), st, D, p, step);
   }
-  e = launch_pdl(k_attn<64>, g, dim3(128), st, D, p, step, kv_static);
+  e = launch_pdl(k_attn<64>, g, dim3(128), st, D, p, step, kv_static, row_split);
   if (e != cudaSuccess) return e;
   return launch_pdl(k_attn_combine<64>, gc, dim3(64), st, D, p, step);
 }
