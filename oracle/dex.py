@@ -17,12 +17,15 @@ from .gumbel import gumbel_row, perturbed
 from .model import argmax_lowest
 
 
-def dex_decode(model, prompt, T, X, decs=True, trace=False, state=None, force_tokens=None, sample=None):
+def dex_decode(model, prompt, T, X, decs=True, trace=False, state=None, force_tokens=None, sample=None, lookahead=0):
     """Returns dict with tokens [T], match_k [T] (anchor index b_k selected at each commit),
     rounds (list of per-round records) and totals.  `force_tokens` (optional [T]) replaces the
     committed token y (teacher forcing used by the GPU parity harness, R17) - never set when
     checking losslessness.  `sample` = (tau, seed, seq): sampling-mode DECS (Alg. 2 lines 10-15) with the
-    shared Gumbel rows of oracle/gumbel.py (reading R24); None: greedy."""
+    shared Gumbel rows of oracle/gumbel.py (reading R24); None: greedy.  `lookahead` = P > 0: the sparse lattice of
+    reading R26 ("prune low-value branches or construct sparse exploration lattices while preserving
+    the final-depth commit invariant"): a node is expanded only if it lies at most P token positions ahead of the
+    commit position and its parent was expanded; 0: the full lattice of Sec. 3.2."""
     X = check_X(X, model.L)
     N = len(X)
     lo = [0] + X[:-1]                          # d_{k-1}, with d_{-1}=0
@@ -38,6 +41,10 @@ def dex_decode(model, prompt, T, X, decs=True, trace=False, state=None, force_to
     while len(Y) < T:
         n = len(x)
         new_nodes = lt.level_nodes(q)
+        if lookahead > 0:                      # R26: position look-ahead cap; the anchor chain (offset 0) always survives
+            new_nodes = [i for i in new_nodes
+                         if lt.pos_offset(i) <= lookahead and (i == 0 or lt.parent(i) in u)]
+        assert lt.anchor(q) in new_nodes
         rec = dict(q=q, n=n, nodes=new_nodes, rows_per_stage=[0] * N, layer_evals=0,
                    exit_rows=len(new_nodes), critical_layers=0)
         new_h, new_u, new_margin = {}, {}, {}
@@ -98,8 +105,8 @@ def dex_decode(model, prompt, T, X, decs=True, trace=False, state=None, force_to
                 rec["ref_logits"] = logits_ref.copy()
             y = ref if force_tokens is None else int(force_tokens[len(Y)])
             k_sel = N - 1                      # fallback b_{N-1}
-            for k in range(N - 1):             # shallowest matching branch (R6)
-                if cand[k] == y:
+            for k in range(N - 1):             # shallowest matching branch (R6) whose continuation was explored
+                if cand[k] == y and (2 * lt.anchor(k) + 2) in u:      # (R26; always true on the full lattice)
                     k_sel = k
                     break
             Y.append(y)
@@ -109,9 +116,9 @@ def dex_decode(model, prompt, T, X, decs=True, trace=False, state=None, force_to
                 ck[l].append(slot_kv[0][l][0])
                 cv[l].append(slot_kv[0][l][1])
             q_new, mp = lt.collapse_map(k_sel, N)
-            u = {j: u[o] for j, o in mp.items()}
+            u = {j: u[o] for j, o in mp.items() if o in u}
             h_out = {j: h_out[o] for j, o in mp.items() if o in h_out}
-            slot_kv = {j: slot_kv[o] for j, o in mp.items() if lt.slot_root(j) == j}
+            slot_kv = {j: slot_kv[o] for j, o in mp.items() if lt.slot_root(j) == j and o in slot_kv}
             rec.update(committed=1, token=y, match_k=k_sel, ref=ref, q_after=q_new)
             q = q_new
         else:
