@@ -73,6 +73,10 @@ typedef struct dex_config {
                             + b2_k) by the shared final norm + LM head; the hidden handed to deeper stages stays h
                             (lossless).  m is the adapter width (paper: 2 d_model), a multiple of 64,
                             <= d_ffn.  Needs round_kernel = 1, N >= 2 and the ad_* tensors of dex_weights.  0: off */
+  int32_t lookahead;     /* P > 0: sparse exploration lattice (reading R26 in DESIGN.md): a node is expanded
+                            only if it lies at most P token positions ahead of the commit position and its parent was
+                            expanded; the commit takes the shallowest matching anchor whose continuation was explored.
+                            Lossless for every P; P >= N-1 or 0: the full lattice of Sec. 3.2 */
 } dex_config;
 
 /* Device pointers to the packed tensors (row-major, "out x in"; layout = dex_synth/gen.py):
@@ -117,6 +121,9 @@ typedef struct dex_step_result {
   float   ref_top2;
   int32_t n_tokens;          /* committed tokens incl. prompt after the round              */
   int32_t done;              /* eos hit or max_ctx reached                                 */
+  int32_t branch_mask;       /* bit k: the continuation of anchor branch b_k (the position child of anchor k) was
+                                explored, so a commit may collapse onto it; all ones on the full lattice */
+  int32_t reserved;
 } dex_step_result;
 
 /* Bytes of device workspace dex_init needs (committed KV pages, slot KV, hidden rows,
@@ -152,7 +159,8 @@ int32_t dex_step(dex_ctx* ctx, uint32_t flags, dex_step_result* out);
  * for sequence `seq`, append the root slot's K/V of all L layers to the committed pages,
  * keep the sub-tree consistent with anchor branch `branch_k` (N-1 = fallback: nothing
  * survives) and compact B, frontier hidden rows and slot K/V in place.  DEX_ESTATE unless a
- * commit is pending; DEX_EINVAL if branch_k < N-1 and B[anchor(branch_k)] != token.
+ * commit is pending; DEX_EINVAL if branch_k < N-1 and B[anchor(branch_k)] != token or the branch's continuation
+ * was not explored (sparse lattice, dex_step_result.branch_mask).
  * Used by tests and by the parity harness to teacher-force the oracle's token (R17). */
 int32_t dex_collapse(dex_ctx* ctx, int32_t seq, int32_t branch_k, int32_t token);
 

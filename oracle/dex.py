@@ -116,10 +116,12 @@ def dex_decode(model, prompt, T, X, decs=True, trace=False, state=None, force_to
                 ck[l].append(slot_kv[0][l][0])
                 cv[l].append(slot_kv[0][l][1])
             q_new, mp = lt.collapse_map(k_sel, N)
+            u_before = u
             u = {j: u[o] for j, o in mp.items() if o in u}
             h_out = {j: h_out[o] for j, o in mp.items() if o in h_out}
             slot_kv = {j: slot_kv[o] for j, o in mp.items() if lt.slot_root(j) == j and o in slot_kv}
-            rec.update(committed=1, token=y, match_k=k_sel, ref=ref, q_after=q_new)
+            rec.update(committed=1, token=y, match_k=k_sel, ref=ref, q_after=q_new,
+                       explored=[(2 * lt.anchor(k) + 2) in u_before for k in range(N - 1)])
             q = q_new
         else:
             rec.update(committed=0, q_after=q + 1)

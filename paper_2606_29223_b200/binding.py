@@ -25,7 +25,7 @@ class DexConfig(C.Structure):
                [("rms_eps", C.c_float), ("rope_theta", C.c_float)] + \
                [(n, C.c_int32) for n in ("max_seqs", "max_ctx", "page_size", "decs", "eos_id", "debug_taps",
                                          "act_planes", "use_graph", "round_kernel", "sample")] + \
-               [("temperature", C.c_float), ("sample_seed", C.c_int32), ("adapter_dim", C.c_int32)]
+               [("temperature", C.c_float), ("sample_seed", C.c_int32), ("adapter_dim", C.c_int32), ("lookahead", C.c_int32)]
 
 
 class DexWeights(C.Structure):
@@ -39,7 +39,8 @@ class DexStepResult(C.Structure):
                 ("q_before", C.c_int32), ("q_after", C.c_int32), ("exit_rows", C.c_int32),
                 ("critical_layers", C.c_int32), ("layer_evals", C.c_int64),
                 ("rows_per_stage", C.c_int32 * DEX_MAX_DEPTHS), ("anchor_tokens", C.c_int32 * DEX_MAX_DEPTHS),
-                ("ref_top1", C.c_float), ("ref_top2", C.c_float), ("n_tokens", C.c_int32), ("done", C.c_int32)]
+                ("ref_top1", C.c_float), ("ref_top2", C.c_float), ("n_tokens", C.c_int32), ("done", C.c_int32),
+                ("branch_mask", C.c_int32), ("reserved", C.c_int32)]
 
 
 _SIGNATURES = {
@@ -164,7 +165,7 @@ class Dex:
 
     def __init__(self, shape, weights, depths, max_seqs=1, max_ctx=1024, page_size=128, decs=1, eos_id=-1,
                  debug_taps=0, act_planes=2, use_graph=1, round_kernel=1, sample=0, temperature=1.0, sample_seed=0,
-                 adapters=None, device="cuda:0", stream=None):
+                 adapters=None, lookahead=0, device="cuda:0", stream=None):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2606_29223_b200 needs a CUDA device (no CPU fallback)")
@@ -179,7 +180,7 @@ class Dex:
         self.cfg = DexConfig(shape.n_layers, shape.d_model, shape.n_heads, shape.n_kv_heads, shape.head_dim,
                              shape.d_ffn, shape.vocab, shape.rms_eps, shape.rope_theta, max_seqs, max_ctx, page_size,
                              decs, eos_id, debug_taps, act_planes, use_graph, round_kernel, sample, temperature,
-                             sample_seed, adapter_dim)
+                             sample_seed, adapter_dim, lookahead)
         with torch.cuda.device(self.device):
             self.w = {}
             for k, v in weights.items():
@@ -228,7 +229,7 @@ class Dex:
             recs.append(dict(q=r.q_before, committed=r.committed, token=r.token, match_k=r.match_k,
                              layer_evals=r.layer_evals, critical_layers=r.critical_layers,
                              rows_per_stage=list(r.rows_per_stage), exit_rows=r.exit_rows,
-                             ref_top1=r.ref_top1, ref_top2=r.ref_top2))
+                             ref_top1=r.ref_top1, ref_top2=r.ref_top2, branch_mask=r.branch_mask))
             if r.committed:
                 out.append(r.token)
             if r.done or not r.active:

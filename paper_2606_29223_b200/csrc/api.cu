@@ -55,6 +55,7 @@ struct RingCfg {        // shared-memory ring of the GEMM for a plan
 struct HostSeq {
   int active = 0, q = 0, ctx_len = 0, n_tok = 0, pending = 0, done = 0;
   int anchor_tokens[DEX_MAX_DEPTHS];
+  int branch_mask = 0;
   int last_q_before = 0;
   std::vector<int> pages;
 };
@@ -135,6 +136,7 @@ int validate(const dex_config* cfg, const int32_t* depths, int32_t n) {
   if (cfg->sample && !cfg->round_kernel) return fail(nullptr, DEX_EINVAL, "sampling mode needs round_kernel = 1");
   if (cfg->act_planes != 1 && cfg->act_planes != 2) return fail(nullptr, DEX_EINVAL, "act_planes must be 1 or 2");
   if (cfg->vocab < 2) return fail(nullptr, DEX_EINVAL, "vocab too small");
+  if (cfg->lookahead < 0) return fail(nullptr, DEX_EINVAL, "lookahead must be >= 0");
   if (cfg->adapter_dim < 0 || cfg->adapter_dim % 64 || cfg->adapter_dim > cfg->d_ffn)
     return fail(nullptr, DEX_EINVAL, "adapter_dim must be a multiple of 64 in [0, d_ffn]");
   if (cfg->adapter_dim && !cfg->round_kernel) return fail(nullptr, DEX_EINVAL, "inducing adapters need round_kernel = 1");
@@ -604,6 +606,7 @@ int32_t dex_init(dex_ctx** out, const dex_config* cfg, const dex_weights* w, con
   D.R_cap = L.R_cap; D.R_dec = L.R_dec; D.exit_chunk = L.exit_chunk; D.decs = cfg->decs; D.planes = cfg->act_planes; D.taps = cfg->debug_taps;
   D.sample = cfg->sample; D.inv_tau = cfg->sample ? 1.0f / cfg->temperature : 1.0f; D.sample_seed = (unsigned)cfg->sample_seed;
   D.max_len = L.max_len; D.max_chunks = L.max_chunks; D.ref_tiles = L.ref_tiles;
+  D.lookahead = (cfg->lookahead >= n_depths - 1) ? 0 : cfg->lookahead;   // P >= N-1 is the full lattice
   c->has_ad = cfg->adapter_dim > 0;
   D.ad_m = cfg->adapter_dim;
   if (c->has_ad) { D.ad_b1 = w->ad_b1; D.ad_b2 = w->ad_b2; D.ad_norm = w->ad_norm; D.ad_alpha = w->ad_alpha; }
@@ -818,6 +821,7 @@ int32_t dex_step(dex_ctx* c, uint32_t flags, dex_step_result* out) {
     hs.done = out[s].done;
     hs.pending = (!out[s].committed && out[s].q_before == D.N - 1) ? 1 : 0;
     memcpy(hs.anchor_tokens, out[s].anchor_tokens, sizeof hs.anchor_tokens);
+    hs.branch_mask = out[s].branch_mask;
   }
   return DEX_OK;
 }
@@ -832,6 +836,8 @@ int32_t dex_collapse(dex_ctx* c, int32_t seq, int32_t branch_k, int32_t token) {
   if (token < 0 || token >= c->cfg.vocab) return fail(c, DEX_EINVAL, "token out of range");
   if (branch_k < N - 1 && hs.anchor_tokens[branch_k] != token)
     return fail(c, DEX_EINVAL, "B[anchor(%d)] = %d != token %d", branch_k, hs.anchor_tokens[branch_k], token);
+  if (branch_k < N - 1 && !((hs.branch_mask >> branch_k) & 1))
+    return fail(c, DEX_EINVAL, "the continuation of branch %d was not explored (sparse lattice)", branch_k);
   CU(c, launch_set_cmd(c->D, seq, branch_k, token, c->stream));
   int rc = enqueue_collapse(c);
   if (rc) return rc;

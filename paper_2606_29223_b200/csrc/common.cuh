@@ -86,6 +86,7 @@ struct Dev {
   float inv_tau;           // 1 / temperature
   unsigned sample_seed;
   int max_len;             // max_m |Pi_m|
+  int lookahead;           // P > 0: position look-ahead cap of the sparse lattice (R26); 0: full lattice
   int ad_m;                // inducing-adapter width m (0: exits decode h directly); adapter k serves stage k < N-1
   const float *ad_b1, *ad_b2, *ad_norm, *ad_alpha;   // [N-1][m], [N-1][d], [N-1][d], [N-1]
   // weights

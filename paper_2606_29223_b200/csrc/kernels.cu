@@ -100,6 +100,8 @@ __global__ void k_rows_decode(Dev D, Plan plan) {
   D.best_key[r] = 0ull;
   RowInfo ri;
   ri.valid = 0;
+  ri.seq = 0; ri.node = -1; ri.pos = -1; ri.grp = 0; ri.slot = 0; ri.n_paged = 0; ri.n_anc = 0;   // a clean dead row
+  ri.parent_row = -1; ri.tok_in = 0; ri.is_ref = 0; ri.n_mask = 0;
   if (r < D.R_dec) {
     int m = 0;
     while (m + 1 < D.N && r >= plan.row_base[m + 1]) ++m;
@@ -109,8 +111,12 @@ __global__ void k_rows_decode(Dev D, Plan plan) {
     if (s < D.max_seqs) {
       const SeqState st = D.seqs[s];
       const int q = st.q;
-      if (seq_live(st) && j < stage_count(q, m)) {
-        const int o = (m == q) ? 0 : ((j << (m + 1)) | (1 << m));
+      const int o = (m == q) ? 0 : ((j << (m + 1)) | (1 << m));
+      bool expand = seq_live(st) && j < stage_count(q, m);
+      // sparse lattice (R26): within P positions of the commit position, under an expanded parent (B holds its token)
+      if (expand && D.lookahead > 0 && q > 0)
+        expand = __popc(o) <= D.lookahead && D.B[s * D.n_nodes + node_id(q - 1, o >> 1)] >= 0;
+      if (expand) {
         ri.valid = 1;
         ri.seq = s;
         ri.node = node_id(q, o);
@@ -581,7 +587,7 @@ __global__ void k_decide(Dev D, Plan plan, int auto_collapse) {
     if (lane == 0) {
       res->active = 0; res->committed = 0; res->token = -1; res->match_k = -1;
       res->q_before = st.q; res->q_after = st.q; res->exit_rows = 0; res->critical_layers = 0;
-      res->layer_evals = 0; res->n_tokens = st.n_tok; res->done = st.done;
+      res->layer_evals = 0; res->n_tokens = st.n_tok; res->done = st.done; res->branch_mask = 0; res->reserved = 0;
       for (int i = 0; i < DEX_MAX_DEPTHS; ++i) res->rows_per_stage[i] = 0, res->anchor_tokens[i] = -1;
       res->ref_top1 = 0.f; res->ref_top2 = 0.f;
       D.cmd[s] = cmd;
@@ -590,12 +596,21 @@ __global__ void k_decide(Dev D, Plan plan, int auto_collapse) {
   }
   const int q = st.q, N = D.N;
   // insert: B[node] = u for every new node of level q
+  int cnt[DEX_MAX_DEPTHS];                            // expanded rows per stage (sparse lattice: counted, not 2^{q-1-m})
+#pragma unroll
+  for (int m = 0; m < DEX_MAX_DEPTHS; ++m) cnt[m] = 0;
   for (int o = lane; o < (1 << q); o += 32) {
     const int m = stage_of(q, o);
     const int r = plan.row_base[m] + s * cap_of(N, m) + idx_in_stage(q, o, m);
-    const unsigned long long key = D.best_key[r];
+    const unsigned long long key = D.best_key[r];      // 0 for a row that was not expanded -> B = -1 (empty)
     D.B[s * D.n_nodes + node_id(q, o)] = (int)(0xFFFFFFFFu - (uint32_t)(key & 0xFFFFFFFFull));
+    const int live = D.rows[r].valid;
+#pragma unroll
+    for (int mm = 0; mm < DEX_MAX_DEPTHS; ++mm) cnt[mm] += (mm == m) ? live : 0;
   }
+#pragma unroll
+  for (int m = 0; m < DEX_MAX_DEPTHS; ++m)
+    for (int off = 16; off > 0; off >>= 1) cnt[m] += __shfl_xor_sync(0xffffffffu, cnt[m], off);
   __syncwarp();
   // top-2 of the reference node's logits (reported; the oracle's margin decides flagging, R17)
   float t1 = -INFINITY, t2 = -INFINITY;
@@ -620,11 +635,12 @@ __global__ void k_decide(Dev D, Plan plan, int auto_collapse) {
   if (lane != 0) return;
   res->active = 1;
   res->q_before = q;
-  res->exit_rows = 1 << q;
   long long evals = 0;
-  int crit = 0;
+  int crit = 0, n_exit = 0;
+#pragma unroll
   for (int m = 0; m < DEX_MAX_DEPTHS; ++m) {
-    const int n = (m < N) ? stage_count(q, m) : 0;
+    const int n = (m < N) ? cnt[m] : 0;
+    n_exit += n;
     res->rows_per_stage[m] = n;
     if (n > 0) {
       const int len = D.depths[m] - (m ? D.depths[m - 1] : 0);
@@ -633,16 +649,22 @@ __global__ void k_decide(Dev D, Plan plan, int auto_collapse) {
     }
     res->anchor_tokens[m] = -1;
   }
+  res->exit_rows = n_exit;
   res->layer_evals = evals;
   res->critical_layers = crit;
+  res->branch_mask = 0; res->reserved = 0;
   res->committed = 0; res->token = -1; res->match_k = -1;
   res->ref_top1 = 0.f; res->ref_top2 = 0.f;
   res->n_tokens = st.n_tok; res->done = 0;
   if (q == N - 1) {                                   // ReachFinalDepth(q)
     int ref = D.B[s * D.n_nodes + node_id(N - 1, 0)];
     int k_sel = N - 1;                                // fallback b_{N-1}
+    int explored = 0;                                 // branches whose continuation (position child of anchor k) exists
+    for (int k = 0; k < N - 1; ++k)
+      if (D.B[s * D.n_nodes + node_id(k + 1, 1)] >= 0) explored |= 1 << k;
+    res->branch_mask = explored;
     for (int k = N - 2; k >= 0; --k)
-      if (D.B[s * D.n_nodes + node_id(k, 0)] == ref) k_sel = k;   // shallowest match (R6)
+      if (D.B[s * D.n_nodes + node_id(k, 0)] == ref && ((explored >> k) & 1)) k_sel = k;   // shallowest explored match (R6, R26)
     for (int k = 0; k < N; ++k) res->anchor_tokens[k] = D.B[s * D.n_nodes + node_id(k, 0)];
     res->token = ref; res->match_k = k_sel;
     res->ref_top1 = t1; res->ref_top2 = t2;

@@ -510,6 +510,8 @@ struct AttnSmem {
   __nv_bfloat16 ql[kAttnPairs][HD + 8];
   int ppos[kAttnPairs];                         // position of the pair's row; -1: not in this pass
   int prow[kAttnPairs], phead[kAttnPairs];
+  int n_vrow;                                   // sparse lattice (R26): the expanded rows of the task's (stage, sequence)
+  short vrow[128];
 };
 
 __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc) {
@@ -701,10 +703,27 @@ __device__ void glue_attention(const RoundArgs& a, int j, int tid_e, int lane, i
     const int ca = is_tail ? n_body : rg * CR;
     const int cb = min(is_tail ? a.n_chunks : min(ca + CR, n_body), (st.ctx_len + st.q) / kChunk + 1);   // no row lies beyond ctx_len + q
     if (ca >= cb) continue;
-    const int cnt = r_stage_count(st.q, m);
+    int cnt = r_stage_count(st.q, m);
     const int layer = a.dec.layer_lo[m] + j;
     const int r0 = a.dec.row_base[m] + s * cap_of(D.N, m);
     const int n_paged = st.ctx_len;
+    const bool sparse = D.lookahead > 0;
+    if (sparse) {                                            // compact list of the rows that were expanded (ascending)
+      if (we == 0) {
+        int base = 0;
+        for (int i0 = 0; i0 < cnt; i0 += 32) {
+          const int i = i0 + lane;
+          const bool v = i < cnt && D.rows[r0 + i].valid;
+          const unsigned bal = __ballot_sync(0xffffffffu, v);
+          if (v) sm->vrow[base + __popc(bal & ((1u << lane) - 1u))] = (short)i;
+          base += __popc(bal);
+        }
+        if (lane == 0) sm->n_vrow = base;
+      }
+      bar_epi<GT>();
+      cnt = sm->n_vrow;
+    }
+    auto row_of = [&](int i) { return r0 + (sparse ? (int)sm->vrow[i] : i); };
     const int n_pairs = cnt * Gq;
 
     for (int pb = 0; pb < n_pairs; pb += kAttnPairs) {
@@ -737,7 +756,7 @@ __device__ void glue_attention(const RoundArgs& a, int j, int tid_e, int lane, i
         const int pi = id / HD, t = id - pi * HD;
         float v = 0.f;
         if (pi < np) {
-          const int r = r0 + (pb + pi) / Gq, h = g * Gq + (pb + pi) % Gq;
+          const int r = row_of((pb + pi) / Gq), h = g * Gq + (pb + pi) % Gq;
           v = D.qbuf[((size_t)r * D.nh + h) * HD + t];
         }
         const __nv_bfloat16 hi = __float2bfloat16_rn(v);
@@ -748,7 +767,7 @@ __device__ void glue_attention(const RoundArgs& a, int j, int tid_e, int lane, i
         const int pi = tid_e;
         int pos = -1, r = 0, h = 0;
         if (pi < np) {
-          r = r0 + (pb + pi) / Gq;
+          r = row_of((pb + pi) / Gq);
           h = g * Gq + (pb + pi) % Gq;
           pos = D.rows[r].pos;
           if (pos < ca * kChunk) pos = -1;                   // the row ends before this range
@@ -775,7 +794,7 @@ __device__ void glue_attention(const RoundArgs& a, int j, int tid_e, int lane, i
           if (we >= t_shared && we < 4) {
             const int t = we, p0 = c0 + t * 16;
             for (int rl = 0; rl < n_rl; ++rl) {
-              const int r = r0 + pb / Gq + rl;
+              const int r = row_of(pb / Gq + rl);
               const RowInfo* ri = &D.rows[r];
               const int pos = ri->pos;
               if (pos < p0) continue;                        // the row does not see this tile (warp-uniform)

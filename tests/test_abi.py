@@ -33,8 +33,8 @@ def test_every_declared_symbol_is_exported(P):
 
 
 def test_struct_layout_matches_header(P):
-    assert ctypes.sizeof(P.DexStepResult) == 120
-    assert ctypes.sizeof(P.DexConfig) == 22 * 4
+    assert ctypes.sizeof(P.DexStepResult) == 128
+    assert ctypes.sizeof(P.DexConfig) == 23 * 4
     assert ctypes.sizeof(P.DexWeights) == 15 * ctypes.sizeof(ctypes.c_void_p)
     assert P.DexStepResult.layer_evals.offset == 32
 
@@ -42,7 +42,7 @@ def test_struct_layout_matches_header(P):
 def _cfg(P, **kw):
     base = dict(n_layers=8, d_model=256, n_heads=4, n_kv_heads=4, head_dim=64, d_ffn=688, vocab=1024, rms_eps=1e-5,
                 rope_theta=1e4, max_seqs=1, max_ctx=256, page_size=128, decs=1, eos_id=-1, debug_taps=0, act_planes=2,
-                use_graph=1, round_kernel=1, sample=0, temperature=1.0, sample_seed=0, adapter_dim=0)
+                use_graph=1, round_kernel=1, sample=0, temperature=1.0, sample_seed=0, adapter_dim=0, lookahead=0)
     base.update(kw)
     return P.DexConfig(*[base[n] for n, _ in P.DexConfig._fields_])
 

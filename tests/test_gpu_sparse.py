@@ -1,0 +1,135 @@
+"""Sparse exploration lattice (dex_config.lookahead = P, reading R26) through the C ABI against the
+oracle's trace: which nodes are expanded (rows per stage, exit rows, layer evaluations: bit-exact), every node's
+candidate token (flip only at an oracle margin < 1e-2, R17) and stage-boundary hidden state, the explored-branch
+mask and the commit rule, and the commit invariant: GPU DEX(P) stream == GPU AR stream, bit-identical."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+MARGIN, HID_TOL = 1e-2, 2e-2
+
+
+@pytest.fixture(scope="module")
+def P():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2606_29223_b200 import build
+    build.build()
+    import paper_2606_29223_b200 as P
+    return P
+
+
+@pytest.fixture(scope="module")
+def c1_bf16(c1):
+    from oracle import OracleModel
+    wl, w, p = c1
+    return OracleModel(wl.shape, w, kv_round="bf16")
+
+
+@pytest.mark.parametrize("rk", [1, 0])
+@pytest.mark.parametrize("X,cap", [((2, 4, 6, 8), 1), ((2, 4, 6, 8), 2), (tuple(range(1, 9)), 1), (tuple(range(1, 9)), 2),
+                                   (tuple(range(1, 9)), 3), ((1, 3, 4, 8), 2)])
+def test_c1_sparse_lattice_matches_oracle(P, c1, c1_bf16, X, cap, rk):
+    from oracle import dex_decode
+    wl, w, p = c1
+    T, N = 24, len(X)
+    od = dex_decode(c1_bf16, p, T, X, trace=True, lookahead=cap)
+    g = P.Dex(wl.shape, w, X, max_ctx=128, debug_taps=1, use_graph=0, lookahead=cap, round_kernel=rk)
+    g.prefill(0, p)
+    worst, flagged, n_cmp = 0.0, 0, 0
+    for ri, orec in enumerate(od["rounds"]):
+        r = g.step(0)[0]
+        assert r.q_before == orec["q"], ri
+        assert list(r.rows_per_stage)[:N] == orec["rows_per_stage"], ri
+        assert r.exit_rows == orec["exit_rows"] and r.layer_evals == orec["layer_evals"]
+        assert r.critical_layers == orec["critical_layers"]
+        B = g.tap_B()
+        level = range((1 << orec["q"]) - 1, (2 << orec["q"]) - 1)
+        assert [i for i in level if B[i] >= 0] == orec["nodes"]             # exactly the oracle's nodes were expanded
+        for node in orec["nodes"]:
+            h = g.tap_hidden(node)
+            o = orec["h_out"][node]
+            worst = max(worst, float(np.abs(h[-1] - o).max() / np.abs(o).max()))
+            n_cmp += 1
+            if B[node] != orec["u"][node]:
+                assert orec["u_margin"][node] < MARGIN, (ri, node, B[node], orec["u"][node], orec["u_margin"][node])
+                flagged += 1
+        if flagged:
+            if r.match_k >= 0:
+                g.collapse(0, r.match_k, r.token)
+            break
+        if orec["committed"]:
+            assert [(r.branch_mask >> k) & 1 == 1 for k in range(N - 1)] == orec["explored"], ri
+            assert r.token == orec["token"] and r.match_k == orec["match_k"], ri
+            g.collapse(0, r.match_k, r.token)
+            assert g.tap_fsm()[0] == orec["q_after"]
+        else:
+            assert r.match_k == -1 and r.q_after == orec["q_after"]
+    assert worst < HID_TOL, worst
+    assert n_cmp > 30 or flagged
+    n_have = len(g.tokens()) - len(p)
+    if n_have < T:
+        g.generate(T - n_have)
+    dex_tokens = g.tokens()[len(p):len(p) + T]
+    g.close()
+    a = P.Dex(wl.shape, w, (wl.shape.n_layers,), max_ctx=128, round_kernel=rk)
+    a.prefill(0, p)
+    ar_gpu, _ = a.generate(T)
+    a.close()
+    assert np.array_equal(ar_gpu, dex_tokens)                               # the commit invariant
+
+
+def test_wide_cap_is_the_full_lattice_and_rows_shrink(P, c1):
+    wl, w, p = c1
+    X = tuple(range(1, 9))
+    runs = {}
+    for cap in (0, 7, 9, 2):
+        g = P.Dex(wl.shape, w, X, max_ctx=128, lookahead=cap)
+        g.prefill(0, p)
+        toks, recs = g.generate(32)
+        runs[cap] = (toks.tolist(), [(r["q"], r["rows_per_stage"], r["match_k"]) for r in recs],
+                     sum(r["layer_evals"] for r in recs))
+        g.close()
+    assert runs[7][:2] == runs[0][:2] and runs[9][:2] == runs[0][:2]
+    assert runs[2][0] == runs[0][0] and runs[2][2] < runs[0][2] // 2
+
+
+def test_collapse_onto_unexplored_branch_is_refused_and_batched_streams(P, c1):
+    import dex_synth
+    wl, w, p = c1
+    X = (2, 4, 6, 8)
+    g = P.Dex(wl.shape, w, X, max_ctx=128, lookahead=1, use_graph=0)
+    g.prefill(0, p)
+    seen = False
+    for _ in range(200):
+        r = g.step(0)[0]
+        if r.match_k < 0:
+            continue
+        missing = [k for k in range(len(X) - 1) if not (r.branch_mask >> k) & 1]
+        if missing and not seen:
+            seen = True
+            with pytest.raises(P.DexError) as e:
+                g.collapse(0, missing[0], r.anchor_tokens[missing[0]])
+            assert e.value.code == P.DEX_EINVAL
+        g.collapse(0, r.match_k, r.token)
+    assert seen                                                             # holes do appear after a collapse at P = 1
+    g.close()
+    # two sequences, graph replay, auto-collapse: each stream equals its own single-sequence stream
+    p2 = dex_synth.make_prompt(wl.shape.vocab, 19, 5)
+    T = 32
+    ref = []
+    for pr in (p, p2):
+        s = P.Dex(wl.shape, w, (wl.shape.n_layers,), max_ctx=128)
+        s.prefill(0, pr)
+        ref.append(s.generate(T)[0])
+        s.close()
+    b = P.Dex(wl.shape, w, X, max_seqs=2, max_ctx=128, lookahead=2)
+    b.prefill(0, p)
+    b.prefill(1, p2)
+    for _ in range(4 * T):
+        b.step()
+    assert np.array_equal(b.tokens(0)[len(p):len(p) + T], ref[0])
+    assert np.array_equal(b.tokens(1)[len(p2):len(p2) + T], ref[1])
+    b.close()
