@@ -212,7 +212,8 @@ def bench_dex(args):
     adapters = None
     if args.adapters:                    # inducing-adapter exits: synthetic, untrained
         adapters = dex_synth.make_adapters(shape, N - 1, seed=wl.weight_seed + 1, alpha=1e-3, m=args.adapter_dim)
-    g = P.Dex(shape, w_dev, X, max_ctx=max_ctx, device=dev, act_planes=args.act_planes, adapters=adapters, **mode)
+    g = P.Dex(shape, w_dev, X, max_ctx=max_ctx, device=dev, act_planes=args.act_planes, adapters=adapters,
+              lookahead=args.lookahead, **mode)
     a = P.Dex(shape, w_dev, (L,), max_ctx=max_ctx, device=dev, act_planes=args.act_planes, **mode)
     g.prefill(0, prompt)
     a.prefill(0, prompt)
@@ -332,7 +333,8 @@ def bench_dex(args):
             "dtype": "bf16", "data": "synthetic",
             "config": {"workload": f"{wl.key}: {shape.name} L={L} d={shape.d_model} X={list(X)} prompt={n_prompt} "
                                    f"gen={T} bs=1 {'greedy' if args.temperature <= 0 else 'sample T=%g' % args.temperature} decs={args.decs}"
-                                   + (f" adapters m={adapters['w1'].shape[1]} (random init)" if adapters is not None else ""),
+                                   + (f" adapters m={adapters['w1'].shape[1]} (random init)" if adapters is not None else "")
+                                   + (f" lookahead={args.lookahead}" if args.lookahead else ""),
                        "parallelism": "replicas only" if world > 1 else "single GPU",
                        "act_planes": args.act_planes,
                        "l2": "inputs larger than L2 (13.5 GB of weights streamed per pass vs 126 MB L2)",
@@ -431,6 +433,7 @@ def main():
     ap.add_argument("--decs", type=int, default=1, help="1: DECS masking (Alg. 2), 0: vanilla decoding of the exits")
     ap.add_argument("--temperature", type=float, default=0.0, help="> 0: sampling-mode DECS (Alg. 2 lines 10-15)")
     ap.add_argument("--sample-seed", type=int, default=2024)
+    ap.add_argument("--lookahead", type=int, default=0, help="P > 0: sparse lattice, position look-ahead cap (PAPER.md:534)")
     ap.add_argument("--adapters", type=int, default=0, help="1: inducing-adapter exits at the non-final depths (random init)")
     ap.add_argument("--adapter-dim", type=int, default=0, help="adapter width m (0: 2 d_model, the paper's)")
     ap.add_argument("--gen-len", type=int, default=0)

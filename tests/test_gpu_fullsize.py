@@ -110,7 +110,8 @@ def _generate_all(g, n_seqs, T):
             if not r.active or len(toks[s]) >= T:
                 continue
             recs[s].append(dict(q=r.q_before, committed=r.committed, token=r.token, k=r.match_k, evals=r.layer_evals,
-                                rows=list(r.rows_per_stage), anchor=list(r.anchor_tokens), exit_rows=r.exit_rows))
+                                rows=list(r.rows_per_stage), anchor=list(r.anchor_tokens), exit_rows=r.exit_rows,
+                                mask=r.branch_mask))
             if r.committed:
                 toks[s].append(r.token)
     return toks, recs
@@ -149,6 +150,25 @@ def test_fullsize_dex_equals_ar_counts_and_gemm(P, key, T):
             if r["committed"]:
                 assert r["token"] == r["anchor"][N - 1]                       # y = u_{N-1}
                 assert r["k"] == next((i for i in range(N) if r["anchor"][i] == r["token"]), N - 1)
+    g.close()
+    # sparse lattice (R26) at full size: same stream, rows within the binomial bound of the cap,
+    # commit = shallowest matching anchor whose continuation was explored
+    from math import comb
+    cap = 2
+    g = P.Dex(wl.shape, wd, X, max_seqs=S, max_ctx=wl.prompt_len + T + 8, lookahead=cap)
+    for s in range(S):
+        g.prefill(s, prompts[s])
+    stoks, srecs = _generate_all(g, S, T)
+    for s in range(S):
+        assert stoks[s][:T] == ar_toks[s][:T], (key, s, "sparse")
+        for r in srecs[s]:
+            q = r["q"]
+            assert r["exit_rows"] == sum(r["rows"][:N]) <= sum(comb(q, j) for j in range(min(cap, q) + 1))
+            assert r["rows"][q] == 1 and r["evals"] == sum(n * ln for n, ln in zip(r["rows"][:N], lens))
+            if r["committed"]:
+                assert r["token"] == r["anchor"][N - 1]
+                assert r["k"] == next((i for i in range(N - 1) if r["anchor"][i] == r["token"] and (r["mask"] >> i) & 1), N - 1)
+        assert sum(r["evals"] for r in srecs[s]) < sum(r["evals"] for r in recs[s])
     # sampled GEMM outputs of this shape
     d = P.Dex(wl.shape, wd, X, max_seqs=1, max_ctx=256, debug_taps=1, use_graph=0)
     rng = np.random.default_rng(5)
