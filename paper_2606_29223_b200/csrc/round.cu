@@ -786,30 +786,60 @@ __device__ void glue_attention(const RoundArgs& a, int j, int tid_e, int lane, i
           const uint32_t kb = smem_u32(sm->kv[buf][0]), vb = smem_u32(sm->kv[buf][1]);
           const int t_shared = max(0, min(4, (n_paged - c0) / 16));   // tiles whose 16 positions are all committed:
           if (we < t_shared) attn_tile<HD>(D, sm, kb, vb, we * 16, c, we, 0, np, lane);   // every pair shares them
-          // tiles that hold private positions: warp t owns tile t of the staged chunk and takes the lattice rows one
-          // at a time, patching the row's ancestor / own K/V rows (from their slots) into the tile IN PLACE at their
+          // tiles that hold private positions: warp t owns tile t of the staged chunk and takes lattice rows one at a
+          // time, patching the row's ancestor / own K/V rows (from their slots) into the tile IN PLACE at their
           // positions.  Rows above the row's own position keep finite data (zeros or an earlier row's patch): they
           // are masked and enter the P.V MMA with weight 0.  No CTA-wide synchronisation: tiles are disjoint.
+          // On the LAST chunk of the range the other staging buffer is idle: warps 4-7 copy the committed rows of a
+          // private tile into a 16-row slot of it and share the tile's lattice rows with the owner (same
+          // instructions on the same tile contents -> same bits, H3).
           const int n_rl = (np + Gq - 1) / Gq;
+          const int t_hi = min(3, (st.ctx_len + st.q - c0) / 16);     // last tile a row of this sequence can see
+          const int n_pt = t_hi - t_shared + 1;                         // tiles with private positions
+          const bool par = c == cb - 1 && n_rl > 1 && n_pt >= 1 && GT / 32 >= 8;
+          int t = -1, rank = 0, nk = 1, tb = buf, trow = 0;
           if (we >= t_shared && we < 4) {
-            const int t = we, p0 = c0 + t * 16;
-            for (int rl = 0; rl < n_rl; ++rl) {
+            t = we; trow = t * 16;
+            if (par && t <= t_hi) nk = 1 + (4 - (t - t_shared) + n_pt - 1) / n_pt;
+          } else if (par && we >= 4 && we < 8) {
+            const int h = we - 4;
+            t = t_shared + h % n_pt; rank = 1 + h / n_pt; nk = 1 + (4 - (t - t_shared) + n_pt - 1) / n_pt;
+            tb = buf ^ 1; trow = h * 16;
+          }
+          if (t >= 0) {
+            const int p0 = c0 + t * 16;
+            const int i_lo = max(n_paged - p0, 0);
+            if (tb != buf) {                                 // helper: committed rows of the tile, zeros above
+              for (int id = lane; id < 16 * CPR; id += 32) {
+                const int i = id / CPR, cj = id % CPR;
+                uint4 kk = make_uint4(0u, 0u, 0u, 0u), vv = kk;
+                if (i < i_lo) {
+                  kk = *reinterpret_cast<const uint4*>(&sm->kv[buf][0][(t * 16 + i) * HD + cj * 8]);
+                  vv = *reinterpret_cast<const uint4*>(&sm->kv[buf][1][(t * 16 + i) * HD + cj * 8]);
+                }
+                *reinterpret_cast<uint4*>(&sm->kv[tb][0][(trow + i) * HD + cj * 8]) = kk;
+                *reinterpret_cast<uint4*>(&sm->kv[tb][1][(trow + i) * HD + cj * 8]) = vv;
+              }
+              __syncwarp();
+            }
+            const uint32_t kbt = smem_u32(sm->kv[tb][0]), vbt = smem_u32(sm->kv[tb][1]);
+            for (int rl = rank; rl < n_rl; rl += nk) {
               const int r = row_of(pb / Gq + rl);
               const RowInfo* ri = &D.rows[r];
               const int pos = ri->pos;
               if (pos < p0) continue;                        // the row does not see this tile (warp-uniform)
-              const int i_lo = max(n_paged - p0, 0), i_hi = min(pos - p0, 15);
+              const int i_hi = min(pos - p0, 15);
               for (int id = lane; id < (i_hi - i_lo + 1) * CPR; id += 32) {
-                const int i = i_lo + id / CPR, cj = id % CPR, pl = t * 16 + i;
+                const int i = i_lo + id / CPR, cj = id % CPR, pl = trow + i;
                 const int ai = p0 + i - n_paged;
                 const int slot = (ai < ri->n_anc) ? ri->anc[ai] : ri->slot;
                 const size_t so = slot_off(D, s, slot, layer) + (size_t)g * HD + cj * 8;
                 const int dj = (cj ^ (pl & 7)) * 8;
-                *reinterpret_cast<uint4*>(&sm->kv[buf][0][pl * HD + dj]) = *reinterpret_cast<const uint4*>(D.kslot + so);
-                *reinterpret_cast<uint4*>(&sm->kv[buf][1][pl * HD + dj]) = *reinterpret_cast<const uint4*>(D.vslot + so);
+                *reinterpret_cast<uint4*>(&sm->kv[tb][0][pl * HD + dj]) = *reinterpret_cast<const uint4*>(D.kslot + so);
+                *reinterpret_cast<uint4*>(&sm->kv[tb][1][pl * HD + dj]) = *reinterpret_cast<const uint4*>(D.vslot + so);
               }
               __syncwarp();
-              attn_tile<HD>(D, sm, kb, vb, t * 16, c, t, rl * Gq, min(np, (rl + 1) * Gq), lane);
+              attn_tile<HD>(D, sm, kbt, vbt, trow, c, t, rl * Gq, min(np, (rl + 1) * Gq), lane);
               __syncwarp();
             }
           }
