@@ -670,9 +670,14 @@ __device__ __forceinline__ void attn_tile(const Dev& D, AttnSmem<HD>* sm, uint32
   }
 }
 
-template <int HD, int GT>
+// PT (pass tasks): a task also fixes ONE pass of <= 16 (row, head) pairs of its (stage, sequence).  Passes re-stage
+// the chunks anyway, and as tasks of their own a wide stage (64 rows at N = 8, 16 passes with GQA) spreads over
+// the grid instead of running its passes back to back on one CTA; with more tasks than CTAs the ranges are dealt
+// from the LAST one (private positions, merges: the heaviest tasks first).  A separate instantiation because
+// lattices whose stages all fit one pass (N <= 5 at MHA) keep the simpler loop and its register allocation.
+template <int HD, int GT, bool PT>
 __device__ void glue_attention(const RoundArgs& a, int j, int tid_e, int lane, int we, int cta, int G,
-                               AttnSmem<HD>* sm, int n_live_ms) {
+                               AttnSmem<HD>* sm, int n_live_ms, const int* cum) {
   constexpr int CPR = HD / 8;                                // 16-byte pieces per K/V row
   constexpr int kEpiThreads = GT;
   const Dev& D = a.D;
@@ -688,15 +693,30 @@ __device__ void glue_attention(const RoundArgs& a, int j, int tid_e, int lane, i
   const int nr_body = tail_own ? nr_fit - 1 : max(nr_fit, 1);
   const int CR = nr_fit >= 1 ? max(1, (n_body + nr_body - 1) / nr_body) : 3;
   const int n_ranges = (n_body + CR - 1) / CR + (tail_own ? 1 : 0);
-  const int per_ms = D.nkv * n_ranges;
-  const int n_tasks = D.N * D.max_seqs * per_ms;
   const int Gq = D.nh / D.nkv;
   const size_t kv_stride = (size_t)D.nkv * HD;
+  const int per_ms = D.nkv * n_ranges;
+  const int fam = PT ? cum[D.N] * D.nkv : 0;                 // cum[m]: (sequence, pass) slots of the stages before m (shared memory)
+  const int n_tasks = PT ? fam * n_ranges : D.N * D.max_seqs * per_ms;
 
   for (int u = cta; u < n_tasks; u += G) {
-    const int ms = u / per_ms, rem = u - ms * per_ms;
-    const int m = ms / D.max_seqs, s = ms - m * D.max_seqs;
-    const int g = rem / n_ranges, rg = rem - g * n_ranges;
+    int m, s, g, rg, pb_task = 0;
+    if constexpr (PT) {
+      const bool lpt = n_tasks > G;                          // one wave: range fastest, as without pass tasks
+      rg = lpt ? n_ranges - 1 - u / fam : u % n_ranges;
+      const int rem = lpt ? u % fam : u / n_ranges;
+      const int psi = rem / D.nkv;
+      g = rem - psi * D.nkv;
+      m = 0;
+      while (psi >= cum[m + 1]) ++m;
+      const int pp_m = (cum[m + 1] - cum[m]) / D.max_seqs;
+      s = (psi - cum[m]) / pp_m;
+      pb_task = ((psi - cum[m]) % pp_m) * kAttnPairs;
+    } else {
+      const int ms = u / per_ms, rem = u - ms * per_ms;
+      m = ms / D.max_seqs; s = ms - m * D.max_seqs;
+      g = rem / n_ranges; rg = rem - g * n_ranges;
+    }
     const SeqState st = D.seqs[s];
     if (!r_seq_live(st) || st.q < m || j >= a.dec.layer_len[m]) continue;
     const bool is_tail = tail_own && rg == n_ranges - 1;
@@ -725,8 +745,9 @@ __device__ void glue_attention(const RoundArgs& a, int j, int tid_e, int lane, i
     }
     auto row_of = [&](int i) { return r0 + (sparse ? (int)sm->vrow[i] : i); };
     const int n_pairs = cnt * Gq;
+    if (PT && pb_task >= n_pairs) continue;                  // this pass has no pairs at the sequence's FSM state
 
-    for (int pb = 0; pb < n_pairs; pb += kAttnPairs) {
+    for (int pb = pb_task; pb < (PT ? min(n_pairs, pb_task + kAttnPairs) : n_pairs); pb += kAttnPairs) {
       const int np = min(kAttnPairs, n_pairs - pb);
       auto stage = [&](int c, int buf) {
         const int c0 = c * kChunk;
@@ -870,7 +891,7 @@ __device__ void glue_attention(const RoundArgs& a, int j, int tid_e, int lane, i
 }
 
 // ---------------------------------------------------------------- the kernel
-template <int kMaxThreads>
+template <int kMaxThreads, bool PT>
 __global__ void __launch_bounds__(kMaxThreads, 1) k_round(const __grid_constant__ TmSet tm, const __grid_constant__ RoundArgs a) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
@@ -888,6 +909,7 @@ __global__ void __launch_bounds__(kMaxThreads, 1) k_round(const __grid_constant_
   __shared__ int s_nb[16];
   __shared__ uint32_t s_valid[32];
   __shared__ int s_live_ms;
+  __shared__ int s_cum[kMaxGrp + 1];
   __shared__ int s_steps;
   __shared__ unsigned s_seen;
 
@@ -907,11 +929,21 @@ __global__ void __launch_bounds__(kMaxThreads, 1) k_round(const __grid_constant_
     s_steps = steps;
     s_seen = 0;
     int lm = 0;
-    for (int s = 0; s < D.max_seqs; ++s) {
+    for (int s = 0; s < D.max_seqs; ++s) {                   // live (stage, sequence[, 16-pair pass]) attention families
       const SeqState st = D.seqs[s];
-      if (r_seq_live(st)) lm += min(st.q, D.N - 1) + 1;
+      if (!r_seq_live(st)) continue;
+      if constexpr (PT) {
+        for (int m = 0; m <= min(st.q, D.N - 1); ++m) lm += (r_stage_count(st.q, m) * (D.nh / D.nkv) + 15) / 16;
+      } else {
+        lm += min(st.q, D.N - 1) + 1;
+      }
     }
     s_live_ms = lm;
+    if constexpr (PT) {
+      s_cum[0] = 0;
+      for (int m = 0; m < kMaxGrp; ++m)
+        s_cum[m + 1] = s_cum[m] + (m < D.N ? D.max_seqs * ((cap_of(D.N, m) * (D.nh / D.nkv) + 15) / 16) : 0);
+    }
     for (int i = 0; i < NS; ++i) {
       mbar_init(&full[i], 1);
       mbar_init(&empty[i], 1);
@@ -1074,8 +1106,8 @@ __global__ void __launch_bounds__(kMaxThreads, 1) k_round(const __grid_constant_
         ++gb; grid_bar<GT>(D.gbar, gb * G, tid_e, &s_seen, gb); stamp();
         {
           void* asm_ = smem + a.attn_smem_off;
-          if (D.hd == 128) glue_attention<128, GT>(a, j, tid_e, lane, we, blockIdx.x, G, reinterpret_cast<AttnSmem<128>*>(asm_), s_live_ms);
-          else glue_attention<64, GT>(a, j, tid_e, lane, we, blockIdx.x, G, reinterpret_cast<AttnSmem<64>*>(asm_), s_live_ms);
+          if (D.hd == 128) glue_attention<128, GT, PT>(a, j, tid_e, lane, we, blockIdx.x, G, reinterpret_cast<AttnSmem<128>*>(asm_), s_live_ms, s_cum);
+          else glue_attention<64, GT, PT>(a, j, tid_e, lane, we, blockIdx.x, G, reinterpret_cast<AttnSmem<64>*>(asm_), s_live_ms, s_cum);
         }
         stamp();
         ++gb; grid_bar<GT>(D.gbar, gb * G, tid_e, &s_seen, gb); stamp();
@@ -1121,7 +1153,9 @@ __global__ void __launch_bounds__(kMaxThreads, 1) k_round(const __grid_constant_
 size_t round_attn_smem(int hd) { return hd == 128 ? sizeof(AttnSmem<128>) : sizeof(AttnSmem<64>); }
 
 cudaError_t round_init() {
-  return cudaFuncSetAttribute(k_round<kRoundThreads>, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024);
+  cudaError_t e = cudaFuncSetAttribute(k_round<kRoundThreads, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024);
+  if (e != cudaSuccess) return e;
+  return cudaFuncSetAttribute(k_round<kRoundThreads, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024);
 }
 
 // Cooperative launch: all CTAs must be co-resident (they meet at grid barriers).
@@ -1136,7 +1170,9 @@ cudaError_t launch_round(const TmSet& tm, const RoundArgs& a, int grid, size_t s
   at[0].val.cooperative = 1;
   cfg.attrs = at;
   cfg.numAttrs = 1;
-  return cudaLaunchKernelEx(&cfg, k_round<kRoundThreads>, tm, a);
+  // pass tasks only where a (stage, sequence) can hold more than one 16-pair pass
+  if (cap_of(a.D.N, 0) * (a.D.nh / a.D.nkv) > kAttnPairs) return cudaLaunchKernelEx(&cfg, k_round<kRoundThreads, true>, tm, a);
+  return cudaLaunchKernelEx(&cfg, k_round<kRoundThreads, false>, tm, a);
 }
 
 }  // namespace dexk
