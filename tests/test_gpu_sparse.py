@@ -133,3 +133,26 @@ def test_collapse_onto_unexplored_branch_is_refused_and_batched_streams(P, c1):
     assert np.array_equal(b.tokens(0)[len(p):len(p) + T], ref[0])
     assert np.array_equal(b.tokens(1)[len(p2):len(p2) + T], ref[1])
     b.close()
+
+
+def test_sparse_lattice_with_adapters_and_sampling(P, c1):
+    """All optional pieces together (sampling-mode DECS, inducing adapters, look-ahead cap, two sequences, graph
+    replay): the stream is still the GPU AR sampling stream with the same Gumbel rows."""
+    import dex_synth
+    wl, w, p = c1
+    X, T = (1, 2, 3, 4, 6, 8), 32
+    ad = dex_synth.make_adapters(wl.shape, len(X) - 1, seed=3, alpha=0.5, m=256)
+    p2 = dex_synth.make_prompt(wl.shape.vocab, 23, 9)
+    kw = dict(sample=1, temperature=0.9, sample_seed=11)
+    a = P.Dex(wl.shape, w, (wl.shape.n_layers,), max_seqs=2, max_ctx=128, **kw)
+    g = P.Dex(wl.shape, w, X, max_seqs=2, max_ctx=128, adapters=ad, lookahead=2, **kw)
+    out = []
+    for d in (a, g):
+        d.prefill(0, p)
+        d.prefill(1, p2)
+        for _ in range(6 * T):
+            d.step()
+        out.append((d.tokens(0)[len(p):len(p) + T].tolist(), d.tokens(1)[len(p2):len(p2) + T].tolist()))
+        d.close()
+    assert len(out[0][0]) == T and len(out[0][1]) == T
+    assert out[0] == out[1]
