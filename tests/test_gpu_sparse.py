@@ -156,3 +156,29 @@ def test_sparse_lattice_with_adapters_and_sampling(P, c1):
         d.close()
     assert len(out[0][0]) == T and len(out[0][1]) == T
     assert out[0] == out[1]
+
+
+@pytest.mark.parametrize("cap", [0, 3])
+def test_two_wide_lattices_batched(P, c1, cap):
+    """N = 8 with two sequences: 128 stage-0 rows, the pass-task instantiation of the round kernel, sequences at
+    different FSM states in the same launches; each stream equals its own AR stream."""
+    import dex_synth
+    wl, w, p = c1
+    X, T = tuple(range(1, 9)), 24
+    p2 = dex_synth.make_prompt(wl.shape.vocab, 37, 21)
+    ref = []
+    for pr in (p, p2):
+        s = P.Dex(wl.shape, w, (wl.shape.n_layers,), max_ctx=128)
+        s.prefill(0, pr)
+        ref.append(s.generate(T)[0])
+        s.close()
+    b = P.Dex(wl.shape, w, X, max_seqs=2, max_ctx=128, lookahead=cap)
+    b.prefill(0, p)
+    b.step()
+    b.step()                      # sequence 0 is two rounds ahead when sequence 1 joins
+    b.prefill(1, p2)
+    for _ in range(9 * T):
+        b.step()
+    assert np.array_equal(b.tokens(0)[len(p):len(p) + T], ref[0])
+    assert np.array_equal(b.tokens(1)[len(p2):len(p2) + T], ref[1])
+    b.close()
