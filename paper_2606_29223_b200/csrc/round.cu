@@ -691,7 +691,10 @@ __device__ void glue_attention(const RoundArgs& a, int j, int tid_e, int lane, i
   const bool tail_own = nr_fit >= 2 && a.n_chunks >= 2;
   const int n_body = tail_own ? a.n_chunks - 1 : a.n_chunks;
   const int nr_body = tail_own ? nr_fit - 1 : max(nr_fit, 1);
-  const int CR = nr_fit >= 1 ? max(1, (n_body + nr_body - 1) / nr_body) : 3;
+  // more families than CTAs: ranges sized for about four tasks per CTA (a task's fixed cost - q staging, first
+  // stage, counters, merges - is several chunks' worth), at least 3 chunks
+  const int nr_many = max(1, (4 * G) / n_msg);
+  const int CR = nr_fit >= 1 ? max(1, (n_body + nr_body - 1) / nr_body) : max(3, (n_body + nr_many - 1) / nr_many);
   const int n_ranges = (n_body + CR - 1) / CR + (tail_own ? 1 : 0);
   const int Gq = D.nh / D.nkv;
   const size_t kv_stride = (size_t)D.nkv * HD;
