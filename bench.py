@@ -439,7 +439,7 @@ def main():
     ap.add_argument("--gen-len", type=int, default=0)
     ap.add_argument("--prompt-len", type=int, default=0)
     ap.add_argument("--act-planes", type=int, default=2)
-    ap.add_argument("--cpu-tokens", type=int, default=4)
+    ap.add_argument("--cpu-tokens", type=int, default=24, help="committed tokens of the oracle sample (c2: about 13 s of CPU work)")
     ap.add_argument("--no-cpu", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":
