@@ -17,7 +17,8 @@ from .gumbel import gumbel_row, perturbed
 from .model import argmax_lowest
 
 
-def dex_decode(model, prompt, T, X, decs=True, trace=False, state=None, force_tokens=None, sample=None, lookahead=0):
+def dex_decode(model, prompt, T, X, decs=True, trace=False, state=None, force_tokens=None, sample=None, lookahead=0,
+               force_u=None):
     """Returns dict with tokens [T], match_k [T] (anchor index b_k selected at each commit),
     rounds (list of per-round records) and totals.  `force_tokens` (optional [T]) replaces the
     committed token y (teacher forcing used by the GPU parity harness, R17) - never set when
@@ -25,7 +26,12 @@ def dex_decode(model, prompt, T, X, decs=True, trace=False, state=None, force_to
     shared Gumbel rows of oracle/gumbel.py (reading R24); None: greedy.  `lookahead` = P > 0: the sparse lattice of
     reading R26 ("prune low-value branches or construct sparse exploration lattices while preserving
     the final-depth commit invariant"): a node is expanded only if it lies at most P token positions ahead of the
-    commit position and its parent was expanded; 0: the full lattice of Sec. 3.2."""
+    commit position and its parent was expanded; 0: the full lattice of Sec. 3.2.
+    `force_u` (optional dict {(round index, node): token}) replaces the candidate token DECS decodes for that node
+    (teacher forcing of EVERY exit decision, used by the GPU parity harness: reading R17b in DESIGN.md); the gap
+    between the oracle's own arg-max and the forced token among the node's unmasked logits is recorded in
+    rec["u_forced"][node] so that the harness can require it to be a near-tie.  Never set when checking
+    losslessness or any other pin."""
     X = check_X(X, model.L)
     N = len(X)
     lo = [0] + X[:-1]                          # d_{k-1}, with d_{-1}=0
@@ -82,6 +88,11 @@ def dex_decode(model, prompt, T, X, decs=True, trace=False, state=None, force_to
             if decs and i != ref_node:         # Alg. 2 lines 1-4: reference node never masked
                 masked = {u[a] if a in u else new_u[a] for a in lt.slot_chain_prior(i)}
             new_u[i] = argmax_lowest(logits, sorted(masked))
+            if force_u is not None and (len(rounds), i) in force_u and int(force_u[(len(rounds), i)]) != new_u[i]:
+                tok = int(force_u[(len(rounds), i)])
+                gap = np.inf if tok in masked else float(logits[new_u[i]] - logits[tok])
+                rec.setdefault("u_forced", {})[i] = (new_u[i], tok, gap)
+                new_u[i] = tok
             if trace:                          # trace only: top-2 gap among the unmasked logits of node i
                 lm = logits.copy()
                 lm[sorted(masked)] = -np.inf

@@ -4,6 +4,7 @@
 #include <algorithm>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <map>
 #include <memory>
@@ -82,6 +83,8 @@ struct dex_ctx {
   RingCfg round_ring;
   int round_attn_off;
   bool round_ok;                      // the round kernel's ring + attention scratch fit shared memory
+  int pf_mode;
+  int pf_dist, pf_lead;               // L2 prefetcher of the round kernel (ring stages ahead of the weight producer)
   bool has_ad;                        // inducing-adapter exits (cfg.adapter_dim > 0, N >= 2): round kernel only
   std::map<long long, cudaGraphExec_t> graphs;
   std::string err;
@@ -427,6 +430,9 @@ int enqueue_round(dex_ctx* c, int n_chunks) {
   a.stacked = c->round_ring.stacked;
   a.n_chunks = n_chunks;
   a.attn_smem_off = c->round_attn_off;
+  a.pf_dist = c->pf_dist;
+  a.pf_lead = c->pf_lead;
+  a.pf_mode = c->pf_mode;
   ph_begin(c, PH_GEMM);
   CU(c, launch_round(c->tms, a, c->n_sms, c->round_ring.smem, c->stream));
   ph_end(c, PH_GEMM);
@@ -608,6 +614,14 @@ int32_t dex_init(dex_ctx** out, const dex_config* cfg, const dex_weights* w, con
   D.max_len = L.max_len; D.max_chunks = L.max_chunks; D.ref_tiles = L.ref_tiles;
   D.lookahead = (cfg->lookahead >= n_depths - 1) ? 0 : cfg->lookahead;   // P >= N-1 is the full lattice
   c->has_ad = cfg->adapter_dim > 0;
+  {   // tuning knobs of the round kernel's L2 prefetcher; the defaults are the measured optimum
+    const char* e1 = getenv("DEX_PF_DIST");
+    const char* e2 = getenv("DEX_PF_LEAD");
+    c->pf_dist = e1 ? atoi(e1) : 0;
+    c->pf_lead = e2 ? atoi(e2) : 2;
+    const char* e3 = getenv("DEX_PF_MODE");
+    c->pf_mode = e3 ? atoi(e3) : 0;
+  }
   D.ad_m = cfg->adapter_dim;
   if (c->has_ad) { D.ad_b1 = w->ad_b1; D.ad_b2 = w->ad_b2; D.ad_norm = w->ad_norm; D.ad_alpha = w->ad_alpha; }
   D.embed = static_cast<const __nv_bfloat16*>(w->embed);

@@ -249,6 +249,8 @@ struct RoundArgs {
   int x_cap, n_stages, acc_cols, stacked;   // shared-memory ring / TMEM geometry
   int n_chunks;                    // attention chunks that can hold a live position (host upper bound)
   int attn_smem_off;               // byte offset of the attention scratch (AttnSmem) in dynamic shared memory
+  int pf_mode;
+  int pf_dist, pf_lead;            // L2 prefetcher: ring stages it may run ahead of the weight producer (0: off) / minimum lead
 };
 
 }  // namespace dexk

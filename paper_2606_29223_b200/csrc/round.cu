@@ -32,7 +32,7 @@ namespace dexk {
 // warps: 0 weight TMA, 1 MMA, 2-5 GEMM epilogue + glue, 6 activation TMA, 7-10 glue only.  A lone warp per
 // scheduler runs the glue phases latency-bound; two per scheduler measured best (12 glue warps push the kernel
 // under 128 registers and spill).
-constexpr int kRoundThreads = 352;
+constexpr int kRoundThreads = 384;
 
 // ---------------------------------------------------------------- small device helpers
 template <int GT>
@@ -915,6 +915,7 @@ __global__ void __launch_bounds__(kMaxThreads, 1) k_round(const __grid_constant_
   __shared__ int s_cum[kMaxGrp + 1];
   __shared__ int s_steps;
   __shared__ unsigned s_seen;
+  __shared__ unsigned s_wpos;        // ring stages requested so far by the weight producer (read by the L2 prefetcher)
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   if (threadIdx.x < 32) s_valid[threadIdx.x] = 0;
@@ -931,6 +932,7 @@ __global__ void __launch_bounds__(kMaxThreads, 1) k_round(const __grid_constant_
     }
     s_steps = steps;
     s_seen = 0;
+    s_wpos = 0;
     int lm = 0;
     for (int s = 0; s < D.max_seqs; ++s) {                   // live (stage, sequence[, 16-pair pass]) attention families
       const SeqState st = D.seqs[s];
@@ -979,7 +981,7 @@ __global__ void __launch_bounds__(kMaxThreads, 1) k_round(const __grid_constant_
     if (warp == 0) {
       // ===================== weight producer: always as far ahead as the ring allows =====================
       Walker w;
-      unsigned st = 0, ph = 0;
+      unsigned st = 0, ph = 0, n_req = 0;
       bool wrapped = false;
       for (w.start(sq); w.valid; w.next(sq)) {
         const CUtensorMap* desc = &tm.w[w.o.which];
@@ -987,12 +989,44 @@ __global__ void __launch_bounds__(kMaxThreads, 1) k_round(const __grid_constant_
         const int c1 = w.it.tile * kTileM, c2 = w.it.layer;
         for (int kb = w.it.kb0; kb < w.it.kb1; ++kb) {
           if (wrapped) mbar_wait(&empty[st], ph ^ 1u);
+          ++n_req;
           if (elect_one()) {
             mbar_expect_tx(&full[st], tx);
-            tma_load_3d(smem + (size_t)st * stage_bytes, desc, &full[st], kb * kTileK, c1, c2, kEvictFirst);
+            tma_load_3d(smem + (size_t)st * stage_bytes, desc, &full[st], kb * kTileK, c1, c2, (a.pf_mode & 1) ? kEvictNormal : kEvictFirst);
+            if (a.pf_dist > 0) *reinterpret_cast<volatile unsigned*>(&s_wpos) = n_req;
           }
           __syncwarp();
           if (++st == (unsigned)NS) { st = 0; ph ^= 1u; wrapped = true; }
+        }
+      }
+    } else if (warp == 11) {
+      // ===================== L2 prefetcher: keeps the HBM stream going while the ring is full =====================
+      // The weight producer blocks as soon as the ring is full (every dependency gap: grid barrier, glue phase,
+      // attention).  This warp walks the same item list and requests the tiles pf_lead .. pf_dist stages ahead of
+      // the producer into L2 (fire and forget), so HBM keeps streaming through the gaps and the ring refills from
+      // L2 afterwards.
+      if (a.pf_dist > 0) {
+        Walker w;
+        unsigned n_pf = 0;
+        for (w.start(sq); w.valid; w.next(sq)) {
+          const CUtensorMap* desc = &tm.w[w.o.which];
+          const int c1 = w.it.tile * kTileM, c2 = w.it.layer;
+          for (int kb = w.it.kb0; kb < w.it.kb1; ++kb, ++n_pf) {
+            unsigned pos = *reinterpret_cast<volatile unsigned*>(&s_wpos);
+            if (n_pf < pos + (unsigned)a.pf_lead) continue;          // the producer is (almost) there already
+            unsigned spins = 0;
+            while (n_pf >= pos + (unsigned)a.pf_dist) {
+              __nanosleep(64);
+              pos = *reinterpret_cast<volatile unsigned*>(&s_wpos);
+              if (++spins > 200000000u) __trap();
+            }
+            if (elect_one()) {
+              if (a.pf_mode & 2) tma_prefetch_3d_hint(desc, kb * kTileK, c1, c2, kEvictLast);
+              else if (a.pf_mode & 4) tma_prefetch_3d_hint(desc, kb * kTileK, c1, c2, kEvictFirst);
+              else tma_prefetch_3d(desc, kb * kTileK, c1, c2);
+            }
+            __syncwarp();
+          }
         }
       }
     } else if (warp == 6) {
@@ -1063,10 +1097,10 @@ __global__ void __launch_bounds__(kMaxThreads, 1) k_round(const __grid_constant_
         __syncwarp();
       }
     } else {
-      // ===================== glue group (12 warps): GEMM epilogues (warps 2-5) + glue + grid barriers =====================
+      // ===================== glue group (8 warps): GEMM epilogues (warps 2-5) + glue + grid barriers =====================
       const int we = warp < 6 ? warp - 2 : warp - 3;        // 0 .. glue warps - 1
       const int tid_e = we * 32 + lane;
-      constexpr int GT = kMaxThreads - 96, kGlueWarps = GT / 32;   // glue threads / warps
+      constexpr int GT = kMaxThreads - 128, kGlueWarps = GT / 32;   // glue threads / warps
       const int quarter = warp & 3;
       const int gw = blockIdx.x * kGlueWarps + we, n_gw = gridDim.x * kGlueWarps;
       EpiCtx ec;

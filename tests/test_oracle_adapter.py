@@ -64,3 +64,53 @@ def test_lossless_with_adapters_and_proposals_change(c1, c1_ar, c1_ad, X):
     plain = dex_decode(OracleModel(wl.shape, w), p, T, X, trace=True)
     differs = any(a["u"] != b["u"] for a, b in zip(od["rounds"], plain["rounds"]) if a["nodes"] == b["nodes"])
     assert differs or od["n_rounds"] != plain["n_rounds"]                                 # the adapters do act
+
+
+def test_delta_against_torch_module_built_from_the_paper(c1_ad):
+    """A pin that is not the oracle's own formula: the adapter as a torch.nn module assembled from the paper's
+    description - input RMSNorm, two biased linears h -> m -> h with the backbone activation between them, a scalar
+    gate on the whole branch - whose parameter count must be the paper's
+    P_ad = hm + mh + m + 2h + 1 = 4h^2 + 4h + 1 at m = 2h.  Evaluated by torch's own layers on the same tensors.
+    Fails if b2 sits outside the gate, if the activation is not SiLU, if the RMSNorm is dropped or if W1/W2 are
+    transposed (variants checked below)."""
+    torch = pytest.importorskip("torch")
+    nn = torch.nn
+    wl, w, p, ad, om = c1_ad
+    hdim, k = wl.shape.d_model, 1
+    m = ad["w1"].shape[1]
+
+    class Adapter(nn.Module):
+        def __init__(self):
+            super().__init__()
+            self.norm = nn.RMSNorm(hdim, eps=wl.shape.rms_eps)
+            self.w1 = nn.Linear(hdim, m, bias=True)
+            self.w2 = nn.Linear(m, hdim, bias=True)
+            self.alpha = nn.Parameter(torch.zeros(()))
+
+        def forward(self, h):
+            return self.alpha * self.w2(nn.functional.silu(self.w1(self.norm(h))))
+
+    mod = Adapter().double()
+    assert sum(q.numel() for q in mod.parameters()) == ead.adapter_params(hdim) == 4 * hdim * hdim + 4 * hdim + 1
+    with torch.no_grad():
+        mod.norm.weight.copy_(ad["norm"][k].double())
+        mod.w1.weight.copy_(ad["w1"][k].double()); mod.w1.bias.copy_(ad["b1"][k].double())
+        mod.w2.weight.copy_(ad["w2"][k].double()); mod.w2.bias.copy_(ad["b2"][k].double())
+        mod.alpha.copy_(ad["alpha"][k].double())
+    rng = np.random.default_rng(4)
+    for _ in range(3):
+        h = rng.standard_normal(hdim) * 3.0
+        with torch.no_grad():
+            ref = mod(torch.from_numpy(h)).numpy()
+        got = om.adapter_delta(h, k)
+        assert np.allclose(got, ref, rtol=1e-10, atol=1e-12)
+        # the plausible mistakes are far outside that tolerance on these tensors
+        with torch.no_grad():
+            t = torch.from_numpy(h)
+            z = mod.w1(mod.norm(t))
+            b2_outside = (mod.alpha * nn.functional.linear(nn.functional.silu(z), mod.w2.weight) + mod.w2.bias).numpy()
+            gelu = (mod.alpha * mod.w2(nn.functional.gelu(z))).numpy()
+            no_norm = (mod.alpha * mod.w2(nn.functional.silu(mod.w1(t)))).numpy()
+        for wrong in (b2_outside, gelu, no_norm):
+            assert np.abs(wrong - ref).max() > 1e-4 * np.abs(ref).max()
+            assert not np.allclose(got, wrong, rtol=1e-6, atol=1e-9)

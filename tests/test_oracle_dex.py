@@ -177,3 +177,35 @@ def test_teacher_forcing_hook_matches_selection(c1, c1_model, c1_ar):
     wl, _, p = c1
     r = dex_decode(c1_model, p, 12, (2, 4, 6, 8), force_tokens=c1_ar["tokens"][:12])
     assert np.array_equal(r["tokens"], c1_ar["tokens"][:12])
+
+
+def test_force_u_hook(c1, c1_model, runs):
+    """dex_decode(force_u=...) (teacher forcing of exit decisions for the GPU parity harness, reading R17b): forcing
+    the oracle's own candidates changes nothing and records nothing; forcing another token at one node records the
+    logit gap between the oracle's arg-max and the forced token and the lattice continues from the forced token."""
+    wl, _, p = c1
+    X = (2, 4, 6, 8)
+    base = runs[(X, True)]
+    T = 12
+    own = {(ri, i): t for ri, rec in enumerate(base["rounds"]) for i, t in rec["u"].items()}
+    same = dex_decode(c1_model, p, T, X, trace=True, force_u=own)
+    assert np.array_equal(same["tokens"], base["tokens"][:T])
+    assert all("u_forced" not in rec for rec in same["rounds"])
+    # force the second-best token at the final-depth anchor of the first commit round
+    ri = next(i for i, rec in enumerate(base["rounds"]) if rec["committed"])
+    rec = base["rounds"][ri]
+    ref_node = lt.anchor(len(X) - 1)
+    lg = rec["ref_logits"]
+    second = int(np.argsort(lg)[-2])
+    forced = dex_decode(c1_model, p, 3, X, trace=True, force_u={(ri, ref_node): second})
+    fr = forced["rounds"][ri]
+    a, t, gap = fr["u_forced"][ref_node]
+    assert a == rec["u"][ref_node] and t == second
+    assert np.isclose(gap, lg[a] - lg[second]) and gap > 0
+    assert forced["tokens"][0] == second and fr["token"] == second        # the forced candidate is what gets committed
+    # a masked token can never be produced by DECS: infinite gap
+    node = next(i for i in base["rounds"][1]["nodes"] if lt.slot_chain_prior(i))
+    prior_tok = base["rounds"][0]["u"][lt.slot_chain_prior(node)[0]]
+    bad = dex_decode(c1_model, p, 1, X, trace=True, force_u={(1, node): prior_tok})
+    if base["rounds"][1]["u"][node] != prior_tok:
+        assert bad["rounds"][1]["u_forced"][node][2] == np.inf

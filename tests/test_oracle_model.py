@@ -126,3 +126,36 @@ def test_prefill_matches_ar_state(c1, c1_model):
     wl, _, p = c1
     ck, cv = prefill(c1_model, p)
     assert len(ck) == wl.shape.n_layers and all(len(c) == len(p) - 1 for c in ck)
+
+
+@pytest.mark.parametrize("kv_round", [None, "bf16"])
+def test_prefill_matrix_equals_positionwise(c1, kv_round):
+    """oracle.ar.prefill_matrix (whole-sequence causal form, used for the long-context GPU parity cases) gives the
+    K/V of the position-at-a-time prefill: c1 (MHA) and a GQA shape with non-unit norm weights."""
+    from oracle.ar import prefill_matrix
+    wl, w, p = c1
+    shp = dex_synth.ModelShape("gqa-mini", 3, 64, 8, 2, 8, 96, 50, rope_theta=5e5)
+    cases = [(wl.shape, w, dex_synth.make_prompt(wl.shape.vocab, 70, 5)),
+             (shp, dex_synth.make_weights(shp, 7, norm_jitter=0.2), dex_synth.make_prompt(shp.vocab, 33, 3))]
+    for shape, ww, pp in cases:
+        m = OracleModel(shape, ww, kv_round=kv_round)
+        ck, cv = prefill(m, pp)
+        mk, mv = prefill_matrix(m, pp)
+        assert len(mk) == len(ck) == shape.n_layers
+        tol = 1e-11 if kv_round is None else 1e-2 * 2.0 ** -7     # bf16 cache: a last-place flip of a rounded value
+        n_flip = 0
+        for l in range(shape.n_layers):
+            assert len(mk[l]) == len(ck[l]) == len(pp) - 1
+            a, b = np.stack(ck[l]), np.stack(mk[l])
+            va, vb = np.stack(cv[l]), np.stack(mv[l])
+            assert np.abs(a - b).max() <= tol * max(1.0, np.abs(a).max())
+            assert np.abs(va - vb).max() <= tol * max(1.0, np.abs(va).max())
+            n_flip += int((a != b).sum() + (va != vb).sum())
+        if kv_round == "bf16":
+            assert n_flip <= 2                     # rounded values are bit-equal up to rare last-place ties
+        # and the decode that continues from either state is the same stream
+        t1 = ar_greedy(m, pp, 6, state=(ck, cv))["tokens"]
+        t2 = ar_greedy(m, pp, 6, state=(mk, mv))["tokens"]
+        assert np.array_equal(t1, t2)
+    ck0, cv0 = prefill_matrix(OracleModel(wl.shape, w), p[:1])   # one-token prompt: nothing to prefill
+    assert all(len(c) == 0 for c in ck0)
