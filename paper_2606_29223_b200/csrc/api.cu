@@ -4,7 +4,6 @@
 #include <algorithm>
 #include <cstdarg>
 #include <cstdio>
-#include <cstdlib>
 #include <cstring>
 #include <map>
 #include <memory>
@@ -27,6 +26,8 @@ cudaError_t launch_silu_mul(const Dev&, const Plan&, int, int, const OpDesc&, cu
 cudaError_t round_init();
 size_t round_attn_smem(int);
 cudaError_t launch_round(const TmSet&, const RoundArgs&, int, size_t, cudaStream_t);
+cudaError_t flow_init();
+cudaError_t launch_flow(const TmSet&, const RoundArgs&, int, size_t, cudaStream_t);
 cudaError_t launch_attn(const Dev&, const Plan&, int, int, int, int, cudaStream_t);
 cudaError_t launch_decide(const Dev&, const Plan&, int, cudaStream_t);
 cudaError_t launch_set_cmd(const Dev&, int, int, int, cudaStream_t);
@@ -83,8 +84,9 @@ struct dex_ctx {
   RingCfg round_ring;
   int round_attn_off;
   bool round_ok;                      // the round kernel's ring + attention scratch fit shared memory
-  int pf_mode;
-  int pf_dist, pf_lead;               // L2 prefetcher of the round kernel (ring stages ahead of the weight producer)
+  bool flow_ok;                       // the shape fits the dataflow round kernel's tables (else round_kernel = 2 runs k_round)
+  const int* flow_tab;                // device copy of the k_flow tables (QKV tile order, KV groups per tile)
+  size_t part_off[4];                 // k_flow: float offsets of the per-op split-K partial regions
   bool has_ad;                        // inducing-adapter exits (cfg.adapter_dim > 0, N >= 2): round kernel only
   std::map<long long, cudaGraphExec_t> graphs;
   std::string err;
@@ -117,6 +119,10 @@ int fail(dex_ctx* c, int code, const char* fmt, ...) {
   } while (0)
 
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+int cu_or_fail0(dex_ctx* c, cudaError_t e, const char* what) {
+  if (e != cudaSuccess) return fail(c, DEX_ECUDA, "%s: %s", what, cudaGetErrorString(e));
+  return DEX_OK;
+}
 int round16i(int v) { return (v + 15) & ~15; }
 
 int validate(const dex_config* cfg, const int32_t* depths, int32_t n) {
@@ -133,16 +139,16 @@ int validate(const dex_config* cfg, const int32_t* depths, int32_t n) {
   if (cfg->page_size < 64 || cfg->page_size % 64) return fail(nullptr, DEX_EINVAL, "page_size must be a multiple of 64");
   if (cfg->max_seqs < 1 || cfg->max_seqs > 8) return fail(nullptr, DEX_EINVAL, "max_seqs must be in [1,8]");
   if (cfg->max_ctx < 2) return fail(nullptr, DEX_EINVAL, "max_ctx too small");
-  if (cfg->round_kernel != 0 && cfg->round_kernel != 1) return fail(nullptr, DEX_EINVAL, "round_kernel must be 0 or 1");
+  if (cfg->round_kernel < 0 || cfg->round_kernel > 2) return fail(nullptr, DEX_EINVAL, "round_kernel must be 0, 1 or 2");
   if (cfg->sample != 0 && cfg->sample != 1) return fail(nullptr, DEX_EINVAL, "sample must be 0 or 1");
   if (cfg->sample && !(cfg->temperature > 0.f)) return fail(nullptr, DEX_EINVAL, "temperature must be > 0");
-  if (cfg->sample && !cfg->round_kernel) return fail(nullptr, DEX_EINVAL, "sampling mode needs round_kernel = 1");
+  if (cfg->sample && !cfg->round_kernel) return fail(nullptr, DEX_EINVAL, "sampling mode needs round_kernel >= 1");
   if (cfg->act_planes != 1 && cfg->act_planes != 2) return fail(nullptr, DEX_EINVAL, "act_planes must be 1 or 2");
   if (cfg->vocab < 2) return fail(nullptr, DEX_EINVAL, "vocab too small");
   if (cfg->lookahead < 0) return fail(nullptr, DEX_EINVAL, "lookahead must be >= 0");
   if (cfg->adapter_dim < 0 || cfg->adapter_dim % 64 || cfg->adapter_dim > cfg->d_ffn)
     return fail(nullptr, DEX_EINVAL, "adapter_dim must be a multiple of 64 in [0, d_ffn]");
-  if (cfg->adapter_dim && !cfg->round_kernel) return fail(nullptr, DEX_EINVAL, "inducing adapters need round_kernel = 1");
+  if (cfg->adapter_dim && !cfg->round_kernel) return fail(nullptr, DEX_EINVAL, "inducing adapters need round_kernel >= 1");
   if (cfg->adapter_dim && n < 2) return fail(nullptr, DEX_EINVAL, "inducing adapters need a non-final depth (N >= 2)");
   if (cfg->d_model > 8192) return fail(nullptr, DEX_ECAPACITY, "d_model > 8192 not supported");
   if (cfg->max_seqs * cap_of(n, 0) > 256) return fail(nullptr, DEX_ECAPACITY, "max_seqs * 2^(N-2) rows exceed 256 per stage");
@@ -178,13 +184,14 @@ struct Layout {
   Plan dec, pre, ext;
   OpCfg op[7];
   size_t part_floats;
+  size_t part_off[4];
   size_t off[40];
   size_t total;
   size_t dbg_floats;
 };
 enum Buf {
   B_SEQS, B_TOKENS, B_B, B_PT, B_ROWS, B_GNB, B_ENB, B_KEY, B_REFT, B_CMD, B_SS, B_ACNT, B_KPOOL, B_VPOOL, B_KSLOT, B_VSLOT,
-  B_XCUR, B_XFRONT, B_ACTA, B_ACTO, B_ACTF, B_ACTE, B_PART, B_QBUF, B_APART, B_ROPE, B_TAPH, B_DBG, B_GBAR, B_TAPT, B_COUNT
+  B_XCUR, B_XFRONT, B_ACTA, B_ACTO, B_ACTF, B_ACTE, B_PART, B_QBUF, B_APART, B_ROPE, B_TAPH, B_DBG, B_GBAR, B_TAPT, B_FCTR, B_FTAB, B_COUNT
 };
 
 void make_layout(const dex_config& c, const int32_t* depths, int n, Layout& L) {
@@ -243,6 +250,14 @@ void make_layout(const dex_config& c, const int32_t* depths, int n, Layout& L) {
       L.part_floats = std::max(L.part_floats, (size_t)L.op[5 + i].dec.ksplit * L.op[5 + i].dec.split_stride);
     }
   }
+  {   // k_flow keeps the partials of the four layer ops in regions of their own (ops of a layer-step overlap there)
+    size_t off = 0;
+    for (int i = 0; i < 4; ++i) {
+      L.part_off[i] = off;
+      off += align_up((size_t)L.op[i].dec.ksplit * L.op[i].dec.split_stride, 256);
+    }
+    L.part_floats = std::max(L.part_floats, off);
+  }
   L.max_chunks = (c.max_ctx + n) / kChunk + 1;
   L.pages_per_seq = (c.max_ctx + c.page_size - 1) / c.page_size;
   L.n_pages = L.pages_per_seq * c.max_seqs;
@@ -283,6 +298,8 @@ void make_layout(const dex_config& c, const int32_t* depths, int n, Layout& L) {
   sz[B_DBG] = sizeof(float) * L.dbg_floats;
   sz[B_GBAR] = 256;
   sz[B_TAPT] = c.debug_taps ? sizeof(unsigned long long) * (20 * (size_t)L.max_len + 68) : 0;
+  sz[B_FCTR] = sizeof(int) * kFcTotal;
+  sz[B_FTAB] = sizeof(int) * kFtTotal;
   size_t off = 0;
   for (int i = 0; i < B_COUNT; ++i) {
     L.off[i] = off;
@@ -430,11 +447,11 @@ int enqueue_round(dex_ctx* c, int n_chunks) {
   a.stacked = c->round_ring.stacked;
   a.n_chunks = n_chunks;
   a.attn_smem_off = c->round_attn_off;
-  a.pf_dist = c->pf_dist;
-  a.pf_lead = c->pf_lead;
-  a.pf_mode = c->pf_mode;
+  a.flow_tab = c->flow_tab;
+  for (int i = 0; i < 4; ++i) a.part_off[i] = c->part_off[i];
   ph_begin(c, PH_GEMM);
-  CU(c, launch_round(c->tms, a, c->n_sms, c->round_ring.smem, c->stream));
+  if (c->cfg.round_kernel == 2 && c->flow_ok) CU(c, launch_flow(c->tms, a, c->n_sms, c->round_ring.smem, c->stream));
+  else CU(c, launch_round(c->tms, a, c->n_sms, c->round_ring.smem, c->stream));
   ph_end(c, PH_GEMM);
   return DEX_OK;
 }
@@ -614,14 +631,6 @@ int32_t dex_init(dex_ctx** out, const dex_config* cfg, const dex_weights* w, con
   D.max_len = L.max_len; D.max_chunks = L.max_chunks; D.ref_tiles = L.ref_tiles;
   D.lookahead = (cfg->lookahead >= n_depths - 1) ? 0 : cfg->lookahead;   // P >= N-1 is the full lattice
   c->has_ad = cfg->adapter_dim > 0;
-  {   // tuning knobs of the round kernel's L2 prefetcher; the defaults are the measured optimum
-    const char* e1 = getenv("DEX_PF_DIST");
-    const char* e2 = getenv("DEX_PF_LEAD");
-    c->pf_dist = e1 ? atoi(e1) : 0;
-    c->pf_lead = e2 ? atoi(e2) : 2;
-    const char* e3 = getenv("DEX_PF_MODE");
-    c->pf_mode = e3 ? atoi(e3) : 0;
-  }
   D.ad_m = cfg->adapter_dim;
   if (c->has_ad) { D.ad_b1 = w->ad_b1; D.ad_b2 = w->ad_b2; D.ad_norm = w->ad_norm; D.ad_alpha = w->ad_alpha; }
   D.embed = static_cast<const __nv_bfloat16*>(w->embed);
@@ -641,6 +650,9 @@ int32_t dex_init(dex_ctx** out, const dex_config* cfg, const dex_weights* w, con
   D.part = WSP(float, B_PART); D.qbuf = WSP(float, B_QBUF); D.attn_part = WSP(float, B_APART);
   D.rope = WSP(float2, B_ROPE); D.tap_hidden = cfg->debug_taps ? WSP(float, B_TAPH) : nullptr;
   D.gbar = WSP(unsigned int, B_GBAR);
+  D.flow_ctr = WSP(int, B_FCTR);
+  c->flow_tab = WSP(int, B_FTAB);
+  for (int i = 0; i < 4; ++i) c->part_off[i] = L.part_off[i];
   D.tap_times = cfg->debug_taps ? WSP(unsigned long long, B_TAPT) : nullptr;
   c->dbg_stage = cfg->debug_taps ? WSP(float, B_DBG) : nullptr;
   c->dbg_floats = L.dbg_floats;
@@ -690,6 +702,10 @@ int32_t dex_init(dex_ctx** out, const dex_config* cfg, const dex_weights* w, con
     delete c;
     return fail(nullptr, DEX_ECUDA, "cannot raise the round kernel's dynamic shared memory limit");
   }
+  if (flow_init() != cudaSuccess) {
+    delete c;
+    return fail(nullptr, DEX_ECUDA, "cannot raise the dataflow round kernel's dynamic shared memory limit");
+  }
   if (gemm_init() != cudaSuccess) {
     delete c;
     return fail(nullptr, DEX_ECUDA, "cannot raise the GEMM kernel's dynamic shared memory limit");
@@ -709,6 +725,31 @@ int32_t dex_init(dex_ctx** out, const dex_config* cfg, const dex_weights* w, con
     const void* aptr[2] = {w->ad_w1, w->ad_w2};
     for (int i = 0; i < 2; ++i)
       INIT_FAIL(encode_3d(c, enc, &c->op[5 + i].tmW, aptr[i], c->op[5 + i].dec.k_dim, c->op[5 + i].dec.out_dim, n_depths - 1, kTileM));
+  }
+  // k_flow: gate/up as [2L][ffn][d] (gate tile b and up tile b of a layer are both 128-row boxes, whatever ffn % 128 is)
+  INIT_FAIL(encode_3d(c, enc, &c->tms.wgu2, w->wgu, D.d, D.ffn, 2 * (uint64_t)D.L, kTileM));
+  {
+    // QKV tile order by KV head group (q tiles of the group, then its k and v tile) and the groups a tile touches
+    const int hd = D.hd, Gq = D.nh / D.nkv, n_t = c->op[0].dec.n_tiles;
+    c->flow_ok = (D.nh * hd) % kTileM == 0 && (D.nkv * hd) % kTileM == 0 && n_t <= kFlowTiles &&
+                 2 * ((D.ffn + kTileM - 1) / kTileM) <= kFlowTiles && (D.d + kTileM - 1) / kTileM <= kFlowTiles && D.nkv <= kFlowSlices;
+    for (int i = 0; i < 4; ++i) c->flow_ok = c->flow_ok && c->op[i].dec.ksplit <= kFlowSlices;
+    std::vector<int> tab(kFtTotal, 0);
+    if (c->flow_ok) {
+      auto grp_of = [&](int hh) { return hh < D.nh ? hh / Gq : (hh < D.nh + D.nkv ? hh - D.nh : hh - D.nh - D.nkv); };
+      for (int t = 0; t < n_t; ++t) {
+        const int h_lo = t * kTileM / hd, h_hi = std::min((t * kTileM + kTileM - 1) / hd, D.nh + 2 * D.nkv - 1);
+        int lo = 1 << 30, hi = -1;
+        for (int hh = h_lo; hh <= h_hi; ++hh) { lo = std::min(lo, grp_of(hh)); hi = std::max(hi, grp_of(hh)); }
+        tab[kFtGlo + t] = lo; tab[kFtGhi + t] = hi;
+        for (int g = lo; g <= hi; ++g) tab[kFtTarget + g] += 1;
+      }
+      int n = 0;
+      for (int g = 0; g < D.nkv; ++g)
+        for (int t = 0; t < n_t; ++t)
+          if (tab[kFtGlo + t] == g) tab[kFtPerm + n++] = t;
+    }
+    INIT_FAIL(cu_or_fail0(c, cudaMemcpy(const_cast<int*>(c->flow_tab), tab.data(), sizeof(int) * kFtTotal, cudaMemcpyHostToDevice), "flow tables"));
   }
   for (int i = 0; i < (c->has_ad ? 7 : 5); ++i) c->tms.w[i] = c->op[i].tmW;
   for (int i = 0; i < 4; ++i) c->tms.x[i] = c->tmX[i];

@@ -111,6 +111,7 @@ struct Dev {
   __nv_bfloat16 *act_a, *act_o, *act_f, *act_e;   // [planes][R_cap][K] MMA operands
   float* part;             // split-K partial sums, per op [S_op][R_cap][ld_op] (OpDesc)
   unsigned int* gbar;      // grid-barrier arrival counter of the round kernel (reset every round)
+  int* flow_ctr;           // [kFcTotal] arrival counters / ready flags of the dataflow round kernel (k_flow), zeroed every round
   float* qbuf;             // [R_cap][nh*hd]
   float* attn_part;        // [R_cap][nh][4 * max_chunks][hd + 2]: (o, max, sum) per 16 positions (k_round) / per chunk (k_attn)
   int max_chunks;
@@ -240,7 +241,21 @@ struct OpDesc {
 struct TmSet {             // TMA descriptors of the round kernel: weights qkv,o,gu,dn,lm_head,ad_w1,ad_w2; operands a,o,f,e
   CUtensorMap w[7];
   CUtensorMap x[4];
+  CUtensorMap wgu2;        // k_flow: gate/up viewed as [2L][ffn][d], so gate tile b and up tile b are both 128-row boxes
 };
+
+// k_flow (flow.cu): counters in Dev::flow_ctr.  All are monotonic within a round (targets scale with the layer-step).
+constexpr int kFlowTiles = 256;                       // max 128-row tiles of one projection (per stage)
+constexpr int kFlowSlices = 64;                       // max K slices (one item's K range) / KV heads
+constexpr int kFcTile = 0;                            // [4 ops][8 stages][kFlowTiles] split arrivals of an out tile
+constexpr int kFcXa = 4 * kMaxGrp * kFlowTiles;       // [8][64] down-proj tiles finalized per K slice of act_a (QKV operand)
+constexpr int kFcAo = kFcXa + kMaxGrp * kFlowSlices;  // [8][64] (row, head) attention outputs merged per K slice of act_o
+constexpr int kFcXf = kFcAo + kMaxGrp * kFlowSlices;  // [8][64] o-proj tiles finalized per K slice of act_a (gate/up operand)
+constexpr int kFcF = kFcXf + kMaxGrp * kFlowSlices;   // [8][64] gate/up pairs finalized per K slice of act_f (down operand)
+constexpr int kFcQkv = kFcF + kMaxGrp * kFlowSlices;  // [8][64] QKV tiles finalized per KV head group
+constexpr int kFcTotal = kFcQkv + kMaxGrp * kFlowSlices;
+// Dev-independent tables of k_flow (host-built, RoundArgs::flow_tab): QKV tile order + the KV groups a tile touches
+constexpr int kFtPerm = 0, kFtGlo = kFlowTiles, kFtGhi = 2 * kFlowTiles, kFtTarget = 3 * kFlowTiles, kFtTotal = 3 * kFlowTiles + kFlowSlices;
 
 struct RoundArgs {
   Dev D;
@@ -249,8 +264,8 @@ struct RoundArgs {
   int x_cap, n_stages, acc_cols, stacked;   // shared-memory ring / TMEM geometry
   int n_chunks;                    // attention chunks that can hold a live position (host upper bound)
   int attn_smem_off;               // byte offset of the attention scratch (AttnSmem) in dynamic shared memory
-  int pf_mode;
-  int pf_dist, pf_lead;            // L2 prefetcher: ring stages it may run ahead of the weight producer (0: off) / minimum lead
+  const int* flow_tab;             // k_flow: [kFtTotal] QKV tile order, KV groups touched by a tile, tiles per group
+  size_t part_off[4];              // k_flow: float offset of each layer op's own split-K partial region in Dev::part
 };
 
 }  // namespace dexk

@@ -1,0 +1,615 @@
+// flow.cu — k_flow: the persistent round kernel as a DATAFLOW program (Alg. 1 lines 5-6).
+//
+// Same work as k_round (round.cu): for every layer-step all live stages run QKV -> attention -> O -> gate/up -> down,
+// then the fused exit.  k_round separates the nine activities of a layer-step by grid barriers; every barrier and
+// glue phase leaves HBM idle once the shared-memory ring is full (2.5 us of stream).  Here the layer-steps have NO
+// grid barrier: every dependency is a counter in global memory.
+//
+//   * split-K partials are reduced by the LAST ARRIVER: the CTA whose item completes an out tile (all K splits
+//     written, counted with one acq_rel atomic per item) sums the partials in split order (H3: the bits do not depend
+//     on who arrives last) and finalizes the tile on its finalizer warps - QKV: deferred-norm scale + RoPE + slot K/V;
+//     O / down: residual add + next operand planes + sum of squares of the 128-column segment; gate/up: SwiGLU (gate
+//     tile b and up tile b are counted together; the weights stay in their [2][ffn][d] layout, the tensor map views
+//     them as [2L][ffn][d]);
+//   * a finished tile bumps the READY counter of the consumer's K slice (an item's K range: 8 K-blocks = 512
+//     columns); the activation producer of a consuming item polls exactly the slice it needs (ld.acquire.gpu), so
+//     consumers start while the producing op is still streaming.  Item orders are chosen for that: QKV by KV head
+//     (q, k, v tiles of a head adjacent) -> attention of the first heads overlaps the rest of the QKV stream; O and
+//     down split-major (early splits need early heads / early gate-up pairs); gate/up pair-major;
+//   * attention tasks wait for the QKV counter of their KV head group, the last merger of a (row, head) bumps the
+//     ready counter of the O operand slice;
+//   * with several live stages (DEX rounds) the ops are stage-major, so the O -> gate/up and down -> QKV dependencies
+//     of one stage are covered by the other stages' streams: depth-parallel stages hide each other's latency.
+// Only the tail of the round (inducing adapters, exit head) keeps grid barriers.
+//
+//   warp 0      weight producer (TMA, always ahead)         warp 6      activation producer (waits on slice counters)
+//   warp 1      tcgen05.mma issuer, owns TMEM               warps 7-10  finalizer group: counts own items, finalizes
+//   warps 2-5   epilogue: TMEM -> split-K partials / arg-max            completed tiles, runs attention tasks
+#include "round_dev.cuh"
+
+namespace dexk {
+
+constexpr int kFlowThreads = 352;
+constexpr int kFT = 128;             // finalizer group threads (warps 7-10)
+
+// ---------------------------------------------------------------- small helpers
+__device__ __forceinline__ int ld_acquire_s32(const int* p) {
+  int v;
+  asm volatile("ld.acquire.gpu.global.s32 %0, [%1];\n" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ void red_release_add_s32(int* p, int v) {
+  asm volatile("red.release.gpu.global.add.s32 [%0], %1;\n" ::"l"(p), "r"(v) : "memory");
+}
+__device__ __forceinline__ int atom_acq_rel_add_s32(int* p, int v) {
+  int old;
+  asm volatile("atom.acq_rel.gpu.global.add.s32 %0, [%1], %2;\n" : "=r"(old) : "l"(p), "r"(v) : "memory");
+  return old;
+}
+__device__ __forceinline__ unsigned ld_acquire_cta_shared(const unsigned* p) {
+  unsigned v;
+  asm volatile("ld.acquire.cta.shared.u32 %0, [%1];\n" : "=r"(v) : "r"(smem_u32(p)) : "memory");
+  return v;
+}
+__device__ __forceinline__ void red_release_cta_shared_add(unsigned* p, unsigned v) {
+  asm volatile("red.release.cta.shared.add.u32 [%0], %1;\n" ::"r"(smem_u32(p)), "r"(v) : "memory");
+}
+__device__ __forceinline__ int tiles_in_slice(int dim, int slice_cols, int s) {   // 128-column tiles overlapping K slice s
+  const int c0 = s * slice_cols, c1 = min(c0 + slice_cols, dim);
+  return (c1 + 127) / 128 - c0 / 128;
+}
+
+// ---------------------------------------------------------------- the round's op / item sequence
+struct FOp {
+  int which, j, ext;
+  unsigned mask;
+  int n_tiles, ksplit, kbps, kb_total, per_grp, n_items;
+};
+struct FItem {
+  int g, nb, tile, split, kb0, kb1, row0, row_end;
+  int c1, c2;              // TMA coordinates: weight row, "layer"
+  int col0, col_end;       // partial column of TMEM lane 0; columns >= col_end are not stored
+  int cnt_idx, cnt_target; // finalization counter of the tile (gate/up: of the pair) and its arrivals per layer-step
+};
+
+struct FSeq {
+  const RoundArgs* a;
+  const int* s_nb;         // [16]
+  const short* s_perm;     // QKV tile order
+  int n_steps, n_ops, n_ad_ops, G, cta, gu_half;   // gu_half = ceil(ffn / 128)
+
+  __device__ __forceinline__ int which_of(int t) const {
+    return t < 4 * n_steps ? (t & 3) : (t < 4 * n_steps + n_ad_ops ? 5 + t - 4 * n_steps : 4);
+  }
+  __device__ __forceinline__ void op_info(int t, FOp& o) const {
+    unsigned mask = 0;
+    if (t < 4 * n_steps) {
+      o.j = t >> 2; o.which = t & 3; o.ext = 0;
+      for (int g = 0; g < a->dec.n_grp; ++g)
+        if (s_nb[g] > 0 && o.j < a->dec.layer_len[g]) mask |= 1u << g;
+    } else if (t < 4 * n_steps + n_ad_ops) {
+      o.j = 0; o.which = 5 + t - 4 * n_steps; o.ext = 0;
+      for (int g = 0; g + 1 < a->dec.n_grp; ++g)
+        if (s_nb[g] > 0) mask |= 1u << g;
+    } else {
+      o.j = 0; o.which = 4; o.ext = 1;
+      for (int g = 0; g < a->ext.n_grp; ++g)
+        if (s_nb[8 + g] > 0) mask |= 1u << g;
+    }
+    o.mask = mask;
+    const OpDesc& d = a->op[o.which];
+    o.n_tiles = (t < 4 * n_steps && o.which == 2) ? 2 * gu_half : d.n_tiles;
+    o.ksplit = d.ksplit; o.kbps = d.kbps; o.kb_total = d.kb_total;
+    o.per_grp = o.n_tiles * d.ksplit;
+    o.n_items = __popc(mask) * o.per_grp;
+  }
+  __device__ __forceinline__ void decode(const FOp& o, int i, FItem& it) const {
+    const int gi = i / o.per_grp, rem = i - gi * o.per_grp;
+    it.g = __fns(o.mask, 0, gi + 1);
+    const Plan& p = o.ext ? a->ext : a->dec;
+    it.nb = s_nb[(o.ext ? 8 : 0) + it.g];
+    it.row0 = p.row_base[it.g];
+    it.row_end = it.row0 + p.rows_cap[it.g];
+    const OpDesc& d = a->op[o.which];
+    if (!o.ext && o.which < 4) {
+      const int layer = p.layer_lo[it.g] + o.j;
+      if (o.which == 0) {                                  // by KV head group, splits fastest
+        const int ti = rem / o.ksplit;
+        it.split = rem - ti * o.ksplit;
+        it.tile = s_perm[ti];
+        it.c1 = it.tile * kTileM; it.c2 = layer;
+        it.col0 = it.tile * kTileM; it.col_end = d.out_dim;
+        it.cnt_idx = it.tile; it.cnt_target = o.ksplit;
+      } else if (o.which == 2) {                           // pair-major: gate tile b, up tile b, splits fastest
+        const int ti = rem / o.ksplit;
+        it.split = rem - ti * o.ksplit;
+        const int half = ti & 1, b = ti >> 1;
+        it.tile = ti;
+        it.c1 = b * kTileM; it.c2 = 2 * layer + half;
+        it.col0 = half * a->D.ffn + b * kTileM; it.col_end = half * a->D.ffn + a->D.ffn;
+        it.cnt_idx = b; it.cnt_target = 2 * o.ksplit;
+      } else {                                             // O, down: split-major
+        it.split = rem / o.n_tiles;
+        it.tile = rem - it.split * o.n_tiles;
+        it.c1 = it.tile * kTileM; it.c2 = layer;
+        it.col0 = it.tile * kTileM; it.col_end = d.out_dim;
+        it.cnt_idx = it.tile; it.cnt_target = o.ksplit;
+      }
+    } else {
+      it.tile = rem / o.ksplit;
+      it.split = rem - it.tile * o.ksplit;
+      it.c1 = it.tile * kTileM; it.c2 = o.ext ? 0 : it.g;  // adapter k serves stage k
+      it.col0 = it.tile * kTileM; it.col_end = d.out_dim;
+      it.cnt_idx = it.tile; it.cnt_target = o.ksplit;
+    }
+    it.kb0 = it.split * o.kbps;
+    it.kb1 = min(it.kb0 + o.kbps, o.kb_total);
+  }
+};
+
+struct FWalker {           // this CTA's items, in order (dealt round-robin, continuing across ops)
+  int t, i, rr;
+  bool valid;
+  FOp o;
+  FItem it;
+  __device__ __forceinline__ void start(const FSeq& q) {
+    t = 0; rr = 0;
+    q.op_info(0, o);
+    i = q.cta;
+    settle(q);
+  }
+  __device__ __forceinline__ void settle(const FSeq& q) {
+    while (t < q.n_ops && i >= o.n_items) {
+      rr = (rr + o.n_items) % q.G;
+      ++t;
+      if (t < q.n_ops) {
+        q.op_info(t, o);
+        i = (q.cta + q.G - rr) % q.G;
+      }
+    }
+    valid = t < q.n_ops;
+    if (valid) q.decode(o, i, it);
+  }
+  __device__ __forceinline__ void next(const FSeq& q) {
+    i += q.G;
+    settle(q);
+  }
+};
+
+template <int GT>
+__device__ __forceinline__ void bar_f() { asm volatile("bar.sync 1, %0;\n" ::"n"(GT) : "memory"); }
+
+// Decision record handed from finalizer warp 0 to the group (double-buffered by loop iteration).
+struct FDec {
+  int kind;                // 0 idle, 1 finalize a tile, 2 attention task, 3 layer-steps done, 4 counted (nothing to do)
+  int which, m, idx, j, row0, row_hi;
+  AttnTask tk;
+};
+
+// ---------------------------------------------------------------- the kernel
+template <bool PT>
+__global__ void __launch_bounds__(kFlowThreads, 1) k_flow(const __grid_constant__ TmSet tm, const __grid_constant__ RoundArgs a) {
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  const Dev& D = a.D;
+  const uint32_t plane_bytes = a.x_cap * 128;
+  const uint32_t stage_bytes = kABytes + D.planes * plane_bytes;
+  const int NS = a.n_stages;
+  uint64_t* bars = reinterpret_cast<uint64_t*>(smem + (size_t)NS * stage_bytes);
+  uint64_t* full = bars;
+  uint64_t* empty = bars + NS;
+  uint64_t* tfull = bars + 2 * NS;
+  uint64_t* tempty = tfull + 2;
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(tempty + 2);
+
+  __shared__ int s_nb[16];
+  __shared__ uint32_t s_valid[32];
+  __shared__ int s_nvalid[kMaxGrp];
+  __shared__ int s_live_ms;
+  __shared__ int s_cum[kMaxGrp + 1];
+  __shared__ int s_steps;
+  __shared__ unsigned s_seen;            // grid barriers completed (tail of the round)
+  __shared__ unsigned s_edone[4];        // items completed by each epilogue warp (an item is written when all four have)
+  __shared__ short s_perm[kFlowTiles];
+  __shared__ unsigned char s_glo[kFlowTiles], s_ghi[kFlowTiles];
+  __shared__ int s_qtarget[kFlowSlices];
+  __shared__ int s_ao_cnt[kFlowSlices];
+  __shared__ FDec s_dec[2];
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  if (threadIdx.x < 32) s_valid[threadIdx.x] = 0;
+  if (threadIdx.x < kMaxGrp) s_nvalid[threadIdx.x] = 0;
+  __syncthreads();
+  for (int r = threadIdx.x; r < D.R_cap; r += blockDim.x)
+    if (D.rows[r].valid) {
+      atomicOr(&s_valid[r >> 5], 1u << (r & 31));
+      if (r < D.R_dec) atomicAdd(&s_nvalid[D.rows[r].grp], 1);
+    }
+  for (int i = threadIdx.x; i < kFlowTiles; i += blockDim.x) {
+    s_perm[i] = (short)a.flow_tab[kFtPerm + i];
+    s_glo[i] = (unsigned char)a.flow_tab[kFtGlo + i];
+    s_ghi[i] = (unsigned char)a.flow_tab[kFtGhi + i];
+  }
+  for (int i = threadIdx.x; i < kFlowSlices; i += blockDim.x) s_qtarget[i] = a.flow_tab[kFtTarget + i];
+  if (threadIdx.x == 0) {
+    int steps = 0;
+    for (int g = 0; g < 8; ++g) {
+      const int nb = (g < a.dec.n_grp) ? D.grp_nb[g] : 0;
+      s_nb[g] = nb;
+      if (nb > 0) steps = max(steps, a.dec.layer_len[g]);
+      s_nb[8 + g] = (g < a.ext.n_grp) ? D.exit_nb[g] : 0;
+    }
+    s_steps = steps;
+    s_seen = 0;
+    s_edone[0] = s_edone[1] = s_edone[2] = s_edone[3] = 0;
+    int lm = 0;
+    for (int s = 0; s < D.max_seqs; ++s) {                   // live (stage, sequence[, 16-pair pass]) attention families
+      const SeqState st = D.seqs[s];
+      if (!r_seq_live(st)) continue;
+      if constexpr (PT) {
+        for (int m = 0; m <= min(st.q, D.N - 1); ++m) lm += (r_stage_count(st.q, m) * (D.nh / D.nkv) + 15) / 16;
+      } else {
+        lm += min(st.q, D.N - 1) + 1;
+      }
+    }
+    s_live_ms = lm;
+    s_cum[0] = 0;
+    for (int m = 0; m < kMaxGrp; ++m)
+      s_cum[m + 1] = s_cum[m] + ((PT && m < D.N) ? D.max_seqs * ((cap_of(D.N, m) * (D.nh / D.nkv) + 15) / 16) : 0);
+    for (int i = 0; i < NS; ++i) {
+      mbar_init(&full[i], 1);
+      mbar_init(&empty[i], 1);
+    }
+    for (int i = 0; i < 2; ++i) {
+      mbar_init(&tfull[i], 1);
+      mbar_init(&tempty[i], 4);
+    }
+    fence_mbar_init();
+    for (int i = 0; i < (D.ad_m > 0 ? 7 : 5); ++i) tma_prefetch_desc(&tm.w[i]);
+    for (int i = 0; i < 4; ++i) tma_prefetch_desc(&tm.x[i]);
+    tma_prefetch_desc(&tm.wgu2);
+  }
+  if (warp == 1) {
+    tmem_alloc(tmem_slot, 2 * a.acc_cols);
+    tmem_relinquish();
+  }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = *tmem_slot;
+
+  FSeq sq;
+  sq.a = &a; sq.s_nb = s_nb; sq.s_perm = s_perm; sq.n_steps = s_steps; sq.n_ad_ops = (D.ad_m > 0 && D.N >= 2) ? 2 : 0;
+  sq.n_ops = 4 * s_steps + sq.n_ad_ops + 1; sq.G = gridDim.x; sq.cta = blockIdx.x; sq.gu_half = (D.ffn + 127) / 128;
+  const unsigned G = gridDim.x;
+  int* const ctr = D.flow_ctr;
+  const int n_layer_ops = 4 * s_steps;
+
+  if (s_steps > 0) {
+    if (warp == 0) {
+      // ===================== weight producer: always as far ahead as the ring allows =====================
+      FWalker w;
+      unsigned st = 0, ph = 0;
+      bool wrapped = false;
+      for (w.start(sq); w.valid; w.next(sq)) {
+        const CUtensorMap* desc = (w.t < n_layer_ops && w.o.which == 2) ? &tm.wgu2 : &tm.w[w.o.which];
+        const uint32_t tx = kABytes + D.planes * w.it.nb * 128;
+        for (int kb = w.it.kb0; kb < w.it.kb1; ++kb) {
+          if (wrapped) mbar_wait(&empty[st], ph ^ 1u);
+          if (elect_one()) {
+            mbar_expect_tx(&full[st], tx);
+            tma_load_3d(smem + (size_t)st * stage_bytes, desc, &full[st], kb * kTileK, w.it.c1, w.it.c2, kEvictFirst);
+          }
+          __syncwarp();
+          if (++st == (unsigned)NS) { st = 0; ph ^= 1u; wrapped = true; }
+        }
+      }
+    } else if (warp == 6) {
+      // ===================== activation producer: waits for the K slice of its item =====================
+      FWalker w;
+      unsigned st = 0, ph = 0;
+      bool wrapped = false;
+      unsigned seen = 0;
+      const int sl_x = a.op[0].kbps * kTileK, sl_o = a.op[1].kbps * kTileK, sl_f = a.op[3].kbps * kTileK;
+      for (w.start(sq); w.valid; w.next(sq)) {
+        const int which = w.o.which;
+        if (w.t < n_layer_ops) {
+          const int m = w.it.g, s = w.it.split, j = w.o.j;
+          const int* flag;
+          int target;
+          if (which == 0) {
+            flag = ctr + kFcXa + m * kFlowSlices + s;
+            target = j * tiles_in_slice(D.d, sl_x, s);
+          } else if (which == 1) {
+            flag = ctr + kFcAo + m * kFlowSlices + s;
+            const int hs = (min((s + 1) * sl_o, D.nh * D.hd) - s * sl_o) / D.hd;
+            target = (j + 1) * s_nvalid[m] * hs;
+          } else if (which == 2) {
+            flag = ctr + kFcXf + m * kFlowSlices + s;
+            target = (j + 1) * tiles_in_slice(D.d, sl_x, s);
+          } else {
+            flag = ctr + kFcF + m * kFlowSlices + s;
+            target = (j + 1) * tiles_in_slice(D.ffn, sl_f, s);
+          }
+          if (target > 0) {
+            unsigned spins = 0;
+            while (ld_acquire_s32(flag) < target) {
+              __nanosleep(40);
+              if (++spins > 50000000u) __trap();
+            }
+            fence_proxy_async();
+          }
+        } else {
+          // tail ops (adapters, exit head): published by grid barriers, as in k_round
+          const int k = w.t - n_layer_ops;
+          const unsigned need = sq.n_ad_ops ? (k == 0 ? 1u : (k == 1 ? 3u : 5u)) : 1u;
+          if (seen < need) {
+            unsigned spins = 0;
+            while ((seen = *reinterpret_cast<volatile unsigned*>(&s_seen)) < need) {
+              __nanosleep(32);
+              if (++spins > 100000000u) __trap();
+            }
+            __threadfence_block();
+            fence_proxy_async();
+          }
+        }
+        const CUtensorMap* desc = &tm.x[(which == 0 || which == 2 || which == 5) ? 0 : (which == 1 ? 1 : (which == 4 ? 3 : 2))];
+        const int row0 = w.it.row0, nb = w.it.nb;
+        for (int kb = w.it.kb0; kb < w.it.kb1; ++kb) {
+          if (wrapped) mbar_wait(&empty[st], ph ^ 1u);
+          if (elect_one()) {
+            uint8_t* sB = smem + (size_t)st * stage_bytes + kABytes;
+            if (a.stacked) {
+              for (int r = 0; r < nb; r += kBoxRows)
+                tma_load_3d(sB + r * 256, desc, &full[st], kb * kTileK, row0 + r, 0, kEvictLast);
+            } else {
+              for (int p = 0; p < D.planes; ++p)
+                for (int r = 0; r < nb; r += kBoxRows)
+                  tma_load_3d(sB + p * plane_bytes + r * 128, desc, &full[st], kb * kTileK, row0 + r, p, kEvictLast);
+            }
+          }
+          __syncwarp();
+          if (++st == (unsigned)NS) { st = 0; ph ^= 1u; wrapped = true; }
+        }
+      }
+    } else if (warp == 1) {
+      // ===================== MMA issuer =====================
+      FWalker w;
+      unsigned st = 0, ph = 0;
+      int n_it = 0;
+      const bool stacked = a.stacked != 0;
+      for (w.start(sq); w.valid; w.next(sq), ++n_it) {
+        const int as = n_it & 1;
+        mbar_wait(&tempty[as], ((n_it >> 1) & 1) ^ 1);
+        tc_fence_after();
+        const uint32_t d_tmem = tmem_base + as * a.acc_cols;
+        const uint32_t idesc = make_idesc_bf16_m128(stacked ? 2 * w.it.nb : w.it.nb);
+        uint32_t acc = 0;
+        for (int kb = w.it.kb0; kb < w.it.kb1; ++kb) {
+          mbar_wait(&full[st], ph);
+          tc_fence_after();
+          if (elect_one()) {
+            mma_stage(smem_u32(smem + (size_t)st * stage_bytes), plane_bytes, D.planes, stacked, d_tmem, idesc, acc);
+            umma_commit(&empty[st]);
+          }
+          __syncwarp();
+          acc = 1;
+          if (++st == (unsigned)NS) { st = 0; ph ^= 1u; }
+        }
+        if (elect_one()) umma_commit(&tfull[as]);
+        __syncwarp();
+      }
+    } else if (warp >= 2 && warp <= 5) {
+      // ===================== epilogue: TMEM -> partials of the op's own region / exit arg-max =====================
+      const int quarter = warp & 3;
+      EpiCtx ec;
+      ec.rows = D.rows; ec.s_valid = s_valid; ec.vocab = D.vocab; ec.best_key = D.best_key;
+      ec.ref_tile = D.ref_tile; ec.ref_tiles = D.ref_tiles; ec.dev = &D;
+      FWalker w;
+      int n_it = 0;
+      for (w.start(sq); w.valid; w.next(sq), ++n_it) {
+        const int which = w.o.which;
+        const OpDesc& od = a.op[which];
+        ec.mode = which == 4 ? 1 : 0;
+        ec.part = D.part + (w.t < n_layer_ops ? a.part_off[which] : 0);
+        ec.part_ld = od.part_ld; ec.split_stride = od.split_stride; ec.out_dim = w.it.col_end;
+        const int as = n_it & 1;
+        mbar_wait(&tfull[as], (n_it >> 1) & 1);
+        tc_fence_after();
+        const uint32_t t_addr = tmem_base + as * a.acc_cols + ((uint32_t)(quarter * 32) << 16);
+        epilogue_item(ec, t_addr, a.stacked != 0, w.it.nb, w.it.row0, w.it.row_end, w.it.tile, w.it.col0, w.it.split, quarter, lane);
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) {
+          mbar_arrive(&tempty[as]);
+          red_release_cta_shared_add(&s_edone[quarter], 1u); // this warp's partials of the item are written
+        }
+      }
+    } else if (warp >= 7) {
+      // ===================== finalizer group =====================
+      const int we = warp - 7, tid_f = we * 32 + lane;
+      constexpr int GT = kFT;
+      AttnPlan pl;
+      attn_plan<PT>(a, G, s_live_ms, s_cum, pl);
+      const int sl_x = a.op[0].kbps * kTileK, sl_f = a.op[3].kbps * kTileK, sl_o = a.op[1].kbps * kTileK;
+      void* const asm_ = smem + a.attn_smem_off;
+      // warp 0 of the group owns the cursors
+      FWalker wf;
+      int n_counted = 0, att_j = 0, att_u = blockIdx.x;
+      if (we == 0) wf.start(sq);
+      unsigned it_no = 0;
+      int n_stamp = 0;
+      if (D.taps && blockIdx.x == 0 && tid_f == 0) D.tap_times[n_stamp] = (unsigned long long)clock64();
+      ++n_stamp;
+      unsigned idle = 0;
+      for (;; ++it_no) {
+        FDec* dec = &s_dec[it_no & 1];
+        if (we == 0) {
+          int kind = 0;
+          const bool items_left = wf.valid && wf.t < n_layer_ops;
+          if (items_left) {
+            unsigned done = ld_acquire_cta_shared(&s_edone[lane & 3]);
+            done = min(done, __shfl_xor_sync(0xffffffffu, done, 1));
+            done = min(done, __shfl_xor_sync(0xffffffffu, done, 2));
+            if ((unsigned)n_counted < done) {
+              // this item's partials are complete: count the split in; the last arriver finalizes the tile
+              const int which = wf.o.which, m = wf.it.g, j = wf.o.j;
+              int old = 0;
+              if (lane == 0) old = atom_acq_rel_add_s32(ctr + kFcTile + (which * kMaxGrp + m) * kFlowTiles + wf.it.cnt_idx, 1);
+              old = __shfl_sync(0xffffffffu, old, 0);
+              kind = 4;
+              if (old + 1 == (j + 1) * wf.it.cnt_target) {
+                kind = 1;
+                if (lane == 0) {
+                  dec->which = which; dec->m = m; dec->idx = wf.it.cnt_idx; dec->j = j;
+                  dec->row0 = wf.it.row0; dec->row_hi = min(wf.it.row0 + wf.it.nb, wf.it.row_end);
+                }
+              }
+              const int t_before = wf.t;
+              wf.next(sq);
+              ++n_counted;
+              if (D.taps && blockIdx.x == 0 && (!wf.valid || (wf.t >> 2) != (t_before >> 2)) && t_before < n_layer_ops) {
+                if (lane == 0 && n_stamp < 20 * D.max_len + 60) D.tap_times[n_stamp] = (unsigned long long)clock64();
+                ++n_stamp;                                    // CTA 0 counted its last item of a layer-step
+              }
+            }
+          }
+          if (kind == 0) {
+            // next live attention task of this CTA (dead ones are skipped without waiting)
+            AttnTask tk;
+            bool have = false;
+            while (att_j < sq.n_steps) {
+              if (att_u >= pl.n_tasks) { ++att_j; att_u = blockIdx.x; continue; }
+              attn_task_of<PT>(a, pl, s_cum, G, att_u, tk);
+              const SeqState sst = D.seqs[tk.s];
+              if (!r_seq_live(sst) || sst.q < tk.m || att_j >= a.dec.layer_len[tk.m]) { att_u += G; continue; }
+              have = true;
+              break;
+            }
+            if (have) {
+              int v = 0;
+              if (lane == 0) v = ld_acquire_s32(ctr + kFcQkv + tk.m * kFlowSlices + tk.g);
+              v = __shfl_sync(0xffffffffu, v, 0);
+              if (v >= s_qtarget[tk.g] * (att_j + 1)) {
+                kind = 2;
+                if (lane == 0) { dec->tk = tk; dec->j = att_j; }
+                att_u += G;
+              }
+            } else if (!items_left) {
+              kind = 3;
+            }
+          }
+          if (lane == 0) dec->kind = kind;
+        }
+        bar_f<GT>();
+        const int kind = dec->kind;
+        if (kind == 3) break;
+        if (kind == 1) {
+          idle = 0;
+          const int which = dec->which, m = dec->m, idx = dec->idx, j = dec->j, row0 = dec->row0, row_hi = dec->row_hi;
+          const float* part = D.part + a.part_off[which];
+          if (which == 0) {
+            const int hpt = kTileM / D.hd, h0 = idx * hpt;    // heads of the fused QKV output in this tile
+            for (int u = we; u < (row_hi - row0) * hpt; u += GT / 32) {
+              const int r = row0 + u / hpt, hh = h0 + u % hpt;
+              if (D.hd == 128) unit_qkv<128>(a, j, part, r, hh, lane); else unit_qkv<64>(a, j, part, r, hh, lane);
+            }
+          } else if (which == 2) {
+            for (int r = row0 + we; r < row_hi; r += GT / 32) unit_silu(a, j, a.op[2], part, r, idx, lane);
+          } else {
+            for (int r = row0 + we; r < row_hi; r += GT / 32) unit_add_norm(a, j, which == 1 ? 0 : 1, a.op[which], part, r, idx, lane);
+          }
+          fence_proxy_async();                               // operand planes are read by TMA
+          bar_f<GT>();
+          if (tid_f == 0) {
+            if (which == 0) {
+              for (int g = s_glo[idx]; g <= s_ghi[idx]; ++g) red_release_add_s32(ctr + kFcQkv + m * kFlowSlices + g, 1);
+            } else if (which == 1) {
+              red_release_add_s32(ctr + kFcXf + m * kFlowSlices + (idx * kTileM) / sl_x, 1);
+            } else if (which == 2) {
+              red_release_add_s32(ctr + kFcF + m * kFlowSlices + (idx * kTileM) / sl_f, 1);
+            } else {
+              red_release_add_s32(ctr + kFcXa + m * kFlowSlices + (idx * kTileM) / sl_x, 1);
+            }
+          }
+        } else if (kind == 2) {
+          idle = 0;
+          const AttnTask tk = dec->tk;
+          const int j = dec->j;
+          if (tid_f < kFlowSlices) s_ao_cnt[tid_f] = 0;
+          bar_f<GT>();
+          if (D.hd == 128) attn_run<128, GT, PT>(a, pl, tk, j, tid_f, lane, we, reinterpret_cast<AttnSmem<128>*>(asm_), s_ao_cnt, sl_o);
+          else attn_run<64, GT, PT>(a, pl, tk, j, tid_f, lane, we, reinterpret_cast<AttnSmem<64>*>(asm_), s_ao_cnt, sl_o);
+          fence_proxy_async();                               // act_o is read by TMA
+          bar_f<GT>();
+          if (tid_f < kFlowSlices) {
+            const int c = s_ao_cnt[tid_f];
+            if (c > 0) red_release_add_s32(ctr + kFcAo + tk.m * kFlowSlices + tid_f, c);
+          }
+        } else if (kind == 0) {
+          __nanosleep(64);
+          if (++idle > 60000000u) __trap();                  // protocol bug: trap instead of hanging the box
+        } else {
+          idle = 0;
+        }
+      }
+      // ---- tail of the round: grid barriers publish the operands of the adapters / the exit head (as in k_round)
+      unsigned gb = 0;
+      ++gb; grid_bar<GT>(D.gbar, gb * G, tid_f, &s_seen, gb);        // every layer-step finalization is done
+      if (D.taps && blockIdx.x == 0 && tid_f == 0 && n_stamp < 20 * D.max_len + 60) D.tap_times[n_stamp] = (unsigned long long)clock64();
+      ++n_stamp;
+      if (sq.n_ad_ops) {
+        const int gw = blockIdx.x * (GT / 32) + we, n_gw = gridDim.x * (GT / 32);
+        for (int k = 0; k < 2; ++k) {
+          // wait until this CTA's epilogue warps have written the partials of all of its items of adapter op k
+          FDec* dec = &s_dec[0];
+          if (we == 0) {
+            while (wf.valid && wf.t == n_layer_ops + k) { wf.next(sq); ++n_counted; }
+            if (lane == 0) dec->idx = n_counted;
+          }
+          bar_f<GT>();
+          if (tid_f == 0) {
+            unsigned spins = 0;
+            while (min(min(ld_acquire_cta_shared(&s_edone[0]), ld_acquire_cta_shared(&s_edone[1])),
+                       min(ld_acquire_cta_shared(&s_edone[2]), ld_acquire_cta_shared(&s_edone[3]))) < (unsigned)dec->idx) {
+              __nanosleep(32);
+              if (++spins > 100000000u) __trap();
+            }
+          }
+          ++gb; grid_bar<GT>(D.gbar, gb * G, tid_f, &s_seen, gb);
+          if (k == 0) glue_ad1(a, a.op[5], gw, n_gw, lane); else glue_ad2(a, a.op[6], gw, n_gw, lane);
+          ++gb; grid_bar<GT>(D.gbar, gb * G, tid_f, &s_seen, gb);
+        }
+      }
+      if (D.taps && blockIdx.x == 0 && tid_f == 0 && n_stamp < 20 * D.max_len + 60) D.tap_times[n_stamp] = (unsigned long long)clock64();
+    }
+  }
+
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 1) tmem_dealloc(tmem_base, 2 * a.acc_cols);
+}
+
+cudaError_t flow_init() {
+  cudaError_t e = cudaFuncSetAttribute(k_flow<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024);
+  if (e != cudaSuccess) return e;
+  return cudaFuncSetAttribute(k_flow<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024);
+}
+
+// Cooperative launch: all CTAs must be co-resident (they wait on one another's counters).
+cudaError_t launch_flow(const TmSet& tm, const RoundArgs& a, int grid, size_t smem_bytes, cudaStream_t stream) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(grid);
+  cfg.blockDim = dim3(kFlowThreads);
+  cfg.dynamicSmemBytes = smem_bytes;
+  cfg.stream = stream;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeCooperative;
+  at[0].val.cooperative = 1;
+  cfg.attrs = at;
+  cfg.numAttrs = 1;
+  if (cap_of(a.D.N, 0) * (a.D.nh / a.D.nkv) > kAttnPairs) return cudaLaunchKernelEx(&cfg, k_flow<true>, tm, a);
+  return cudaLaunchKernelEx(&cfg, k_flow<false>, tm, a);
+}
+
+}  // namespace dexk

@@ -193,7 +193,7 @@ k_gemm(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CUtensor
       tc_fence_after();
       const uint32_t t_addr = tmem_base + as * a.acc_cols + ((uint32_t)(quarter * 32) << 16);
       const int row0 = a.plan.row_base[it.g];
-      epilogue_item(ec, t_addr, a.stacked != 0, it.nb, row0, row0 + a.plan.rows_cap[it.g], it.tile, it.split, quarter, lane);
+      epilogue_item(ec, t_addr, a.stacked != 0, it.nb, row0, row0 + a.plan.rows_cap[it.g], it.tile, it.tile * kTileM, it.split, quarter, lane);
       tc_fence_before();
       __syncwarp();
       if (lane == 0) mbar_arrive(&tempty[as]);

@@ -48,9 +48,10 @@ __device__ __forceinline__ void mma_stage(uint32_t sA, uint32_t plane_bytes, int
 // Epilogue of one item by one warp: TMEM lanes 32*quarter..+31 = out features tile*128 + 32*quarter + lane,
 // TMEM columns 0..nb-1 = rows row0..row0+nb-1 (rows >= row_end belong to other groups: skipped).
 // stacked: see mma_stage (hi at column 2*c0 + i, lo 16 columns further; added here).
+// col0: out feature (partial column / vocabulary id) of TMEM lane 0; columns >= e.out_dim are not stored.
 __device__ __forceinline__ void epilogue_item(const EpiCtx& e, uint32_t t_addr, bool stacked, int nb, int row0, int row_end,
-                                              int tile, int split, int quarter, int lane) {
-  const int col = tile * kTileM + quarter * 32 + lane;   // out feature / vocabulary id
+                                              int tile, int col0, int split, int quarter, int lane) {
+  const int col = col0 + quarter * 32 + lane;            // out feature / vocabulary id
   for (int c0 = 0; c0 < nb; c0 += 16) {
     if (row0 + c0 >= row_end) break;
     uint32_t v[16];

@@ -75,6 +75,7 @@ __device__ __forceinline__ int stage_count(int q, int m) { return m > q ? 0 : (m
 // a0: expand bookkeeping.  One thread per row slot of the decode plan.
 __global__ void k_rows_decode(Dev D, Plan plan) {
   const int r = blockIdx.x * blockDim.x + threadIdx.x;
+  for (int i = r; i < kFcTotal; i += gridDim.x * blockDim.x) D.flow_ctr[i] = 0;   // k_flow: arrival counters / ready flags
   if (r == 0) {
     *D.gbar = 0u;                                     // grid-barrier counter of this round's k_round
     // live row extent of every stage group and of every exit chunk
