@@ -180,6 +180,9 @@ int32_t dex_get_tokens(dex_ctx* ctx, int32_t seq, int32_t* out, int32_t cap, int
  *                    residual stream after each layer of that node's stage
  *   DEX_TAP_LOGITS : final-depth anchor logits of the last round -> float[vocab]
  *                    (recomputed by a plain CUDA-core kernel from the anchor's exit row)
+ *   DEX_TAP_REF_BLOCKS : what the FUSED exit itself reduced for the final-depth anchor of the last round (tcgen05
+ *                    accumulators, no recompute): float[2 * 4 * ceil(vocab / 128)] = (top-1, top-2) logit of every block
+ *                    of 32 consecutive vocabulary ids (-inf where a block has fewer than 1 / 2 live ids)
  *   DEX_TAP_B      : explore buffer B of `seq` -> int32[2^N - 1] (-1 = empty)
  *   DEX_TAP_FSM    : int32[4] = {q, ctx_len, n_tokens, pending}
  *   DEX_TAP_ROUND_TIMES : uint64[20 * max_m|Pi_m| + 4] SM clock-cycle stamps taken by CTA 0 of
@@ -189,6 +192,7 @@ int32_t dex_get_tokens(dex_ctx* ctx, int32_t seq, int32_t* out, int32_t cap, int
 #define DEX_TAP_B      3
 #define DEX_TAP_FSM    4
 #define DEX_TAP_ROUND_TIMES 5
+#define DEX_TAP_REF_BLOCKS 6
 int32_t dex_debug_read(dex_ctx* ctx, int32_t what, int32_t seq, int32_t a, void* dst, size_t dst_bytes);
 
 /* Kernel-level tap for parity tests of the weight-streaming GEMM:
@@ -207,7 +211,8 @@ int32_t dex_debug_phase_us(dex_ctx* ctx, float* out8);
  * per-class device microseconds accumulated over the dex_step calls since the last reset
  * (same classes as dex_debug_phase_us; zeros unless profiling was on) and the counters
  * {rounds, kernel launches, segment-GEMM launches, segment-GEMM algorithmic weight bytes,
- *  exit-GEMM LM-head bytes, committed-KV bytes attended, 0, 0}; then, if on >= 0, resets both
+ *  exit-GEMM LM-head bytes (algorithmic: once per round), committed-KV bytes attended, LM-head bytes re-streamed for
+ *  further live exit chunks (traffic, not algorithmic), 0}; then, if on >= 0, resets both
  * and switches profiling off (0), on (1: the configured launch structure, graph replay off) or on
  * through the per-op kernels (2: phase breakdown even when round_kernel = 1).  on < 0: read only. */
 int32_t dex_profile(dex_ctx* ctx, int32_t on, double* phase_us_acc8, double* counters8);

@@ -8,7 +8,7 @@ import numpy as np
 DEX_OK, DEX_EINVAL, DEX_ECAPACITY, DEX_ESTATE, DEX_ECUDA = 0, -1, -2, -3, -4
 DEX_MAX_DEPTHS = 8
 DEX_STEP_AUTOCOLLAPSE = 1
-DEX_TAP_HIDDEN, DEX_TAP_LOGITS, DEX_TAP_B, DEX_TAP_FSM, DEX_TAP_ROUND_TIMES = 1, 2, 3, 4, 5
+DEX_TAP_HIDDEN, DEX_TAP_LOGITS, DEX_TAP_B, DEX_TAP_FSM, DEX_TAP_ROUND_TIMES, DEX_TAP_REF_BLOCKS = 1, 2, 3, 4, 5, 6
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 lib_path = os.path.join(_HERE, "libdex_b200.so")
@@ -246,6 +246,11 @@ class Dex:
 
     def tap_logits(self, seq=0):
         return dex_debug_read(self.ctx, DEX_TAP_LOGITS, seq, 0, np.zeros(self.shape.vocab, dtype=np.float32))
+
+    def tap_ref_blocks(self, seq=0):
+        """(top-1, top-2) of every 32-id vocabulary block as reduced by the fused exit epilogue: [n_blocks, 2]."""
+        n = 4 * ((self.shape.vocab + 127) // 128)
+        return dex_debug_read(self.ctx, DEX_TAP_REF_BLOCKS, seq, 0, np.zeros((n, 2), dtype=np.float32))
 
     def tap_B(self, seq=0):
         return dex_debug_read(self.ctx, DEX_TAP_B, seq, 0, np.zeros((1 << len(self.depths)) - 1, dtype=np.int32))

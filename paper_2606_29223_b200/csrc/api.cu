@@ -4,6 +4,7 @@
 #include <algorithm>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <map>
 #include <memory>
@@ -33,6 +34,7 @@ cudaError_t launch_decide(const Dev&, const Plan&, int, cudaStream_t);
 cudaError_t launch_set_cmd(const Dev&, int, int, int, cudaStream_t);
 cudaError_t launch_collapse(const Dev&, const Plan&, int, cudaStream_t);
 cudaError_t launch_tap_logits(const Dev&, int, float*, cudaStream_t);
+cudaError_t launch_tap_ref_tiles(const Dev&, int, int, float2*, cudaStream_t);
 cudaError_t launch_debug_rows(const Dev&, int, cudaStream_t);
 cudaError_t launch_debug_split(const float*, __nv_bfloat16*, int, int, size_t, int, cudaStream_t);
 cudaError_t launch_debug_sum(const float*, float*, int, int, int, int, size_t, cudaStream_t);
@@ -540,7 +542,22 @@ void account_round(dex_ctx* c) {
   c->counters[1] += mega ? 7.0 : 2 + 10.0 * D.max_len + 1 + 1 + 3;
   c->counters[2] += mega ? 1 : gemm_launches;
   c->counters[3] += wbytes;
-  c->counters[4] += 2.0 * c->op[4].dec.out_dim * c->op[4].dec.k_dim * c->exit_plan.n_grp;
+  // algorithmic: the LM head once per round; the kernel re-streams it once per LIVE exit chunk (chunks of
+  // exit_chunk rows; 2 at N = 8 when more than 64 rows are live) - that re-stream is traffic, reported separately
+  int max_end = 0;
+  for (int m = 0; m < D.N; ++m) {
+    int ext = 0;
+    const int cap = cap_of(D.N, m);
+    for (int s = 0; s < c->cfg.max_seqs; ++s) {
+      const HostSeq& hs = c->seqs[s];
+      if (!hs.active || hs.done || hs.q < m) continue;
+      ext = std::max(ext, s * cap + (m == hs.q ? 1 : (1 << (hs.q - 1 - m))));
+    }
+    if (ext > 0) max_end = std::max(max_end, c->dec_plan.row_base[m] + ext);
+  }
+  const int live_chunks = (max_end + D.exit_chunk - 1) / D.exit_chunk;
+  c->counters[4] += 2.0 * c->op[4].dec.out_dim * c->op[4].dec.k_dim;
+  c->counters[6] += 2.0 * c->op[4].dec.out_dim * c->op[4].dec.k_dim * std::max(0, live_chunks - 1);
   c->counters[5] += kv;
 }
 
@@ -669,7 +686,7 @@ int32_t dex_init(dex_ctx** out, const dex_config* cfg, const dex_weights* w, con
     // the round kernel also carves its attention scratch out of dynamic shared memory: fewer ring stages
     const size_t stage = 16384 + (size_t)cfg->act_planes * c->round_ring.x_cap * 128;
     const size_t attn = (round_attn_smem(cfg->head_dim) + 1023) / 1024 * 1024;
-    const size_t budget = 222 * 1024 - attn - 2048;
+    const size_t budget = 219 * 1024 - attn - 2048;
     c->round_ok = budget / stage >= 3;                    // too few ring stages (very wide stages): per-op path
     if ((cfg->sample || c->has_ad) && !c->round_ok) {
       delete c;
@@ -761,12 +778,13 @@ int32_t dex_init(dex_ctx** out, const dex_config* cfg, const dex_weights* w, con
   };
   INIT_FAIL(cu_or_fail(cudaMemsetAsync(ws, 0, L.off[B_KPOOL], c->stream), "memset state"));
   INIT_FAIL(cu_or_fail(cudaMemsetAsync(D.rows, 0, sizeof(RowInfo) * D.R_cap, c->stream), "memset rows"));
-  INIT_FAIL(cu_or_fail(cudaHostAlloc(reinterpret_cast<void**>(&c->result_host), sizeof(dex_step_result) * cfg->max_seqs,
+  INIT_FAIL(cu_or_fail(cudaHostAlloc(reinterpret_cast<void**>(&c->result_host), sizeof(dex_step_result) * cfg->max_seqs + 64,
                                      cudaHostAllocMapped),
                        "cudaHostAlloc"));
-  memset(c->result_host, 0, sizeof(dex_step_result) * cfg->max_seqs);
+  memset(c->result_host, 0, sizeof(dex_step_result) * cfg->max_seqs + 64);
   INIT_FAIL(cu_or_fail(cudaHostGetDevicePointer(reinterpret_cast<void**>(&D.result_dev), c->result_host, 0),
                        "cudaHostGetDevicePointer"));
+  D.dbg_host = reinterpret_cast<int*>(D.result_dev + cfg->max_seqs);
   c->seqs.resize(cfg->max_seqs);
   c->page_table_host.assign((size_t)D.n_pages, 0);
   for (int p = D.n_pages - 1; p >= 0; --p) c->free_pages.push_back(p);
@@ -844,7 +862,10 @@ int32_t dex_step(dex_ctx* c, uint32_t flags, dex_step_result* out) {
         CU(c, cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal));
         int rc = enqueue_step(c, flags, n_chunks);
         cudaError_t e = cudaStreamEndCapture(c->stream, &g);
-        if (rc) return rc;
+        if (rc) {
+          if (e == cudaSuccess && g) cudaGraphDestroy(g);
+          return rc;
+        }
         CU(c, e);
         cudaGraphExec_t ge;
         CU(c, cudaGraphInstantiate(&ge, g, 0));
@@ -856,7 +877,15 @@ int32_t dex_step(dex_ctx* c, uint32_t flags, dex_step_result* out) {
       int rc = enqueue_step(c, flags, n_chunks);
       if (rc) return rc;
     }
-    CU(c, cudaStreamSynchronize(c->stream));
+    {
+      cudaError_t e_ = cudaStreamSynchronize(c->stream);
+      if (e_ != cudaSuccess) {
+        const int* dbg = reinterpret_cast<const int*>(c->result_host + c->cfg.max_seqs);
+        return fail(c, DEX_ECUDA, "dex_step: %s (kernel timeout record: code %d cta %d args %d %d %d %d | %d %d %d %d %d %d %d %d %d %d)",
+                    cudaGetErrorString(e_), dbg[0], dbg[1], dbg[2], dbg[3], dbg[4], dbg[5], dbg[6], dbg[7], dbg[8], dbg[9], dbg[10],
+                    dbg[11], dbg[12], dbg[13], dbg[14], dbg[15]);
+      }
+    }
     collect_phase_times(c);
   }
   for (int s = 0; s < c->cfg.max_seqs; ++s) {
@@ -982,6 +1011,17 @@ int32_t dex_debug_read(dex_ctx* c, int32_t what, int32_t seq, int32_t a, void* d
     float* tmp = c->dbg_stage + (c->dbg_floats - D.vocab);
     CU(c, launch_tap_logits(D, row, tmp, c->stream));
     CU(c, cudaMemcpyAsync(dst, tmp, sizeof(float) * D.vocab, cudaMemcpyDeviceToHost, c->stream));
+    CU(c, cudaStreamSynchronize(c->stream));
+    return DEX_OK;
+  }
+  if (what == DEX_TAP_REF_BLOCKS) {
+    if (hs.last_q_before != D.N - 1) return fail(c, DEX_ESTATE, "the last round did not reach final depth");
+    const size_t bytes = sizeof(float2) * D.ref_tiles;
+    if (dst_bytes < bytes || c->dbg_floats < 2 * (size_t)D.ref_tiles) return fail(c, DEX_EINVAL, "dst too small");
+    const int row = c->dec_plan.row_base[D.N - 1] + seq * cap_of(D.N, D.N - 1);
+    float2* tmp = reinterpret_cast<float2*>(c->dbg_stage);
+    CU(c, launch_tap_ref_tiles(D, row, seq, tmp, c->stream));
+    CU(c, cudaMemcpyAsync(dst, tmp, bytes, cudaMemcpyDeviceToHost, c->stream));
     CU(c, cudaStreamSynchronize(c->stream));
     return DEX_OK;
   }

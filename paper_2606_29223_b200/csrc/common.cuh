@@ -121,6 +121,7 @@ struct Dev {
   int ref_tiles;
   CollapseCmd* cmd;        // [max_seqs]
   dex_step_result* result_dev;    // [max_seqs] (mapped pinned host memory)
+  int* dbg_host;           // [16] mapped pinned host words behind the results: written by a kernel before it traps on a protocol timeout
   float* tap_hidden;       // [R_cap][max_len][d] (taps only)
   unsigned long long* tap_times;  // [20 * max_len + 4] globaltimer stamps of CTA 0 in k_round (taps only)
   int n_pages;

@@ -23,19 +23,26 @@
 // Only the tail of the round (inducing adapters, exit head) keeps grid barriers.
 //
 //   warp 0      weight producer (TMA, always ahead)         warp 6      activation producer (waits on slice counters)
-//   warp 1      tcgen05.mma issuer, owns TMEM               warps 7-10  finalizer group: counts own items, finalizes
-//   warps 2-5   epilogue: TMEM -> split-K partials / arg-max            completed tiles, runs attention tasks
+//   warp 1      tcgen05.mma issuer, owns TMEM               warps 7-10  finalizer group: finalizes completed tiles,
+//   warps 2-5   epilogue: TMEM -> split-K partials / arg-max            runs attention tasks
+//   warp 11     counter: counts this CTA's finished items into the tile counters (one atomic per item, a batch of up
+//               to 32 in flight), queues the tiles it completed for the finalizer group
 #include "round_dev.cuh"
 
 namespace dexk {
 
-constexpr int kFlowThreads = 352;
+constexpr int kFlowThreads = 384;
 constexpr int kFT = 128;             // finalizer group threads (warps 7-10)
 
 // ---------------------------------------------------------------- small helpers
 __device__ __forceinline__ int ld_acquire_s32(const int* p) {
   int v;
   asm volatile("ld.acquire.gpu.global.s32 %0, [%1];\n" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ int ld_relaxed_s32(const int* p) {
+  int v;
+  asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];\n" : "=r"(v) : "l"(p) : "memory");
   return v;
 }
 __device__ __forceinline__ void red_release_add_s32(int* p, int v) {
@@ -53,6 +60,26 @@ __device__ __forceinline__ unsigned ld_acquire_cta_shared(const unsigned* p) {
 }
 __device__ __forceinline__ void red_release_cta_shared_add(unsigned* p, unsigned v) {
   asm volatile("red.release.cta.shared.add.u32 [%0], %1;\n" ::"r"(smem_u32(p)), "r"(v) : "memory");
+}
+// A bounded wait ran out: leave a record in mapped host memory (dex_step reports it), then trap instead of hanging.
+__device__ __noinline__ void flow_die(const Dev& D, int code, int v0, int v1, int v2, int v3) {
+  if ((threadIdx.x & 31) == 0 || code < 0) {
+    volatile int* h = D.dbg_host;
+    h[1] = blockIdx.x; h[2] = v0; h[3] = v1; h[4] = v2; h[5] = v3;
+    if (code == 1) {                                         // the waiting item's stage: what has arrived so far
+      const int m = v1 >> 16;
+      const volatile int* c = D.flow_ctr;
+      h[6] = c[kFcTile + (0 * kMaxGrp + m) * kFlowTiles + 0]; h[7] = c[kFcTile + (0 * kMaxGrp + m) * kFlowTiles + 1];
+      h[8] = c[kFcTile + (1 * kMaxGrp + m) * kFlowTiles + 0]; h[9] = c[kFcTile + (1 * kMaxGrp + m) * kFlowTiles + 1];
+      h[10] = c[kFcQkv + m * kFlowSlices + 0]; h[11] = c[kFcQkv + m * kFlowSlices + 1];
+      h[12] = c[kFcAo + m * kFlowSlices + 0]; h[13] = c[kFcXf + m * kFlowSlices + 0];
+      h[14] = c[kFcXa + m * kFlowSlices + 0]; h[15] = c[kFcF + m * kFlowSlices + 0];
+    }
+    h[0] = code;
+    __threadfence_system();
+  }
+  __nanosleep(1000000);
+  __trap();
 }
 __device__ __forceinline__ int tiles_in_slice(int dim, int slice_cols, int s) {   // 128-column tiles overlapping K slice s
   const int c0 = s * slice_cols, c1 = min(c0 + slice_cols, dim);
@@ -113,7 +140,7 @@ struct FSeq {
     const OpDesc& d = a->op[o.which];
     if (!o.ext && o.which < 4) {
       const int layer = p.layer_lo[it.g] + o.j;
-      if (o.which == 0) {                                  // by KV head group, splits fastest
+      if (o.which == 0) {                           // by KV head group, splits fastest
         const int ti = rem / o.ksplit;
         it.split = rem - ti * o.ksplit;
         it.tile = s_perm[ti];
@@ -180,9 +207,14 @@ template <int GT>
 __device__ __forceinline__ void bar_f() { asm volatile("bar.sync 1, %0;\n" ::"n"(GT) : "memory"); }
 
 // Decision record handed from finalizer warp 0 to the group (double-buffered by loop iteration).
-struct FDec {
-  int kind;                // 0 idle, 1 finalize a tile, 2 attention task, 3 layer-steps done, 4 counted (nothing to do)
+struct FJob {              // a completed out tile (gate/up: pair) waiting for its finalization
   int which, m, idx, j, row0, row_hi;
+};
+constexpr int kFlowQueue = 64;
+struct FDec {
+  int kind;                // 0 idle, 1 finalize a tile, 2 attention task, 3 layer-steps done
+  int j;
+  FJob job;
   AttnTask tk;
 };
 
@@ -215,6 +247,10 @@ __global__ void __launch_bounds__(kFlowThreads, 1) k_flow(const __grid_constant_
   __shared__ int s_qtarget[kFlowSlices];
   __shared__ int s_ao_cnt[kFlowSlices];
   __shared__ FDec s_dec[2];
+  __shared__ FJob s_queue[kFlowQueue];
+  __shared__ unsigned s_qhead, s_qtail;  // jobs pushed by the counter warp / taken by the finalizer group
+  __shared__ unsigned s_cdone;           // the counter warp has counted every layer-step item of this CTA
+  __shared__ unsigned s_tail_items[3];   // this CTA's items up to and including tail op k (adapters W1, W2)
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   if (threadIdx.x < 32) s_valid[threadIdx.x] = 0;
@@ -231,10 +267,13 @@ __global__ void __launch_bounds__(kFlowThreads, 1) k_flow(const __grid_constant_
     s_ghi[i] = (unsigned char)a.flow_tab[kFtGhi + i];
   }
   for (int i = threadIdx.x; i < kFlowSlices; i += blockDim.x) s_qtarget[i] = a.flow_tab[kFtTarget + i];
+  __syncthreads();
   if (threadIdx.x == 0) {
     int steps = 0;
     for (int g = 0; g < 8; ++g) {
-      const int nb = (g < a.dec.n_grp) ? D.grp_nb[g] : 0;
+      // a stage without an expanded row (sparse lattice: only holes) is not live here: the counters order the ops of
+      // a stage through waits that its rows satisfy, and it has nothing to compute anyway
+      const int nb = (g < a.dec.n_grp && s_nvalid[g] > 0) ? D.grp_nb[g] : 0;
       s_nb[g] = nb;
       if (nb > 0) steps = max(steps, a.dec.layer_len[g]);
       s_nb[8 + g] = (g < a.ext.n_grp) ? D.exit_nb[g] : 0;
@@ -242,6 +281,8 @@ __global__ void __launch_bounds__(kFlowThreads, 1) k_flow(const __grid_constant_
     s_steps = steps;
     s_seen = 0;
     s_edone[0] = s_edone[1] = s_edone[2] = s_edone[3] = 0;
+    s_qhead = s_qtail = 0;
+    s_cdone = 0;
     int lm = 0;
     for (int s = 0; s < D.max_seqs; ++s) {                   // live (stage, sequence[, 16-pair pass]) attention families
       const SeqState st = D.seqs[s];
@@ -291,11 +332,17 @@ __global__ void __launch_bounds__(kFlowThreads, 1) k_flow(const __grid_constant_
       FWalker w;
       unsigned st = 0, ph = 0;
       bool wrapped = false;
+      long long t_wait = 0;
+      const bool prof = D.taps && blockIdx.x == 0;
       for (w.start(sq); w.valid; w.next(sq)) {
         const CUtensorMap* desc = (w.t < n_layer_ops && w.o.which == 2) ? &tm.wgu2 : &tm.w[w.o.which];
         const uint32_t tx = kABytes + D.planes * w.it.nb * 128;
         for (int kb = w.it.kb0; kb < w.it.kb1; ++kb) {
-          if (wrapped) mbar_wait(&empty[st], ph ^ 1u);
+          if (wrapped) {
+            const long long t0 = prof ? clock64() : 0;
+            mbar_wait(&empty[st], ph ^ 1u);
+            if (prof) t_wait += clock64() - t0;
+          }
           if (elect_one()) {
             mbar_expect_tx(&full[st], tx);
             tma_load_3d(smem + (size_t)st * stage_bytes, desc, &full[st], kb * kTileK, w.it.c1, w.it.c2, kEvictFirst);
@@ -304,39 +351,57 @@ __global__ void __launch_bounds__(kFlowThreads, 1) k_flow(const __grid_constant_
           if (++st == (unsigned)NS) { st = 0; ph ^= 1u; wrapped = true; }
         }
       }
+      if (prof && lane == 0) D.tap_times[20 * D.max_len + 60] = (unsigned long long)t_wait;   // W: waiting for a free ring slot
     } else if (warp == 6) {
       // ===================== activation producer: waits for the K slice of its item =====================
-      FWalker w;
+      // The counter of item i + 1 is requested (relaxed load) before the boxes of item i are issued and consumed after
+      // them, so its L2 round trip (microseconds under the weight stream) is off the critical path.  The load is
+      // relaxed: what depends on it are async-proxy (TMA) reads issued after fence.proxy.async, of data the finalizer
+      // released at gpu scope before it bumped the counter; a gpu-scope acquire fence here stalls on the SM's
+      // in-flight TMA traffic (measured: every fence.acq_rel.gpu costs microseconds of stream).
+      FWalker w, wn;
       unsigned st = 0, ph = 0;
       bool wrapped = false;
       unsigned seen = 0;
       const int sl_x = a.op[0].kbps * kTileK, sl_o = a.op[1].kbps * kTileK, sl_f = a.op[3].kbps * kTileK;
-      for (w.start(sq); w.valid; w.next(sq)) {
+      auto dep_of = [&](const FWalker& x, const int*& flag, int& target) {
+        flag = nullptr; target = 0;
+        if (!x.valid || x.t >= n_layer_ops) return;
+        const int which = x.o.which, m = x.it.g, s = x.it.split, j = x.o.j;
+        if (which == 0) {
+          flag = ctr + kFcXa + m * kFlowSlices + s;
+          target = j * tiles_in_slice(D.d, sl_x, s);
+        } else if (which == 1) {
+          flag = ctr + kFcAo + m * kFlowSlices + s;
+          const int hs = (min((s + 1) * sl_o, D.nh * D.hd) - s * sl_o) / D.hd;
+          target = (j + 1) * s_nvalid[m] * hs;
+        } else if (which == 2) {
+          flag = ctr + kFcXf + m * kFlowSlices + s;
+          target = (j + 1) * tiles_in_slice(D.d, sl_x, s);
+        } else {
+          flag = ctr + kFcF + m * kFlowSlices + s;
+          target = (j + 1) * tiles_in_slice(D.ffn, sl_f, s);
+        }
+      };
+      long long t_flag = 0, t_slot = 0;
+      const bool prof = D.taps && blockIdx.x == 0;
+      w.start(sq);
+      const int* f_cur;
+      int t_cur, v_cur = 0;
+      dep_of(w, f_cur, t_cur);
+      if (t_cur > 0) v_cur = ld_relaxed_s32(f_cur);
+      while (w.valid) {
         const int which = w.o.which;
         if (w.t < n_layer_ops) {
-          const int m = w.it.g, s = w.it.split, j = w.o.j;
-          const int* flag;
-          int target;
-          if (which == 0) {
-            flag = ctr + kFcXa + m * kFlowSlices + s;
-            target = j * tiles_in_slice(D.d, sl_x, s);
-          } else if (which == 1) {
-            flag = ctr + kFcAo + m * kFlowSlices + s;
-            const int hs = (min((s + 1) * sl_o, D.nh * D.hd) - s * sl_o) / D.hd;
-            target = (j + 1) * s_nvalid[m] * hs;
-          } else if (which == 2) {
-            flag = ctr + kFcXf + m * kFlowSlices + s;
-            target = (j + 1) * tiles_in_slice(D.d, sl_x, s);
-          } else {
-            flag = ctr + kFcF + m * kFlowSlices + s;
-            target = (j + 1) * tiles_in_slice(D.ffn, sl_f, s);
-          }
-          if (target > 0) {
+          if (t_cur > 0) {
             unsigned spins = 0;
-            while (ld_acquire_s32(flag) < target) {
-              __nanosleep(40);
-              if (++spins > 50000000u) __trap();
+            const long long t0 = prof ? clock64() : 0;
+            while (v_cur < t_cur) {
+              __nanosleep(20);
+              v_cur = ld_relaxed_s32(f_cur);
+              if (++spins > 20000000u) flow_die(D, 1, which, (w.it.g << 16) | w.it.split, w.o.j, t_cur);
             }
+            if (prof) t_flag += clock64() - t0;
             fence_proxy_async();
           }
         } else {
@@ -353,10 +418,20 @@ __global__ void __launch_bounds__(kFlowThreads, 1) k_flow(const __grid_constant_
             fence_proxy_async();
           }
         }
+        wn = w;
+        wn.next(sq);
+        const int* f_n;
+        int t_n, v_n = 0;
+        dep_of(wn, f_n, t_n);
+        if (t_n > 0) v_n = ld_relaxed_s32(f_n);              // consumed after this item's boxes are issued
         const CUtensorMap* desc = &tm.x[(which == 0 || which == 2 || which == 5) ? 0 : (which == 1 ? 1 : (which == 4 ? 3 : 2))];
         const int row0 = w.it.row0, nb = w.it.nb;
         for (int kb = w.it.kb0; kb < w.it.kb1; ++kb) {
-          if (wrapped) mbar_wait(&empty[st], ph ^ 1u);
+          if (wrapped) {
+            const long long t0 = prof ? clock64() : 0;
+            mbar_wait(&empty[st], ph ^ 1u);
+            if (prof) t_slot += clock64() - t0;
+          }
           if (elect_one()) {
             uint8_t* sB = smem + (size_t)st * stage_bytes + kABytes;
             if (a.stacked) {
@@ -371,6 +446,11 @@ __global__ void __launch_bounds__(kFlowThreads, 1) k_flow(const __grid_constant_
           __syncwarp();
           if (++st == (unsigned)NS) { st = 0; ph ^= 1u; wrapped = true; }
         }
+        w = wn; f_cur = f_n; t_cur = t_n; v_cur = v_n;
+      }
+      if (prof && lane == 0) {
+        D.tap_times[20 * D.max_len + 61] = (unsigned long long)t_flag;   // A: waiting for a ready counter
+        D.tap_times[20 * D.max_len + 62] = (unsigned long long)t_slot;   // A: waiting for a free ring slot
       }
     } else if (warp == 1) {
       // ===================== MMA issuer =====================
@@ -378,26 +458,43 @@ __global__ void __launch_bounds__(kFlowThreads, 1) k_flow(const __grid_constant_
       unsigned st = 0, ph = 0;
       int n_it = 0;
       const bool stacked = a.stacked != 0;
+      long long t_acc = 0, t_full = 0, t_issue = 0;
+      const bool prof = D.taps && blockIdx.x == 0;
       for (w.start(sq); w.valid; w.next(sq), ++n_it) {
         const int as = n_it & 1;
-        mbar_wait(&tempty[as], ((n_it >> 1) & 1) ^ 1);
+        {
+          const long long t0 = prof ? clock64() : 0;
+          mbar_wait(&tempty[as], ((n_it >> 1) & 1) ^ 1);
+          if (prof) t_acc += clock64() - t0;
+        }
         tc_fence_after();
         const uint32_t d_tmem = tmem_base + as * a.acc_cols;
         const uint32_t idesc = make_idesc_bf16_m128(stacked ? 2 * w.it.nb : w.it.nb);
         uint32_t acc = 0;
         for (int kb = w.it.kb0; kb < w.it.kb1; ++kb) {
-          mbar_wait(&full[st], ph);
+          {
+            const long long t0 = prof ? clock64() : 0;
+            mbar_wait(&full[st], ph);
+            if (prof) t_full += clock64() - t0;
+          }
           tc_fence_after();
+          const long long t1 = prof ? clock64() : 0;
           if (elect_one()) {
             mma_stage(smem_u32(smem + (size_t)st * stage_bytes), plane_bytes, D.planes, stacked, d_tmem, idesc, acc);
             umma_commit(&empty[st]);
           }
           __syncwarp();
+          if (prof) t_issue += clock64() - t1;
           acc = 1;
           if (++st == (unsigned)NS) { st = 0; ph ^= 1u; }
         }
         if (elect_one()) umma_commit(&tfull[as]);
         __syncwarp();
+      }
+      if (prof && lane == 0) {
+        D.tap_times[20 * D.max_len + 65] = (unsigned long long)t_issue;  // M: issuing the MMAs of a stage
+        D.tap_times[20 * D.max_len + 63] = (unsigned long long)t_acc;    // M: waiting for a free accumulator stage
+        D.tap_times[20 * D.max_len + 64] = (unsigned long long)t_full;   // M: waiting for weights + operand of a ring stage
       }
     } else if (warp >= 2 && warp <= 5) {
       // ===================== epilogue: TMEM -> partials of the op's own region / exit arg-max =====================
@@ -425,56 +522,100 @@ __global__ void __launch_bounds__(kFlowThreads, 1) k_flow(const __grid_constant_
           red_release_cta_shared_add(&s_edone[quarter], 1u); // this warp's partials of the item are written
         }
       }
+    } else if (warp == 11) {
+      // ===================== counter warp =====================
+      // Every finished item of this CTA (all four epilogue warps have written its partials) is counted into its out
+      // tile's counter; the arrival that completes the tile queues it for the finalizer group.  Lane l of a batch
+      // handles item n_counted + l: the atomics of a batch are in flight together.
+      FWalker wf;
+      wf.start(sq);
+      unsigned n_counted = 0, head = 0;
+      int n_stamp = 0;
+      if (D.taps && blockIdx.x == 0 && lane == 0) D.tap_times[n_stamp] = (unsigned long long)clock64();
+      ++n_stamp;
+      unsigned idle = 0;
+      while (wf.valid && wf.t < n_layer_ops) {
+        unsigned done = ld_acquire_cta_shared(&s_edone[lane & 3]);
+        done = min(done, __shfl_xor_sync(0xffffffffu, done, 1));
+        done = min(done, __shfl_xor_sync(0xffffffffu, done, 2));
+        if (done <= n_counted) {
+          __nanosleep(200);
+          if (++idle > 30000000u) flow_die(D, 2, (int)n_counted, (int)done, wf.t, wf.i);
+          continue;
+        }
+        idle = 0;
+        const int n = (int)min(done - n_counted, 32u);
+        FJob mine;
+        int* cnt = nullptr;
+        int target = 0, taken = 0;
+        for (int i = 0; i < n && wf.valid && wf.t < n_layer_ops; ++i) {
+          if (i == lane) {
+            mine.which = wf.o.which; mine.m = wf.it.g; mine.idx = wf.it.cnt_idx; mine.j = wf.o.j;
+            mine.row0 = wf.it.row0; mine.row_hi = min(wf.it.row0 + wf.it.nb, wf.it.row_end);
+            cnt = ctr + kFcTile + (mine.which * kMaxGrp + mine.m) * kFlowTiles + mine.idx;
+            target = (mine.j + 1) * wf.it.cnt_target;
+          }
+          const int t_before = wf.t;
+          wf.next(sq);
+          ++taken;
+          if (D.taps && blockIdx.x == 0 && (!wf.valid || wf.t != t_before)) {
+            if (lane == 0 && n_stamp < 20 * D.max_len + 60) D.tap_times[n_stamp] = (unsigned long long)clock64();
+            ++n_stamp;                                        // CTA 0 counted its last item of an op
+          }
+        }
+        n_counted += taken;
+        bool last = false;
+        // release: publishes this CTA's partials of the item.  The acquire side (an L1 invalidation on this SM, which
+        // also costs the TMA units their cached descriptors) is paid only by an arrival that completes a tile.
+        if (lane < taken) last = atom_acq_rel_add_s32(cnt, 1) + 1 == target;
+        const unsigned bal = __ballot_sync(0xffffffffu, last);
+        if (bal) {
+          const int n_new = __popc(bal);
+          unsigned spins = 0;
+          while (head + n_new - ld_acquire_cta_shared(&s_qtail) > (unsigned)kFlowQueue) {   // queue space
+            __nanosleep(32);
+            if (++spins > 100000000u) __trap();
+          }
+          if (last) s_queue[(head + __popc(bal & ((1u << lane) - 1u))) % kFlowQueue] = mine;
+          __syncwarp();
+          head += n_new;
+          if (lane == 0) asm volatile("st.release.cta.shared.u32 [%0], %1;\n" ::"r"(smem_u32(&s_qhead)), "r"(head) : "memory");
+        }
+      }
+      // this CTA's item counts through the adapter ops (the finalizer group waits for their partials in the tail)
+      for (int k = 0; k < 2; ++k) {
+        while (wf.valid && wf.t == n_layer_ops + k && sq.n_ad_ops) { wf.next(sq); ++n_counted; }
+        if (lane == 0) s_tail_items[k] = n_counted;
+      }
+      __syncwarp();
+      if (lane == 0) asm volatile("st.release.cta.shared.u32 [%0], %1;\n" ::"r"(smem_u32(&s_cdone)), "r"(1u) : "memory");
+      if (D.taps && blockIdx.x == 0 && lane == 0 && n_stamp < 20 * D.max_len + 60) D.tap_times[n_stamp] = (unsigned long long)clock64();
     } else if (warp >= 7) {
-      // ===================== finalizer group =====================
+      // ===================== finalizer group (warps 7-10) =====================
       const int we = warp - 7, tid_f = we * 32 + lane;
       constexpr int GT = kFT;
       AttnPlan pl;
       attn_plan<PT>(a, G, s_live_ms, s_cum, pl);
       const int sl_x = a.op[0].kbps * kTileK, sl_f = a.op[3].kbps * kTileK, sl_o = a.op[1].kbps * kTileK;
       void* const asm_ = smem + a.attn_smem_off;
-      // warp 0 of the group owns the cursors
-      FWalker wf;
-      int n_counted = 0, att_j = 0, att_u = blockIdx.x;
-      if (we == 0) wf.start(sq);
-      unsigned it_no = 0;
-      int n_stamp = 0;
-      if (D.taps && blockIdx.x == 0 && tid_f == 0) D.tap_times[n_stamp] = (unsigned long long)clock64();
-      ++n_stamp;
-      unsigned idle = 0;
+      // warp 0 of the group owns the cursors: queue tail, next attention task
+      unsigned tail = 0;
+      int att_j = 0, att_u = blockIdx.x;
+      unsigned it_no = 0, idle = 0;
       for (;; ++it_no) {
         FDec* dec = &s_dec[it_no & 1];
         if (we == 0) {
           int kind = 0;
-          const bool items_left = wf.valid && wf.t < n_layer_ops;
-          if (items_left) {
-            unsigned done = ld_acquire_cta_shared(&s_edone[lane & 3]);
-            done = min(done, __shfl_xor_sync(0xffffffffu, done, 1));
-            done = min(done, __shfl_xor_sync(0xffffffffu, done, 2));
-            if ((unsigned)n_counted < done) {
-              // this item's partials are complete: count the split in; the last arriver finalizes the tile
-              const int which = wf.o.which, m = wf.it.g, j = wf.o.j;
-              int old = 0;
-              if (lane == 0) old = atom_acq_rel_add_s32(ctr + kFcTile + (which * kMaxGrp + m) * kFlowTiles + wf.it.cnt_idx, 1);
-              old = __shfl_sync(0xffffffffu, old, 0);
-              kind = 4;
-              if (old + 1 == (j + 1) * wf.it.cnt_target) {
-                kind = 1;
-                if (lane == 0) {
-                  dec->which = which; dec->m = m; dec->idx = wf.it.cnt_idx; dec->j = j;
-                  dec->row0 = wf.it.row0; dec->row_hi = min(wf.it.row0 + wf.it.nb, wf.it.row_end);
-                }
-              }
-              const int t_before = wf.t;
-              wf.next(sq);
-              ++n_counted;
-              if (D.taps && blockIdx.x == 0 && (!wf.valid || (wf.t >> 2) != (t_before >> 2)) && t_before < n_layer_ops) {
-                if (lane == 0 && n_stamp < 20 * D.max_len + 60) D.tap_times[n_stamp] = (unsigned long long)clock64();
-                ++n_stamp;                                    // CTA 0 counted its last item of a layer-step
-              }
+          const unsigned cdone = ld_acquire_cta_shared(&s_cdone);      // read BEFORE the head: done => head is final
+          const unsigned head = ld_acquire_cta_shared(&s_qhead);
+          if (tail < head) {
+            kind = 1;
+            if (lane == 0) {
+              dec->job = s_queue[tail % kFlowQueue];
+              asm volatile("st.release.cta.shared.u32 [%0], %1;\n" ::"r"(smem_u32(&s_qtail)), "r"(tail + 1) : "memory");
             }
-          }
-          if (kind == 0) {
+            ++tail;
+          } else {
             // next live attention task of this CTA (dead ones are skipped without waiting)
             AttnTask tk;
             bool have = false;
@@ -482,20 +623,23 @@ __global__ void __launch_bounds__(kFlowThreads, 1) k_flow(const __grid_constant_
               if (att_u >= pl.n_tasks) { ++att_j; att_u = blockIdx.x; continue; }
               attn_task_of<PT>(a, pl, s_cum, G, att_u, tk);
               const SeqState sst = D.seqs[tk.s];
-              if (!r_seq_live(sst) || sst.q < tk.m || att_j >= a.dec.layer_len[tk.m]) { att_u += G; continue; }
+              if (!r_seq_live(sst) || sst.q < tk.m || att_j >= a.dec.layer_len[tk.m] || s_nb[tk.m] == 0) { att_u += G; continue; }
               have = true;
               break;
             }
             if (have) {
               int v = 0;
-              if (lane == 0) v = ld_acquire_s32(ctr + kFcQkv + tk.m * kFlowSlices + tk.g);
+              if (lane == 0) v = ld_relaxed_s32(ctr + kFcQkv + tk.m * kFlowSlices + tk.g);
               v = __shfl_sync(0xffffffffu, v, 0);
               if (v >= s_qtarget[tk.g] * (att_j + 1)) {
+                // polled with relaxed loads (an acquire costs the SM an L1 invalidation every time); ONE acquire load of
+                // the counter that has reached its target
+                if (lane == 0) v = ld_acquire_s32(ctr + kFcQkv + tk.m * kFlowSlices + tk.g);
                 kind = 2;
                 if (lane == 0) { dec->tk = tk; dec->j = att_j; }
                 att_u += G;
               }
-            } else if (!items_left) {
+            } else if (cdone) {
               kind = 3;
             }
           }
@@ -506,7 +650,8 @@ __global__ void __launch_bounds__(kFlowThreads, 1) k_flow(const __grid_constant_
         if (kind == 3) break;
         if (kind == 1) {
           idle = 0;
-          const int which = dec->which, m = dec->m, idx = dec->idx, j = dec->j, row0 = dec->row0, row_hi = dec->row_hi;
+          const int which = dec->job.which, m = dec->job.m, idx = dec->job.idx, j = dec->job.j;
+          const int row0 = dec->job.row0, row_hi = dec->job.row_hi;
           const float* part = D.part + a.part_off[which];
           if (which == 0) {
             const int hpt = kTileM / D.hd, h0 = idx * hpt;    // heads of the fused QKV output in this tile
@@ -546,32 +691,23 @@ __global__ void __launch_bounds__(kFlowThreads, 1) k_flow(const __grid_constant_
             const int c = s_ao_cnt[tid_f];
             if (c > 0) red_release_add_s32(ctr + kFcAo + tk.m * kFlowSlices + tid_f, c);
           }
-        } else if (kind == 0) {
-          __nanosleep(64);
-          if (++idle > 60000000u) __trap();                  // protocol bug: trap instead of hanging the box
         } else {
-          idle = 0;
+          __nanosleep(200);
+          if (++idle > 30000000u) flow_die(D, 3, (int)tail, att_j, att_u, (int)ld_acquire_cta_shared(&s_cdone));   // protocol bug
         }
       }
       // ---- tail of the round: grid barriers publish the operands of the adapters / the exit head (as in k_round)
       unsigned gb = 0;
       ++gb; grid_bar<GT>(D.gbar, gb * G, tid_f, &s_seen, gb);        // every layer-step finalization is done
-      if (D.taps && blockIdx.x == 0 && tid_f == 0 && n_stamp < 20 * D.max_len + 60) D.tap_times[n_stamp] = (unsigned long long)clock64();
-      ++n_stamp;
       if (sq.n_ad_ops) {
         const int gw = blockIdx.x * (GT / 32) + we, n_gw = gridDim.x * (GT / 32);
         for (int k = 0; k < 2; ++k) {
           // wait until this CTA's epilogue warps have written the partials of all of its items of adapter op k
-          FDec* dec = &s_dec[0];
-          if (we == 0) {
-            while (wf.valid && wf.t == n_layer_ops + k) { wf.next(sq); ++n_counted; }
-            if (lane == 0) dec->idx = n_counted;
-          }
-          bar_f<GT>();
           if (tid_f == 0) {
+            const unsigned need = s_tail_items[k];
             unsigned spins = 0;
             while (min(min(ld_acquire_cta_shared(&s_edone[0]), ld_acquire_cta_shared(&s_edone[1])),
-                       min(ld_acquire_cta_shared(&s_edone[2]), ld_acquire_cta_shared(&s_edone[3]))) < (unsigned)dec->idx) {
+                       min(ld_acquire_cta_shared(&s_edone[2]), ld_acquire_cta_shared(&s_edone[3]))) < need) {
               __nanosleep(32);
               if (++spins > 100000000u) __trap();
             }
@@ -581,7 +717,6 @@ __global__ void __launch_bounds__(kFlowThreads, 1) k_flow(const __grid_constant_
           ++gb; grid_bar<GT>(D.gbar, gb * G, tid_f, &s_seen, gb);
         }
       }
-      if (D.taps && blockIdx.x == 0 && tid_f == 0 && n_stamp < 20 * D.max_len + 60) D.tap_times[n_stamp] = (unsigned long long)clock64();
     }
   }
 
@@ -591,9 +726,9 @@ __global__ void __launch_bounds__(kFlowThreads, 1) k_flow(const __grid_constant_
 }
 
 cudaError_t flow_init() {
-  cudaError_t e = cudaFuncSetAttribute(k_flow<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024);
+  cudaError_t e = cudaFuncSetAttribute(k_flow<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024);
   if (e != cudaSuccess) return e;
-  return cudaFuncSetAttribute(k_flow<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024);
+  return cudaFuncSetAttribute(k_flow<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024);
 }
 
 // Cooperative launch: all CTAs must be co-resident (they wait on one another's counters).

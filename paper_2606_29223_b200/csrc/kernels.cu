@@ -204,7 +204,7 @@ __global__ void k_seq_init(Dev D, int seq, int n) {
     st.n_tok = n;
     st.last_tok = D.tokens[seq * (D.max_ctx + 1) + n - 1];
     st.pending = 0;
-    st.done = 0;
+    st.done = (n >= D.max_ctx) ? 1 : 0;               // same rule as the host mirror (dex_prefill / dex_rewind)
     st.pad = 0;
     D.seqs[seq] = st;
   }
@@ -836,6 +836,16 @@ __global__ void k_tap_logits(Dev D, int row, float* out) {
   if (lane == 0) out[v] = acc * inv_rms(D, row);
 }
 
+// The fused exit's own per-block maxima of the final-depth anchor row (what the tcgen05 epilogue reduced: top-1 / top-2
+// of every 32 consecutive vocabulary ids), with the deferred RMSNorm scale of the row applied.
+__global__ void k_tap_ref_tiles(Dev D, int row, int seq, float2* out) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= D.ref_tiles) return;
+  const float inv = D.sample ? 1.f : inv_rms(D, row);
+  const float2 v = D.ref_tile[(size_t)seq * D.ref_tiles + i];
+  out[i] = make_float2(v.x * inv, v.y * inv);
+}
+
 __global__ void k_debug_rows(Dev D, int R) {
   const int r = blockIdx.x * blockDim.x + threadIdx.x;
   if (r == 0)
@@ -947,6 +957,10 @@ cudaError_t launch_collapse(const Dev& D, const Plan& p, int eos_id, cudaStream_
 }
 cudaError_t launch_tap_logits(const Dev& D, int row, float* out, cudaStream_t st) {
   k_tap_logits<<<(D.vocab + 7) / 8, 256, 0, st>>>(D, row, out);
+  DEX_LAUNCH_CHECK();
+}
+cudaError_t launch_tap_ref_tiles(const Dev& D, int row, int seq, float2* out, cudaStream_t st) {
+  k_tap_ref_tiles<<<(D.ref_tiles + 255) / 256, 256, 0, st>>>(D, row, seq, out);
   DEX_LAUNCH_CHECK();
 }
 cudaError_t launch_debug_rows(const Dev& D, int R, cudaStream_t st) {

@@ -32,38 +32,13 @@ def _adapters(shape, n_ad, m=0, seed=99):
     return ad
 
 
-def _trace_compare(g, od, n_depths):
-    """Walks the oracle's Alg. 1 trace; returns (#node candidates compared, #near-tie flips, worst hidden error)."""
-    n_cmp, flagged, worst = 0, 0, 0.0
-    for ri, orec in enumerate(od["rounds"]):
-        r = g.step(0)[0]
-        assert r.q_before == orec["q"] and r.layer_evals == orec["layer_evals"], ri
-        assert list(r.rows_per_stage)[:n_depths] == orec["rows_per_stage"]
-        B = g.tap_B()
-        for node in orec["nodes"]:
-            h = g.tap_hidden(node)
-            o = orec["h_out"][node]
-            worst = max(worst, float(np.abs(h[-1] - o).max() / np.abs(o).max()))
-            n_cmp += 1
-            if B[node] != orec["u"][node]:
-                assert orec["u_margin"][node] < MARGIN, (ri, node, B[node], orec["u"][node], orec["u_margin"][node])
-                flagged += 1
-        if flagged:
-            if r.match_k >= 0:
-                g.collapse(0, r.match_k, r.token)
-            break
-        if orec["committed"]:
-            assert r.token == orec["token"] and r.match_k == orec["match_k"], ri
-            g.collapse(0, r.match_k, r.token)
-        else:
-            assert r.match_k == -1 and r.q_after == orec["q_after"]
-    return n_cmp, flagged, worst
-
-
+@pytest.mark.parametrize("rk", [1, 2])
 @pytest.mark.parametrize("X,m", [((2, 4, 6, 8), 0), ((4, 8), 0), ((1, 3, 4, 8), 128), (tuple(range(1, 9)), 0)])
-def test_c1_adapter_exits_match_oracle(P, c1, X, m):
+def test_c1_adapter_exits_match_oracle(P, c1, X, m, rk):
+    """Every round of a 24-token run (tests/trace_util.py: the oracle replays with the GPU's exit decisions forced)."""
     import dex_synth
     from oracle import OracleModel, ar_greedy, dex_decode
+    from trace_util import gpu_trace, compare_with_oracle
     wl, w, p = c1
     T = 24
     ad = _adapters(wl.shape, len(X) - 1, m=m)
@@ -73,17 +48,14 @@ def test_c1_adapter_exits_match_oracle(P, c1, X, m):
     ar = ar_greedy(om, p, T)
     assert np.array_equal(od["tokens"], ar["tokens"])                   # lossless with adapters
     assert [r["u"] for r in od["rounds"]] != [r["u"] for r in plain["rounds"]]   # ... and they do act
-    g = P.Dex(wl.shape, w, X, max_ctx=128, debug_taps=1, use_graph=0, adapters=ad)
+    g = P.Dex(wl.shape, w, X, max_ctx=128, debug_taps=1, use_graph=0, adapters=ad, round_kernel=rk)
     g.prefill(0, p)
-    n_cmp, flagged, worst = _trace_compare(g, od, len(X))
-    assert worst < HID_TOL, worst
-    assert n_cmp > 20 or flagged
-    n_have = len(g.tokens()) - len(p)
-    if n_have < T:
-        g.generate(T - n_have)
+    recs = gpu_trace(g, T)
     dex_tokens = g.tokens()[len(p):len(p) + T]
     g.close()
-    a = P.Dex(wl.shape, w, (wl.shape.n_layers,), max_ctx=128)
+    res = compare_with_oracle(recs, om, p, X, T)
+    assert res["rounds"] == len(recs) >= T and res["nodes"] > 20
+    a = P.Dex(wl.shape, w, (wl.shape.n_layers,), max_ctx=128, round_kernel=rk)
     a.prefill(0, p)
     ar_gpu, _ = a.generate(T)
     a.close()

@@ -93,11 +93,14 @@ def test_gemm_single_plane_is_bf16_rounded_input(P, c1):
     d.close()
 
 
-@pytest.mark.parametrize("rk", [1, 0])
+@pytest.mark.parametrize("rk", [1, 0, 2])
 def test_c1_ar_hidden_logits_tokens(P, c1, c1_bf16, rk):
-    """T3 on config c1 with X = {L} (the AR baseline): every layer's hidden state, the final
-    logits and the token stream against oracle AR greedy."""
+    """T3 on config c1 with X = {L} (the AR baseline): every layer's hidden state, the final logits - both the
+    debug recompute and the fused exit's OWN per-block maxima (tcgen05 accumulators, DEX_TAP_REF_BLOCKS) - and the
+    token stream against oracle AR greedy.  Teacher-forced (R17): a token that differs at an oracle margin < 1e-2
+    is counted and the oracle's token is committed, so all T positions are always compared."""
     from oracle import ar_greedy
+    from trace_util import check_ref_blocks
     wl, w, p = c1
     T = wl.gen_len
     ar = ar_greedy(c1_bf16, p, T, keep_hidden=True, keep_logits=True)
@@ -105,85 +108,56 @@ def test_c1_ar_hidden_logits_tokens(P, c1, c1_bf16, rk):
     d = P.Dex(wl.shape, w, (wl.shape.n_layers,), max_ctx=128, debug_taps=1, use_graph=0, round_kernel=rk)
     d.prefill(0, p)
     assert d.tap_fsm().tolist() == [0, len(p) - 1, len(p), 0]
-    worst_h = worst_l = 0.0
-    toks = []
+    worst_h = worst_l = worst_b = 0.0
+    flagged = 0
     for t in range(T):
-        r = d.step()[0]
-        assert r.committed == 1 and r.match_k == 0 and r.q_before == 0 and r.q_after == 0
+        r = d.step(0)[0]
+        assert r.committed == 0 and r.match_k == 0 and r.q_before == 0
         assert r.layer_evals == wl.shape.n_layers and r.exit_rows == 1
         h = d.tap_hidden(0)
         for l in range(wl.shape.n_layers):
             worst_h = max(worst_h, rel_err(h[l], ar["hidden"][t][l]))
         lg = d.tap_logits()
         worst_l = max(worst_l, float(np.abs(lg - ar["logits"][t]).max()))
+        worst_b = max(worst_b, check_ref_blocks(d.tap_ref_blocks(), ar["logits"][t]))
         assert abs(r.ref_top1 - ar["top1"][t]) < LOGIT_TOL and abs(r.ref_top2 - ar["top2"][t]) < LOGIT_TOL
         if r.token != ar["tokens"][t]:
-            assert margins[t] < MARGIN
-            pytest.skip("low-margin divergence in the auto-collapse run (covered by the forced run)")
-        toks.append(r.token)
+            assert margins[t] < MARGIN, (t, r.token, ar["tokens"][t], margins[t])
+            flagged += 1
+        d.collapse(0, 0, int(ar["tokens"][t]))
     assert worst_h < HID_TOL, worst_h
-    assert worst_l < LOGIT_TOL, worst_l
-    assert np.array_equal(toks, ar["tokens"])
+    assert worst_l < LOGIT_TOL and worst_b < LOGIT_TOL, (worst_l, worst_b)
+    assert flagged <= 2, flagged
     assert np.array_equal(d.tokens()[len(p):], ar["tokens"])
     d.close()
 
 
-@pytest.mark.parametrize("rk", [1, 0])
+@pytest.mark.parametrize("rk", [1, 0, 2])
 @pytest.mark.parametrize("decs", [0, 1])
 @pytest.mark.parametrize("X", [(2, 4, 6, 8), (4, 8), (3, 8), (1, 3, 4, 8), tuple(range(1, 9))])
 def test_c1_dex_matches_oracle(P, c1, c1_bf16, decs, X, rk):
-    """T3/T4 on c1: DEX rounds against the oracle's Alg. 1 trace: committed tokens, selected
-    branch b_k, per-round rows per stage / layer evaluations / critical layers (bit-exact),
-    every new node's candidate token u and stage-boundary hidden state; and the GPU DEX stream
-    against the GPU AR stream (bit-identical)."""
-    from oracle import dex_decode, ar_greedy
+    """T3/T4 on c1: EVERY round of a 32-token DEX run against the oracle's Alg. 1 trace (tests/trace_util.py: the GPU
+    runs free, the oracle replays with the GPU's exit decisions forced; a forced decision must be a near-tie of the
+    oracle's logits): nodes expanded, rows per stage / layer evaluations / critical layers (bit-exact), every new
+    node's candidate token and stage-boundary hidden state, every commit (token, branch b_k, anchor top-2 logits, FSM
+    state after the collapse); then the GPU DEX stream against the GPU AR stream (bit-identical)."""
+    from oracle import ar_greedy
+    from trace_util import gpu_trace, compare_with_oracle
     wl, w, p = c1
     T = 32
-    ar = ar_greedy(c1_bf16, p, T)
-    margins = np.array(ar["top1"]) - np.array(ar["top2"])
-    od = dex_decode(c1_bf16, p, T, X, decs=bool(decs), trace=True)
-    assert np.array_equal(od["tokens"], ar["tokens"])            # losslessness (PAPER.md:208)
     g = P.Dex(wl.shape, w, X, max_ctx=128, debug_taps=1, use_graph=0, decs=decs, round_kernel=rk)
     g.prefill(0, p)
-    n_commit, flagged, worst_h = 0, 0, 0.0
-    for ri, orec in enumerate(od["rounds"]):
-        r = g.step(0)[0]
-        assert r.q_before == orec["q"], ri
-        assert list(r.rows_per_stage)[:len(X)] == orec["rows_per_stage"]
-        assert r.layer_evals == orec["layer_evals"] and r.critical_layers == orec["critical_layers"]
-        assert r.exit_rows == orec["exit_rows"]
-        B = g.tap_B()
-        for node in orec["nodes"]:
-            h = g.tap_hidden(node)
-            worst_h = max(worst_h, rel_err(h[-1], orec["h_out"][node]))
-            if B[node] != orec["u"][node]:
-                # an exit may flip only at a near-tie of the oracle's (masked) logits of that node (R17)
-                assert orec["u_margin"][node] < MARGIN, (ri, node, B[node], orec["u"][node], orec["u_margin"][node])
-                flagged += 1
-        if flagged:
-            # the lattices now explore different candidates: the node-by-node trace no longer applies.
-            # Finish the pending commit, if any; the stream checks below still hold.
-            if r.match_k >= 0:
-                g.collapse(0, r.match_k, r.token)
-            break
-        if orec["committed"]:
-            tok, k = r.token, r.match_k
-            assert tok == orec["token"] and k == orec["match_k"], (ri, tok, orec["token"], k, orec["match_k"])
-            assert abs(r.ref_top1 - orec["ref_top1"]) < LOGIT_TOL
-            g.collapse(0, k, tok)
-            n_commit += 1
-            assert g.tap_fsm().tolist() == [orec["q_after"], len(p) - 1 + n_commit, len(p) + n_commit, 0]
-        else:
-            assert r.match_k == -1 and r.q_after == orec["q_after"]
-    assert worst_h < HID_TOL, worst_h
-    n_have = len(g.tokens()) - len(p)
-    if n_have < T:
-        g.generate(T - n_have)
+    recs = gpu_trace(g, T)
     dex_tokens = g.tokens()[len(p):len(p) + T]
-    bad = np.nonzero(dex_tokens != od["tokens"])[0]
-    if len(bad):                                                  # only a near-tie of the final-depth logits may differ
-        assert margins[bad[0]] < MARGIN, (bad[0], margins[bad[0]])
     g.close()
+    res = compare_with_oracle(recs, c1_bf16, p, X, T, decs=bool(decs))
+    assert res["rounds"] == len(recs) >= T and res["nodes"] >= T                         # coverage: every round, every node
+    assert np.array_equal(res["tokens"], dex_tokens)
+    # the oracle's free-running AR stream may differ from the GPU's only at a near-tie of the final-depth logits
+    ar = ar_greedy(c1_bf16, p, T)
+    bad = np.nonzero(dex_tokens != ar["tokens"])[0]
+    if len(bad):
+        assert ar["top1"][bad[0]] - ar["top2"][bad[0]] < MARGIN, (bad[0],)
     a = P.Dex(wl.shape, w, (wl.shape.n_layers,), max_ctx=128, decs=decs, round_kernel=rk)
     a.prefill(0, p)
     ar_gpu, _ = a.generate(T)
@@ -191,7 +165,7 @@ def test_c1_dex_matches_oracle(P, c1, c1_bf16, decs, X, rk):
     assert np.array_equal(ar_gpu, dex_tokens)                    # H3: bit-identical streams
 
 
-@pytest.mark.parametrize("rk", [1, 0])
+@pytest.mark.parametrize("rk", [1, 0, 2])
 def test_c1_full_run_graph_replay_and_counts(P, c1, c1_bf16, rk):
     """The bench configuration of c1 (64 tokens, CUDA-graph replay, auto-collapse): tokens ==
     oracle, rounds and layer evaluations equal the closed forms of SURVEY 8(c)."""

@@ -28,52 +28,24 @@ def c1_bf16(c1):
     return OracleModel(wl.shape, w, kv_round="bf16")
 
 
-@pytest.mark.parametrize("rk", [1, 0])
+@pytest.mark.parametrize("rk", [1, 0, 2])
 @pytest.mark.parametrize("X,cap", [((2, 4, 6, 8), 1), ((2, 4, 6, 8), 2), (tuple(range(1, 9)), 1), (tuple(range(1, 9)), 2),
                                    (tuple(range(1, 9)), 3), ((1, 3, 4, 8), 2)])
 def test_c1_sparse_lattice_matches_oracle(P, c1, c1_bf16, X, cap, rk):
-    from oracle import dex_decode
+    """Every round of a 24-token run against the oracle's trace with the same cap (tests/trace_util.py: the oracle
+    replays with the GPU's exit decisions forced, so nothing is skipped after a near-tie flip): exactly the oracle's
+    nodes are expanded, counts bit-exact, hidden states, the explored-branch mask and the R26 commit rule."""
+    from trace_util import gpu_trace, compare_with_oracle
     wl, w, p = c1
-    T, N = 24, len(X)
-    od = dex_decode(c1_bf16, p, T, X, trace=True, lookahead=cap)
+    T = 24
     g = P.Dex(wl.shape, w, X, max_ctx=128, debug_taps=1, use_graph=0, lookahead=cap, round_kernel=rk)
     g.prefill(0, p)
-    worst, flagged, n_cmp = 0.0, 0, 0
-    for ri, orec in enumerate(od["rounds"]):
-        r = g.step(0)[0]
-        assert r.q_before == orec["q"], ri
-        assert list(r.rows_per_stage)[:N] == orec["rows_per_stage"], ri
-        assert r.exit_rows == orec["exit_rows"] and r.layer_evals == orec["layer_evals"]
-        assert r.critical_layers == orec["critical_layers"]
-        B = g.tap_B()
-        level = range((1 << orec["q"]) - 1, (2 << orec["q"]) - 1)
-        assert [i for i in level if B[i] >= 0] == orec["nodes"]             # exactly the oracle's nodes were expanded
-        for node in orec["nodes"]:
-            h = g.tap_hidden(node)
-            o = orec["h_out"][node]
-            worst = max(worst, float(np.abs(h[-1] - o).max() / np.abs(o).max()))
-            n_cmp += 1
-            if B[node] != orec["u"][node]:
-                assert orec["u_margin"][node] < MARGIN, (ri, node, B[node], orec["u"][node], orec["u_margin"][node])
-                flagged += 1
-        if flagged:
-            if r.match_k >= 0:
-                g.collapse(0, r.match_k, r.token)
-            break
-        if orec["committed"]:
-            assert [(r.branch_mask >> k) & 1 == 1 for k in range(N - 1)] == orec["explored"], ri
-            assert r.token == orec["token"] and r.match_k == orec["match_k"], ri
-            g.collapse(0, r.match_k, r.token)
-            assert g.tap_fsm()[0] == orec["q_after"]
-        else:
-            assert r.match_k == -1 and r.q_after == orec["q_after"]
-    assert worst < HID_TOL, worst
-    assert n_cmp > 30 or flagged
-    n_have = len(g.tokens()) - len(p)
-    if n_have < T:
-        g.generate(T - n_have)
+    recs = gpu_trace(g, T)
     dex_tokens = g.tokens()[len(p):len(p) + T]
     g.close()
+    res = compare_with_oracle(recs, c1_bf16, p, X, T, lookahead=cap)
+    assert res["rounds"] == len(recs) >= T and res["nodes"] > 30                # coverage: every round, every node
+    assert np.array_equal(res["tokens"], dex_tokens)
     a = P.Dex(wl.shape, w, (wl.shape.n_layers,), max_ctx=128, round_kernel=rk)
     a.prefill(0, p)
     ar_gpu, _ = a.generate(T)
