@@ -145,31 +145,40 @@ def job_tokens_per_s(world, steps, tokens_per_step, ms_max):
     return world * steps * tokens_per_step / (ms_max * 1e-3)
 
 
-def run_rounds(g, T, flags):
-    """DEX rounds until T tokens are committed.  Returns (#rounds, layer_evals, critical_layers, k histogram)."""
-    n, rounds, evals, crit = 0, 0, 0, 0
+def run_rounds(g, T, flags, S=1):
+    """DEX rounds until every one of the S batched sequences has committed T tokens (a sequence that is done keeps
+    stepping with the others, as in a serving batch; only its first T tokens count).  Returns (#rounds,
+    layer_evals, critical_layers, k histogram)."""
+    n = [0] * S
+    rounds, evals, crit = 0, 0, 0
     hist = [0] * 8
-    while n < T:
-        r = g.step(flags)[0]
+    while min(n) < T:
+        res = g.step(flags)
         rounds += 1
-        evals += r.layer_evals
-        crit += r.critical_layers
-        if r.committed:
-            n += 1
-            hist[r.match_k] += 1
-        if r.done or not r.active:
+        alive = False
+        for s in range(S):
+            r = res[s]
+            if n[s] < T:
+                evals += r.layer_evals
+                crit += r.critical_layers
+            if r.committed and n[s] < T:
+                n[s] += 1
+                hist[r.match_k] += 1
+            alive |= bool(r.active and not r.done)
+        if not alive:
             break
     return rounds, evals, crit, hist
 
 
-def time_steps(torch, g, n_prompt, T, K, flags):
-    """K steps (rewind + T committed tokens each) between two CUDA events on the library's stream."""
+def time_steps(torch, g, n_prompt, T, K, flags, S=1):
+    """K steps (rewind + T committed tokens per sequence each) between two CUDA events on the library's stream."""
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     stats = None
     e0.record(g.stream)
     for _ in range(K):
-        g.rewind(0, n_prompt)
-        stats = run_rounds(g, T, flags)
+        for s_ in range(S):
+            g.rewind(s_, n_prompt)
+        stats = run_rounds(g, T, flags, S)
     e1.record(g.stream)
     torch.cuda.synchronize()
     return e0.elapsed_time(e1), stats
@@ -202,9 +211,11 @@ def bench_dex(args):
              for k, v in w_host.items()}
     del w_host
     # the prompt lives in PINNED host memory: dex_prefill copies it to the device inside the e2e region
-    prompt_pin = torch.empty(n_prompt, dtype=torch.int32).pin_memory()
-    prompt = prompt_pin.numpy()
-    prompt[:] = dex_synth.make_prompt(shape.vocab, n_prompt, wl.prompt_seed, seq=replica_prompt_seq(rank))
+    S = wl.n_seqs                        # independent lattices batched into the same launches (c5: 4)
+    prompt_pin = torch.empty((S, n_prompt), dtype=torch.int32).pin_memory()
+    prompts = prompt_pin.numpy()
+    for s_ in range(S):
+        prompts[s_, :] = dex_synth.make_prompt(shape.vocab, n_prompt, wl.prompt_seed, seq=replica_prompt_seq(rank) * S + s_)
     max_ctx = n_prompt + T + 8
     FL = P.DEX_STEP_AUTOCOLLAPSE
     mode = dict(decs=args.decs, sample=1 if args.temperature > 0 else 0, temperature=max(args.temperature, 1e-6),
@@ -212,11 +223,20 @@ def bench_dex(args):
     adapters = None
     if args.adapters:                    # inducing-adapter exits: synthetic, untrained
         adapters = dex_synth.make_adapters(shape, N - 1, seed=wl.weight_seed + 1, alpha=1e-3, m=args.adapter_dim)
-    g = P.Dex(shape, w_dev, X, max_ctx=max_ctx, device=dev, act_planes=args.act_planes, adapters=adapters,
-              lookahead=args.lookahead, **mode)
-    a = P.Dex(shape, w_dev, (L,), max_ctx=max_ctx, device=dev, act_planes=args.act_planes, **mode)
-    g.prefill(0, prompt)
-    a.prefill(0, prompt)
+    g = P.Dex(shape, w_dev, X, max_seqs=S, max_ctx=max_ctx, device=dev, act_planes=args.act_planes, adapters=adapters,
+              lookahead=args.lookahead, round_kernel=args.round_kernel, **mode)
+    a = P.Dex(shape, w_dev, (L,), max_seqs=S, max_ctx=max_ctx, device=dev, act_planes=args.act_planes,
+              round_kernel=args.round_kernel, **mode)
+    for s_ in range(S):
+        g.prefill(s_, prompts[s_])
+        a.prefill(s_, prompts[s_])
+
+    def rewind_all(d):
+        for s_ in range(S):
+            d.rewind(s_, n_prompt)
+
+    def tokens_all(d):
+        return np.stack([d.tokens(s_)[n_prompt:n_prompt + T] for s_ in range(S)])
 
     def barrier():
         torch.cuda.synchronize()
@@ -230,34 +250,34 @@ def bench_dex(args):
     # ---- warm-up (>= 3 steps), also captures the CUDA graphs ----
     W = max(3, args.warmup)
     for _ in range(W):
-        g.rewind(0, n_prompt)
-        run_rounds(g, T, FL)
+        rewind_all(g)
+        run_rounds(g, T, FL, S)
     for _ in range(2):
-        a.rewind(0, n_prompt)
-        run_rounds(a, T, FL)
+        rewind_all(a)
+        run_rounds(a, T, FL, S)
 
     # ---- timed region: K steps, device time, max over ranks ----
     g.profile(0)
     clocks = ClockSampler(local_rank)
     clocks.start()
     barrier()
-    ms, (rounds, evals, crit, hist) = time_steps(torch, g, n_prompt, T, args.steps, FL)
+    ms, (rounds, evals, crit, hist) = time_steps(torch, g, n_prompt, T, args.steps, FL, S)
     barrier()
     clk = clocks.stop()
     _, counters = g.profile(-1)
     ms = max_ranks(ms)
-    dex_tokens = g.tokens()[n_prompt:n_prompt + T].copy()
-    value = job_tokens_per_s(world, args.steps, T, ms)
+    dex_tokens = tokens_all(g)
+    value = job_tokens_per_s(world, args.steps, S * T, ms)
 
     # ---- same-kernel AR baseline (X = {L}) ----
     a.profile(0)
     barrier()
-    ms_ar, (rounds_ar, _, _, _) = time_steps(torch, a, n_prompt, T, args.steps, FL)
+    ms_ar, (rounds_ar, _, _, _) = time_steps(torch, a, n_prompt, T, args.steps, FL, S)
     barrier()
     _, counters_ar = a.profile(-1)
     ms_ar = max_ranks(ms_ar)
-    ar_tokens = a.tokens()[n_prompt:n_prompt + T].copy()
-    ar_value = job_tokens_per_s(world, args.steps, T, ms_ar)
+    ar_tokens = tokens_all(a)
+    ar_value = job_tokens_per_s(world, args.steps, S * T, ms_ar)
     lossless = bool(np.array_equal(dex_tokens, ar_tokens))
 
     # ---- e2e: host prompt -> dex_prefill -> rounds -> dex_get_tokens (host), per step ----
@@ -267,18 +287,19 @@ def bench_dex(args):
     e0.record(g.stream)
     e2e_rounds = 0
     for _ in range(args.steps):
-        g.prefill(0, prompt)
-        e2e_rounds += run_rounds(g, T, FL)[0]
-        out = g.tokens(0, n_prompt + T)
+        for s_ in range(S):
+            g.prefill(s_, prompts[s_])
+        e2e_rounds += run_rounds(g, T, FL, S)[0]
+        out = np.stack([g.tokens(s_, n_prompt + T) for s_ in range(S)])
     e1.record(g.stream)
     barrier()
     wall_ms = (time.perf_counter() - t0) * 1e3
     ms_e2e = max_ranks(max(e0.elapsed_time(e1), 0.0))
-    assert np.array_equal(out[n_prompt:], dex_tokens)
+    assert np.array_equal(out[:, n_prompt:], dex_tokens)
     res_bytes = __import__("ctypes").sizeof(P.DexStepResult)
-    e2e = {"value": world * args.steps * T / (ms_e2e * 1e-3), "unit": UNIT,
-           "h2d_bytes_per_step": int(4 * n_prompt + 4 * g.cfg.max_ctx // g.cfg.page_size + 4),
-           "d2h_bytes_per_step": int(res_bytes * e2e_rounds // args.steps + 4 * (n_prompt + T)),
+    e2e = {"value": world * args.steps * S * T / (ms_e2e * 1e-3), "unit": UNIT,
+           "h2d_bytes_per_step": int(S * (4 * n_prompt + 4 * g.cfg.max_ctx // g.cfg.page_size + 4)),
+           "d2h_bytes_per_step": int(res_bytes * S * e2e_rounds // args.steps + 4 * S * (n_prompt + T)),
            "wall_ms_per_step": wall_ms / args.steps,
            "includes": "dex_prefill of the pinned host prompt, all rounds with per-round host results, dex_get_tokens"}
 
@@ -289,9 +310,9 @@ def bench_dex(args):
     peak, peak_src = measured_hbm_peak()
     roofline, phases = None, None
     if rank == 0:
-        g.rewind(0, n_prompt)
+        rewind_all(g)
         g.profile(1)
-        run_rounds(g, T, FL)
+        run_rounds(g, T, FL, S)
         ph, ct = g.profile(0)
         k_us, k_launches, k_bytes = ph[1], ct[2], ct[3] + ct[4] + ct[5]
         ach = k_bytes / (k_us * 1e-6) / 1e9
@@ -299,9 +320,11 @@ def bench_dex(args):
         roofline = {"kernel": "k_round (persistent round kernel: segment GEMMs + glue + lattice attention + fused exit)",
                     "bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
                     "frac_of_8TBs": ach / NOMINAL_HBM_GBS, "peak_source": peak_src,
-                    "traffic": (ratio * k_bytes / max(1, k_launches)) if ratio else None,
-                    "traffic_source": (f"dram read+write / algorithmic = {ratio:.4f} from {ratio_src} (ncu --set full), "
-                                       "x algorithmic bytes per launch") if ratio else None,
+                    "traffic": (ratio * k_bytes / max(1, k_launches)) if (ratio and wl.key == "c2") else None,
+                    "traffic_source": (f"NOT a counter of this run: dram read+write / algorithmic = {ratio:.4f} measured by the "
+                                       f"committed ncu --set full capture {ratio_src} (c2), x this run's algorithmic bytes "
+                                       "per launch") if ratio else None,
+                    "lm_head_restream_bytes_per_launch": ct[6] / max(1, k_launches),
                     "launches": int(k_launches), "avg_launch_us": k_us / max(1, k_launches),
                     "algorithmic_bytes_per_launch": k_bytes / max(1, k_launches),
                     "share_of_step": k_us / max(1e-9, ph[7] if ph[7] > 0 else sum(ph[:6])),
@@ -309,14 +332,14 @@ def bench_dex(args):
                            "library stream (graph replay off); bytes = bf16 weights of the live stages + LM head + "
                            "committed K/V attended (dex_profile counters)"}
         # the same rounds through the per-op kernels (round_kernel bypassed): where the time would go without k_round
-        g.rewind(0, n_prompt)
+        rewind_all(g)
         g.profile(2)
-        run_rounds(g, T, FL)
+        run_rounds(g, T, FL, S)
         ph2, ct2 = g.profile(0)
         names = ("bookkeeping", "segment_gemm", "glue", "attention", "exit_gemm", "commit_collapse")
-        phases = {n: ph2[i] / T for i, n in enumerate(names)}
+        phases = {n: ph2[i] / (S * T) for i, n in enumerate(names)}
         phases["unit"] = "us per committed token, per-op kernel path (profiled pass, kernels serialised)"
-        phases["k_round_path"] = {"bookkeeping": ph[0] / T, "k_round": ph[1] / T, "commit_collapse": ph[5] / T}
+        phases["k_round_path"] = {"bookkeeping": ph[0] / (S * T), "k_round": ph[1] / (S * T), "commit_collapse": ph[5] / (S * T)}
 
     # whole-step roofline of the timed region (north_star: weight + KV bytes touched per step)
     step_bytes = (counters[3] + counters[4] + counters[5]) / args.steps
@@ -332,22 +355,22 @@ def bench_dex(args):
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "bf16", "data": "synthetic",
             "config": {"workload": f"{wl.key}: {shape.name} L={L} d={shape.d_model} X={list(X)} prompt={n_prompt} "
-                                   f"gen={T} bs=1 {'greedy' if args.temperature <= 0 else 'sample T=%g' % args.temperature} decs={args.decs}"
+                                   f"gen={T} bs={S} {'greedy' if args.temperature <= 0 else 'sample T=%g' % args.temperature} decs={args.decs}"
                                    + (f" adapters m={adapters['w1'].shape[1]} (random init)" if adapters is not None else "")
                                    + (f" lookahead={args.lookahead}" if args.lookahead else ""),
                        "parallelism": "replicas only" if world > 1 else "single GPU",
-                       "act_planes": args.act_planes,
+                       "act_planes": args.act_planes, "round_kernel": args.round_kernel,
                        "l2": "inputs larger than L2 (13.5 GB of weights streamed per pass vs 126 MB L2)",
                        "step": "dex_rewind to the prompt + DEX rounds until gen tokens are committed"},
             "clocks": clk, "e2e": e2e, "gpu_launches": int(counters[1]),
             "roofline": roofline, "cpu_baseline": cpu,
-            "ar_baseline": {"value": ar_value, "unit": UNIT, "ms_per_token": ms_ar / (args.steps * T),
+            "ar_baseline": {"value": ar_value, "unit": UNIT, "ms_per_token": ms_ar / (args.steps * S * T),
                             "hbm_GBs": ar_ach, "frac_of_measured_peak": ar_ach / peak, "frac_of_8TBs": ar_ach / NOMINAL_HBM_GBS,
                             "what": "same library and kernels, X = {L}"},
             "dex_over_ar": value / ar_value,
             "dex_equals_ar_tokens": lossless,
-            "per_token": {"rounds": rounds / T, "layer_evals": evals / T, "critical_layers": crit / T,
-                          "ms": ms / (args.steps * T), "match_k_hist": hist[:N]},
+            "per_token": {"rounds_per_sequence_token": rounds / T, "layer_evals": evals / (S * T), "critical_layers": crit / (S * T),
+                          "ms": ms / (args.steps * S * T), "match_k_hist": hist[:N]},
             "step_roofline": {"bytes_per_step": step_bytes, "achieved_GBs": step_ach, "frac_of_measured_peak": step_ach / peak,
                               "frac_of_8TBs": step_ach / NOMINAL_HBM_GBS,
                               "what": "weights of live stages + LM head per round + committed K/V attended, / timed region"},
@@ -361,7 +384,7 @@ def bench_dex(args):
 
 
 # ------------------------------------------------------------------------------------------------
-def oracle_sample(wl, n_prompt, n_tokens, n_steps):
+def oracle_sample(wl, n_prompt, n_tokens, n_steps, ar_tokens=0):
     """The CPU oracle (NumPy, fp32 at the 7B-class shapes) on a bounded sample of the workload:
     the workload's model tensors and exploration set, a prompt shortened to `n_prompt` tokens
     (prefill untimed), `n_tokens` committed DEX tokens per step.  Returns (seconds per step list,
@@ -383,18 +406,25 @@ def oracle_sample(wl, n_prompt, n_tokens, n_steps):
         t0 = time.perf_counter()
         oracle.dex_decode(om, p, n_tokens, X, decs=True, state=st)
         times.append(time.perf_counter() - t0)
+    ar_s = None
+    if ar_tokens:                          # CPU AR leg: the oracle's own AR greedy, same tensors
+        st = ([list(x) for x in state[0]], [list(x) for x in state[1]])
+        t0 = time.perf_counter()
+        oracle.ar_greedy(om, p, ar_tokens, state=st)
+        ar_s = (ar_tokens, time.perf_counter() - t0)
     try:
         from threadpoolctl import threadpool_info
         threads = max([i.get("num_threads", 1) for i in threadpool_info()] + [1])
     except Exception:
         threads = os.cpu_count()
-    return times, threads
+    return (times, threads, ar_s) if ar_tokens else (times, threads)
 
 
 def cpu_baseline(args, wl):
     n_prompt, n_tok = (wl.prompt_len, 16) if wl.key == "c1" else (8, args.cpu_tokens)
-    times, threads = oracle_sample(wl, n_prompt, n_tok, 1)
+    times, threads, ar_s = oracle_sample(wl, n_prompt, n_tok, 1, ar_tokens=max(4, n_tok // 3))
     return {"value": n_tok / times[0], "unit": UNIT, "cores": int(threads), "kind": "oracle",
+            "ar_value": ar_s[0] / ar_s[1], "ar_what": f"oracle AR greedy on the same tensors, {ar_s[0]} tokens, {ar_s[1]:.1f} s",
             "sample": f"{wl.key} tensors and X, prompt shortened to {n_prompt} tokens (prefill untimed), "
                       f"{n_tok} committed DEX tokens, NumPy {'fp64' if wl.key == 'c1' else 'fp32'}, {times[0]:.1f} s"}
 
@@ -439,6 +469,7 @@ def main():
     ap.add_argument("--gen-len", type=int, default=0)
     ap.add_argument("--prompt-len", type=int, default=0)
     ap.add_argument("--act-planes", type=int, default=2)
+    ap.add_argument("--round-kernel", type=int, default=1, help="1: k_round (grid barriers), 2: k_flow (dataflow, experimental), 0: per-op kernels")
     ap.add_argument("--cpu-tokens", type=int, default=24, help="committed tokens of the oracle sample (c2: about 13 s of CPU work)")
     ap.add_argument("--no-cpu", action="store_true")
     args = ap.parse_args()

@@ -53,7 +53,7 @@ struct OpCfg {          // one projection: Y = X . W^T
 };
 constexpr int kDecodeKb = 8;
 struct RingCfg {        // shared-memory ring of the GEMM for a plan
-  int x_cap, n_stages, acc_cols, stacked;
+  int x_cap, n_stages, acc_cols, n_acc, stacked;
   size_t smem;
 };
 struct HostSeq {
@@ -318,8 +318,9 @@ RingCfg make_ring(const Plan& p, int planes) {
   const size_t budget = 200 * 1024;
   r.n_stages = (int)std::max<size_t>(2, std::min<size_t>(12, budget / stage));
   r.stacked = (planes == 2 && 2 * r.x_cap <= 256) ? 1 : 0;   // one {64, 16, 2} box per 16 rows, N = 2*nb
-  r.acc_cols = 32;
-  while (r.acc_cols < (r.stacked ? 2 : 1) * r.x_cap) r.acc_cols *= 2;
+  r.acc_cols = 32;                                           // hi and lo sums in columns of their own in either layout
+  while (r.acc_cols < planes * r.x_cap) r.acc_cols *= 2;
+  r.n_acc = 2 * r.acc_cols <= 512 ? 2 : 1;
   r.smem = r.n_stages * stage + 1024 + 512;
   return r;
 }
@@ -375,6 +376,7 @@ int run_gemm(dex_ctx* c, int which, const OpDesc& o, const CUtensorMap& tmX, con
   a.x_cap = ring.x_cap;
   a.n_stages = ring.n_stages;
   a.acc_cols = ring.acc_cols;
+  a.n_acc = ring.n_acc;
   a.stacked = ring.stacked;
   a.grp_nb = grp_nb;
   a.rows = c->D.rows;
@@ -687,7 +689,7 @@ int32_t dex_init(dex_ctx** out, const dex_config* cfg, const dex_weights* w, con
     const size_t stage = 16384 + (size_t)cfg->act_planes * c->round_ring.x_cap * 128;
     const size_t attn = (round_attn_smem(cfg->head_dim) + 1023) / 1024 * 1024;
     const size_t budget = 219 * 1024 - attn - 2048;
-    c->round_ok = budget / stage >= 3;                    // too few ring stages (very wide stages): per-op path
+    c->round_ok = budget / stage >= 3 && c->round_ring.n_acc == 2;   // too few ring stages (very wide stages): per-op path
     if ((cfg->sample || c->has_ad) && !c->round_ok) {
       delete c;
       return fail(nullptr, DEX_ECAPACITY, "sampling mode / inducing adapters need the round kernel, whose ring does not fit this stage width");

@@ -149,6 +149,13 @@ __device__ __forceinline__ float key2f(uint32_t k) {
   return __uint_as_float(u);
 }
 
+// Sum of squares of four values in ONE fixed instruction sequence: every producer of ss_part (k_gather_norm, k_add_norm,
+// the glue units of the round kernels) must give the same bits for the same x, whichever kernel computes it - a row's
+// first norm of a stage is taken by k_gather_norm in a DEX round and by the previous layer's add+norm in the AR pass (H3).
+__device__ __forceinline__ float sumsq4(float4 v) {
+  return __fmaf_rn(v.w, v.w, __fmaf_rn(v.z, v.z, __fmaf_rn(v.y, v.y, __fmul_rn(v.x, v.x))));
+}
+
 __device__ __forceinline__ float inv_rms(const Dev& D, int r) {
   const float4* p = reinterpret_cast<const float4*>(D.ss_part + (size_t)r * kSsSeg);
   const int n4 = ((D.d + 127) / 128 + 3) / 4;            // float4 groups that hold segments (unused segments hold 0)
@@ -216,6 +223,7 @@ struct GemmArgs {
   int x_cap;               // activation rows per ring stage (multiple of 16)
   int n_stages;            // ring depth
   int acc_cols;            // TMEM columns per accumulator stage (power of two >= 32)
+  int n_acc;               // accumulator stages (2; 1 when two planes of 256 rows fill the 512 TMEM columns)
   int stacked;             // 1: both activation planes are one B operand of N = x_cap + nb (gemm_dev.cuh)
   const int* grp_nb;
   const RowInfo* rows;

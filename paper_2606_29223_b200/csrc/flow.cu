@@ -318,6 +318,7 @@ __global__ void __launch_bounds__(kFlowThreads, 1) k_flow(const __grid_constant_
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot;
+  const uint32_t lo_off = (!a.stacked && D.planes == 2) ? (uint32_t)a.x_cap : 0u;   // lo-plane accumulator columns (gemm_dev.cuh)
 
   FSeq sq;
   sq.a = &a; sq.s_nb = s_nb; sq.s_perm = s_perm; sq.n_steps = s_steps; sq.n_ad_ops = (D.ad_m > 0 && D.N >= 2) ? 2 : 0;
@@ -480,7 +481,7 @@ __global__ void __launch_bounds__(kFlowThreads, 1) k_flow(const __grid_constant_
           tc_fence_after();
           const long long t1 = prof ? clock64() : 0;
           if (elect_one()) {
-            mma_stage(smem_u32(smem + (size_t)st * stage_bytes), plane_bytes, D.planes, stacked, d_tmem, idesc, acc);
+            mma_stage(smem_u32(smem + (size_t)st * stage_bytes), plane_bytes, D.planes, stacked, d_tmem, lo_off, idesc, acc);
             umma_commit(&empty[st]);
           }
           __syncwarp();
@@ -514,7 +515,7 @@ __global__ void __launch_bounds__(kFlowThreads, 1) k_flow(const __grid_constant_
         mbar_wait(&tfull[as], (n_it >> 1) & 1);
         tc_fence_after();
         const uint32_t t_addr = tmem_base + as * a.acc_cols + ((uint32_t)(quarter * 32) << 16);
-        epilogue_item(ec, t_addr, a.stacked != 0, w.it.nb, w.it.row0, w.it.row_end, w.it.tile, w.it.col0, w.it.split, quarter, lane);
+        epilogue_item(ec, t_addr, a.stacked != 0, lo_off, w.it.nb, w.it.row0, w.it.row_end, w.it.tile, w.it.col0, w.it.split, quarter, lane);
         tc_fence_before();
         __syncwarp();
         if (lane == 0) {

@@ -95,7 +95,7 @@ k_gemm(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CUtensor
     tma_prefetch_desc(&tmX);
   }
   if (warp == 1) {
-    tmem_alloc(tmem_slot, 2 * a.acc_cols);
+    tmem_alloc(tmem_slot, a.n_acc * a.acc_cols);
     tmem_relinquish();
   }
   tc_fence_before();
@@ -103,6 +103,7 @@ k_gemm(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CUtensor
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot;
   const int n_items = n_live_s * a.n_tiles * a.ksplit;
+  const uint32_t lo_off = (!a.stacked && a.planes == 2) ? (uint32_t)a.x_cap : 0u;   // lo-plane accumulator columns (gemm_dev.cuh)
 
   if (warp == 0) {
     // ===================== TMA producer =====================
@@ -156,8 +157,8 @@ k_gemm(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CUtensor
       int n_it = 0;
       for (int item = blockIdx.x; item < n_items; item += gridDim.x, ++n_it) {
         Item it = decode_item(a, item, live_g, live_nb);
-        const int as = n_it & 1;
-        const uint32_t aphase = (n_it >> 1) & 1;
+        const int as = n_it % a.n_acc;
+        const uint32_t aphase = (n_it / a.n_acc) & 1;
         mbar_wait(&tempty[as], aphase ^ 1);
         tc_fence_after();
         const uint32_t d_tmem = tmem_base + as * a.acc_cols;
@@ -166,7 +167,8 @@ k_gemm(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CUtensor
         for (int kb = it.kb0; kb < it.kb1; ++kb) {
           mbar_wait(&full[stage], phase);
           tc_fence_after();
-          mma_stage(smem_u32(smem + (size_t)stage * stage_bytes), plane_bytes, a.planes, a.stacked != 0, d_tmem, idesc, acc);
+          mma_stage(smem_u32(smem + (size_t)stage * stage_bytes), plane_bytes, a.planes, a.stacked != 0, d_tmem, lo_off, idesc, acc);
+          acc = 1;
           umma_commit(&empty[stage]);   // frees the ring slot when these MMAs have read it
           if (++stage == a.n_stages) {
             stage = 0;
@@ -187,13 +189,13 @@ k_gemm(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CUtensor
     int n_it = 0;
     for (int item = blockIdx.x; item < n_items; item += gridDim.x, ++n_it) {
       Item it = decode_item(a, item, live_g, live_nb);
-      const int as = n_it & 1;
-      const uint32_t aphase = (n_it >> 1) & 1;
+      const int as = n_it % a.n_acc;
+      const uint32_t aphase = (n_it / a.n_acc) & 1;
       mbar_wait(&tfull[as], aphase);
       tc_fence_after();
       const uint32_t t_addr = tmem_base + as * a.acc_cols + ((uint32_t)(quarter * 32) << 16);
       const int row0 = a.plan.row_base[it.g];
-      epilogue_item(ec, t_addr, a.stacked != 0, it.nb, row0, row0 + a.plan.rows_cap[it.g], it.tile, it.tile * kTileM, it.split, quarter, lane);
+      epilogue_item(ec, t_addr, a.stacked != 0, lo_off, it.nb, row0, row0 + a.plan.rows_cap[it.g], it.tile, it.tile * kTileM, it.split, quarter, lane);
       tc_fence_before();
       __syncwarp();
       if (lane == 0) mbar_arrive(&tempty[as]);
@@ -202,7 +204,7 @@ k_gemm(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CUtensor
 
   tc_fence_before();
   __syncthreads();
-  if (warp == 1) tmem_dealloc(tmem_base, 2 * a.acc_cols);
+  if (warp == 1) tmem_dealloc(tmem_base, a.n_acc * a.acc_cols);
 }
 
 cudaError_t gemm_init() {

@@ -28,19 +28,22 @@ struct EpiCtx {
 //             [rows 0-15 hi | rows 0-15 lo | rows 16-31 hi | ...]: ONE B operand of N = 2*nb.  hi products of
 //             row r accumulate in TMEM column 32*(r/16) + r%16, lo products 16 columns further, the epilogue
 //             adds the two.  Half the MMA and TMA instructions of the plane-by-plane form.
-//   otherwise (2*nb > 256, or one plane): plane p at byte offset p*plane_bytes, N = nb, planes one after
-//             the other into the same columns.
+//   otherwise (2*nb > 256, or one plane): plane p at byte offset p*plane_bytes, N = nb; the lo plane accumulates in
+//             columns of its own, lo_off columns after the hi plane's, and the epilogue adds the two - the SAME
+//             arithmetic as the stacked form (sum of hi products + sum of lo products), so a row's bits do not depend
+//             on which layout the context's row capacity selects (H3: a 256-row DEX context and its AR baseline).
 __device__ __forceinline__ void mma_stage(uint32_t sA, uint32_t plane_bytes, int planes, bool stacked, uint32_t d_tmem,
-                                          uint32_t idesc, uint32_t& acc) {
+                                          uint32_t lo_off, uint32_t idesc, uint32_t acc) {
   const uint32_t sB = sA + kABytes;
   const uint64_t da = make_sw128_kmajor_desc(sA);
   const int np = stacked ? 1 : planes;
   for (int p = 0; p < np; ++p) {
     const uint64_t db = make_sw128_kmajor_desc(sB + p * plane_bytes);
+    uint32_t ac = acc;
 #pragma unroll
     for (int k = 0; k < kTileK / 16; ++k) {
-      umma_bf16(d_tmem, da + (k * 32 >> 4), db + (k * 32 >> 4), idesc, acc);
-      acc = 1;
+      umma_bf16(d_tmem + p * lo_off, da + (k * 32 >> 4), db + (k * 32 >> 4), idesc, ac);
+      ac = 1;
     }
   }
 }
@@ -49,16 +52,17 @@ __device__ __forceinline__ void mma_stage(uint32_t sA, uint32_t plane_bytes, int
 // TMEM columns 0..nb-1 = rows row0..row0+nb-1 (rows >= row_end belong to other groups: skipped).
 // stacked: see mma_stage (hi at column 2*c0 + i, lo 16 columns further; added here).
 // col0: out feature (partial column / vocabulary id) of TMEM lane 0; columns >= e.out_dim are not stored.
-__device__ __forceinline__ void epilogue_item(const EpiCtx& e, uint32_t t_addr, bool stacked, int nb, int row0, int row_end,
-                                              int tile, int col0, int split, int quarter, int lane) {
+// lo_off > 0 (two planes, not stacked): the lo plane's sums sit lo_off columns after the hi plane's.
+__device__ __forceinline__ void epilogue_item(const EpiCtx& e, uint32_t t_addr, bool stacked, uint32_t lo_off, int nb, int row0,
+                                              int row_end, int tile, int col0, int split, int quarter, int lane) {
   const int col = col0 + quarter * 32 + lane;            // out feature / vocabulary id
   for (int c0 = 0; c0 < nb; c0 += 16) {
     if (row0 + c0 >= row_end) break;
     uint32_t v[16];
     tmem_ld16(t_addr + (stacked ? 2 * c0 : c0), v);
-    if (stacked) {
+    if (stacked || lo_off) {
       uint32_t v2[16];
-      tmem_ld16(t_addr + 2 * c0 + 16, v2);
+      tmem_ld16(stacked ? t_addr + 2 * c0 + 16 : t_addr + lo_off + c0, v2);
       tmem_ld_wait();
 #pragma unroll
       for (int i = 0; i < 16; ++i) v[i] = __float_as_uint(__uint_as_float(v[i]) + __uint_as_float(v2[i]));

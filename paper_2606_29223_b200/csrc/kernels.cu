@@ -225,44 +225,37 @@ __global__ void k_rope_table(Dev D, double theta, int n_pos) {
 // a1 + first RMSNorm: h_in = parent's frontier hidden (depth expansion) or Embed[tok]
 // (position expansion), then a = RMSNorm(h_in; w_attn[first layer of the stage]).
 __global__ void __launch_bounds__(1024) k_gather_norm(Dev D, Plan plan) {
-  __shared__ float red[33];
   const int r = blockIdx.x;
   const RowInfo ri = D.rows[r];
   if (!ri.valid) return;
   float* x = D.x_cur + (size_t)r * D.d;
-  const int nv = D.d >> 2;
-  float4 xv[2];
-  float ss = 0.f;
-#pragma unroll
-  for (int it = 0; it < 2; ++it) {
-    const int i = threadIdx.x + it * blockDim.x;
-    if (i < nv) {
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, n_warps = blockDim.x >> 5;
+  const int n_seg = (D.d + 127) / 128;
+  const float* w = D.norm_attn + (size_t)plan.layer_lo[ri.grp] * D.d;
+  const size_t ps = (size_t)D.R_cap * D.d;
+  // Warp unit = 128-element segment, lane = 4 consecutive elements, sum of squares per segment: the SAME reduction as
+  // the add+norm units of the round kernels and k_add_norm (deferred RMSNorm scale, H3: a row's norm must not depend
+  // on which kernel produced it)
+  for (int seg = warp; seg < kSsSeg; seg += n_warps) {
+    float ss = 0.f;
+    const int i = seg * 128 + lane * 4;
+    if (seg < n_seg && i < D.d) {
       float4 v;
       if (ri.parent_row >= 0) {
-        v = ld4(D.x_front + (size_t)ri.parent_row * D.d + 4 * i);
+        v = ld4(D.x_front + (size_t)ri.parent_row * D.d + i);
       } else {
-        const uint2 pk = *reinterpret_cast<const uint2*>(D.embed + (size_t)ri.tok_in * D.d + 4 * i);
+        const uint2 pk = *reinterpret_cast<const uint2*>(D.embed + (size_t)ri.tok_in * D.d + i);
         const float2 a = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(&pk.x));
         const float2 b = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(&pk.y));
         v = make_float4(a.x, a.y, b.x, b.y);
       }
-      xv[it] = v;
-      *reinterpret_cast<float4*>(x + 4 * i) = v;
-      ss += v.x * v.x + v.y * v.y + v.z * v.z + v.w * v.w;
+      *reinterpret_cast<float4*>(x + i) = v;
+      ss = sumsq4(v);
+      const float4 wv = ld4(w + i);
+      split_store4(D.act_a, ps, (size_t)r * D.d + i, make_float4(v.x * wv.x, v.y * wv.y, v.z * wv.z, v.w * wv.w), D.planes);
     }
-  }
-  ss = block_sum(ss, red);
-  if (threadIdx.x < kSsSeg) D.ss_part[(size_t)r * kSsSeg + threadIdx.x] = threadIdx.x == 0 ? ss : 0.f;   // deferred scale
-  const float* w = D.norm_attn + (size_t)plan.layer_lo[ri.grp] * D.d;
-  const size_t ps = (size_t)D.R_cap * D.d;
-#pragma unroll
-  for (int it = 0; it < 2; ++it) {
-    const int i = threadIdx.x + it * blockDim.x;
-    if (i < nv) {
-      const float4 wv = ld4(w + 4 * i), v = xv[it];
-      split_store4(D.act_a, ps, (size_t)r * D.d + 4 * i,
-                   make_float4(v.x * wv.x, v.y * wv.y, v.z * wv.z, v.w * wv.w), D.planes);
-    }
+    ss = warp_sum(ss);
+    if (lane == 0) D.ss_part[(size_t)r * kSsSeg + seg] = ss;                 // unused segments hold 0
   }
 }
 
@@ -270,9 +263,8 @@ __global__ void __launch_bounds__(1024) k_gather_norm(Dev D, Plan plan) {
 //   mode 0 (after o_proj):    w = norm_ffn[l]                      -> act_a
 //   mode 1 (after down_proj): w = norm_attn[l+1] if the stage continues -> act_a,
 //                             else the shared final norm (exit) -> act_e
-// One CTA per row, one float4 per thread and pass (d <= 8192), all split loads in flight at once.
+// One CTA per row; warp unit = 128-element segment (see k_gather_norm), all split loads of a unit in flight at once.
 __global__ void __launch_bounds__(1024) k_add_norm(Dev D, Plan plan, int step, int mode, int ksplit, size_t split_stride, int ld) {
-  __shared__ float red[33];
   pdl_trigger();
   const int r = blockIdx.x;
   const RowInfo ri = D.rows[r];
@@ -280,24 +272,8 @@ __global__ void __launch_bounds__(1024) k_add_norm(Dev D, Plan plan, int step, i
   const int layer = plan.layer_lo[ri.grp] + step;
   float* x = D.x_cur + (size_t)r * D.d;
   const float* p = D.part + (size_t)r * ld;
-  const int nv = D.d >> 2;
-  pdl_wait();
-  float4 xv[2];
-  float ss = 0.f;
-#pragma unroll
-  for (int it = 0; it < 2; ++it) {
-    const int i = threadIdx.x + it * blockDim.x;
-    if (i < nv) {
-      float4 a = sum_splits4(p + 4 * i, ksplit, split_stride);
-      float4 v = add4(ld4(x + 4 * i), a);
-      xv[it] = v;
-      *reinterpret_cast<float4*>(x + 4 * i) = v;
-      ss += v.x * v.x + v.y * v.y + v.z * v.z + v.w * v.w;
-      if (mode == 1 && D.taps) *reinterpret_cast<float4*>(D.tap_hidden + ((size_t)r * D.max_len + step) * D.d + 4 * i) = v;
-    }
-  }
-  ss = block_sum(ss, red);
-  if (threadIdx.x < kSsSeg) D.ss_part[(size_t)r * kSsSeg + threadIdx.x] = threadIdx.x == 0 ? ss : 0.f;   // deferred scale
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, n_warps = blockDim.x >> 5;
+  const int n_seg = (D.d + 127) / 128;
   const float* w;
   __nv_bfloat16* dst = D.act_a;
   if (mode == 0) {
@@ -309,14 +285,21 @@ __global__ void __launch_bounds__(1024) k_add_norm(Dev D, Plan plan, int step, i
     dst = D.act_e;
   }
   const size_t ps = (size_t)D.R_cap * D.d;
-#pragma unroll
-  for (int it = 0; it < 2; ++it) {
-    const int i = threadIdx.x + it * blockDim.x;
-    if (i < nv) {
-      const float4 wv = ld4(w + 4 * i), v = xv[it];
-      split_store4(dst, ps, (size_t)r * D.d + 4 * i,
-                   make_float4(v.x * wv.x, v.y * wv.y, v.z * wv.z, v.w * wv.w), D.planes);
+  pdl_wait();
+  for (int seg = warp; seg < n_seg; seg += n_warps) {
+    float ss = 0.f;
+    const int i = seg * 128 + lane * 4;
+    if (i < D.d) {
+      const float4 a = sum_splits4(p + i, ksplit, split_stride);
+      const float4 v = add4(ld4(x + i), a);
+      *reinterpret_cast<float4*>(x + i) = v;
+      ss = sumsq4(v);
+      if (mode == 1 && D.taps) *reinterpret_cast<float4*>(D.tap_hidden + ((size_t)r * D.max_len + step) * D.d + i) = v;
+      const float4 wv = ld4(w + i);
+      split_store4(dst, ps, (size_t)r * D.d + i, make_float4(v.x * wv.x, v.y * wv.y, v.z * wv.z, v.w * wv.w), D.planes);
     }
+    ss = warp_sum(ss);
+    if (lane == 0) D.ss_part[(size_t)r * kSsSeg + seg] = ss;
   }
 }
 

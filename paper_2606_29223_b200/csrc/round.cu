@@ -101,6 +101,7 @@ __global__ void __launch_bounds__(kMaxThreads, 1) k_round(const __grid_constant_
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot;
+  const uint32_t lo_off = (!a.stacked && D.planes == 2) ? (uint32_t)a.x_cap : 0u;   // lo-plane accumulator columns (gemm_dev.cuh)
 
   Seq sq;
   sq.a = &a; sq.s_nb = s_nb; sq.n_steps = s_steps; sq.n_ad_ops = (D.ad_m > 0 && D.N >= 2) ? 2 : 0;
@@ -186,7 +187,7 @@ __global__ void __launch_bounds__(kMaxThreads, 1) k_round(const __grid_constant_
           mbar_wait(&full[st], ph);
           tc_fence_after();
           if (elect_one()) {
-            mma_stage(smem_u32(smem + (size_t)st * stage_bytes), plane_bytes, D.planes, stacked, d_tmem, idesc, acc);
+            mma_stage(smem_u32(smem + (size_t)st * stage_bytes), plane_bytes, D.planes, stacked, d_tmem, lo_off, idesc, acc);
             umma_commit(&empty[st]);     // frees the ring slot when these MMAs have read it
           }
           __syncwarp();
@@ -229,7 +230,7 @@ __global__ void __launch_bounds__(kMaxThreads, 1) k_round(const __grid_constant_
           mbar_wait(&tfull[as], (n_it >> 1) & 1);
           tc_fence_after();
           const uint32_t t_addr = tmem_base + as * a.acc_cols + ((uint32_t)(quarter * 32) << 16);
-          epilogue_item(ec, t_addr, a.stacked != 0, w.it.nb, w.it.row0, w.it.row_end, w.it.tile, w.it.tile * kTileM, w.it.split, quarter, lane);
+          epilogue_item(ec, t_addr, a.stacked != 0, lo_off, w.it.nb, w.it.row0, w.it.row_end, w.it.tile, w.it.tile * kTileM, w.it.split, quarter, lane);
           tc_fence_before();
           __syncwarp();
           if (lane == 0) mbar_arrive(&tempty[as]);

@@ -240,7 +240,7 @@ __device__ __forceinline__ void unit_add_norm(const RoundArgs& a, int j, int mod
     const float4 s4 = sv[0];
     const float4 v = r_add4(xv, s4);
     *reinterpret_cast<float4*>(x) = v;
-    ss = v.x * v.x + v.y * v.y + v.z * v.z + v.w * v.w;
+    ss = sumsq4(v);
     if (mode == 1 && D.taps) *reinterpret_cast<float4*>(D.tap_hidden + ((size_t)r * D.max_len + j) * D.d + i) = v;
     r_split_store4(dst, (size_t)D.R_cap * D.d, (size_t)r * D.d + i, make_float4(v.x * wv.x, v.y * wv.y, v.z * wv.z, v.w * wv.w),
                    D.planes);
@@ -343,7 +343,7 @@ static __device__ void glue_ad2(const RoundArgs& a, const OpDesc& op, int gw, in
       const float4 wv = r_ld4(D.norm_final + i);
       const float4 v = make_float4(xv.x + al * (sv[0].x + bv.x), xv.y + al * (sv[0].y + bv.y), xv.z + al * (sv[0].z + bv.z),
                                    xv.w + al * (sv[0].w + bv.w));
-      ss = v.x * v.x + v.y * v.y + v.z * v.z + v.w * v.w;
+      ss = sumsq4(v);
       r_split_store4(D.act_e, (size_t)D.R_cap * D.d, (size_t)r * D.d + i, make_float4(v.x * wv.x, v.y * wv.y, v.z * wv.z, v.w * wv.w),
                      D.planes);
     }

@@ -118,7 +118,7 @@ def _generate_all(g, n_seqs, T):
     return toks, recs
 
 
-@pytest.mark.parametrize("key,T", [("c3", 24), ("c4", 16), ("c5", 12)])
+@pytest.mark.parametrize("key,T", [("c3", 24), ("c4", 16), ("c5", 48)])
 def test_fullsize_dex_equals_ar_counts_and_gemm(P, key, T):
     import dex_synth
     wl = dex_synth.workload(key)
@@ -207,6 +207,25 @@ def test_c2_dex_short_run_against_fp32_oracle(P, c2, with_ad):
     g.close()
     res = compare_with_oracle(recs, om, p, wl.depths, T)
     assert res["rounds"] == len(recs) >= len(wl.depths) + 1 and res["nodes"] >= 16
+
+
+@pytest.mark.parametrize("rk", [1, 0])
+def test_c2_single_plane_dex_equals_ar(P, c2, rk):
+    """H3 with act_planes = 1 (activations enter the MMAs as plain bf16): rounding to bf16 amplifies ANY difference
+    between the arithmetic of a DEX round and of the AR pass into token flips, so this run is the sharpest detector of
+    a non-identical code path (it found one in round 2: the first norm of a stage was reduced in another order by
+    k_gather_norm than by the previous layer's add+norm unit).  200 tokens at the bench context."""
+    import dex_synth
+    wl, w = c2
+    p = dex_synth.make_prompt(wl.shape.vocab, wl.prompt_len, wl.prompt_seed)
+    T = 200
+    out = {}
+    for name, X in (("ar", (wl.shape.n_layers,)), ("dex", wl.depths)):
+        d = P.Dex(wl.shape, w, X, max_ctx=wl.prompt_len + T + 8, act_planes=1, round_kernel=rk)
+        d.prefill(0, p)
+        out[name], _ = d.generate(T)
+        d.close()
+    assert np.array_equal(out["dex"], out["ar"])
 
 
 def test_c2_sampling_dex_equals_ar(P, c2):
