@@ -61,7 +61,10 @@ typedef struct dex_config {
   int32_t debug_taps;    /* 1: keep per-layer hidden rows / anchor logits for dex_debug_read */
   int32_t act_planes;    /* 1: activations enter the MMAs as bf16; 2: as bf16 hi+lo pair  */
   int32_t use_graph;     /* 1: replay the step as a CUDA graph                            */
-  int32_t round_kernel;  /* 1: one persistent kernel per round (k_round); 0: one launch per op */
+  int32_t round_kernel;  /* 1: one persistent kernel per round (k_round: phases separated by grid barriers; the
+                            measured path); 0: one launch per op; 2: k_flow, the round as a barrier-free dataflow
+                            program (experimental: bit-identical results, slower; falls back to k_round for shapes
+                            its tables do not cover) */
   int32_t sample;        /* 0: greedy (Alg. 2 line 9); 1: sampling-mode DECS (Alg. 2 lines 10-15):
                             y = argmax_v (l_v / temperature + G_v) with a Gumbel(0,1) row shared by every depth of a
                             slot chain, drawn by a counter-based generator from (sample_seed, sequence, absolute

@@ -20,6 +20,10 @@ Parity pins (tests/test_oracle_*.py, all ``-m "not gpu"``):
   dex.py     Alg. 1, 2     node hidden == from-scratch forward of its own prefix;
                            losslessness; y == final-depth argmax
                            (PAPER.md:204); closed-form round / layer-eval counts
+  ar.py      prefill_matrix  whole-sequence causal form == the position-wise prefill (K/V, continued decode)
+  dex.py     force_u hook  forcing the oracle's own decisions changes nothing; a forced decision records the logit gap
+  model.py   adapter_delta a torch.nn module assembled from the paper's description, parameter count
+                           4h^2+4h+1; fails when b2 leaves the gate, sigma != SiLU, the RMSNorm is dropped
   gumbel.py  Alg. 2 l.10-15  Gumbel-Max frequencies == softmax(l/tau) (chi-square), moments of the rows,
                            sampled DEX stream == sampled AR stream for every X
 Nothing is "parity unpinned".

@@ -187,13 +187,14 @@ struct Layout {
   OpCfg op[7];
   size_t part_floats;
   size_t part_off[4];
+  int item_cap;
   size_t off[40];
   size_t total;
   size_t dbg_floats;
 };
 enum Buf {
   B_SEQS, B_TOKENS, B_B, B_PT, B_ROWS, B_GNB, B_ENB, B_KEY, B_REFT, B_CMD, B_SS, B_ACNT, B_KPOOL, B_VPOOL, B_KSLOT, B_VSLOT,
-  B_XCUR, B_XFRONT, B_ACTA, B_ACTO, B_ACTF, B_ACTE, B_PART, B_QBUF, B_APART, B_ROPE, B_TAPH, B_DBG, B_GBAR, B_TAPT, B_FCTR, B_FTAB, B_COUNT
+  B_XCUR, B_XFRONT, B_ACTA, B_ACTO, B_ACTF, B_ACTE, B_PART, B_QBUF, B_APART, B_ROPE, B_TAPH, B_DBG, B_GBAR, B_TAPT, B_FCTR, B_FTAB, B_ITEMS, B_COUNT
 };
 
 void make_layout(const dex_config& c, const int32_t* depths, int n, Layout& L) {
@@ -300,6 +301,15 @@ void make_layout(const dex_config& c, const int32_t* depths, int n, Layout& L) {
   sz[B_DBG] = sizeof(float) * L.dbg_floats;
   sz[B_GBAR] = 256;
   sz[B_TAPT] = c.debug_taps ? sizeof(unsigned long long) * (20 * (size_t)L.max_len + 68) : 0;
+  {   // k_flow item records: all items of a round / 128 CTAs (the launch needs >= 128 SMs) + one per op + slack
+    size_t items = 0;
+    for (int i = 0; i < 4; ++i) items += (size_t)L.op[i].dec.n_tiles * L.op[i].dec.ksplit;
+    items *= (size_t)n * L.max_len;
+    if (c.adapter_dim > 0) items += (size_t)(n - 1) * ((size_t)L.op[5].dec.n_tiles * L.op[5].dec.ksplit + (size_t)L.op[6].dec.n_tiles * L.op[6].dec.ksplit);
+    items += (size_t)L.ext.n_grp * L.op[4].dec.n_tiles;
+    L.item_cap = (int)(items / 128 + 4 * L.max_len * n + 3 + 16);   // + one per (op, stage) for the round-robin remainders
+  }
+  sz[B_ITEMS] = (size_t)32 * L.item_cap * 160;              // up to 160 CTAs
   sz[B_FCTR] = sizeof(int) * kFcTotal;
   sz[B_FTAB] = sizeof(int) * kFtTotal;
   size_t off = 0;
@@ -670,6 +680,8 @@ int32_t dex_init(dex_ctx** out, const dex_config* cfg, const dex_weights* w, con
   D.rope = WSP(float2, B_ROPE); D.tap_hidden = cfg->debug_taps ? WSP(float, B_TAPH) : nullptr;
   D.gbar = WSP(unsigned int, B_GBAR);
   D.flow_ctr = WSP(int, B_FCTR);
+  D.item_recs = WSP(void, B_ITEMS);
+  D.item_cap = L.item_cap;
   c->flow_tab = WSP(int, B_FTAB);
   for (int i = 0; i < 4; ++i) c->part_off[i] = L.part_off[i];
   D.tap_times = cfg->debug_taps ? WSP(unsigned long long, B_TAPT) : nullptr;
@@ -689,7 +701,7 @@ int32_t dex_init(dex_ctx** out, const dex_config* cfg, const dex_weights* w, con
     const size_t stage = 16384 + (size_t)cfg->act_planes * c->round_ring.x_cap * 128;
     const size_t attn = (round_attn_smem(cfg->head_dim) + 1023) / 1024 * 1024;
     const size_t budget = 219 * 1024 - attn - 2048;
-    c->round_ok = budget / stage >= 3 && c->round_ring.n_acc == 2;   // too few ring stages (very wide stages): per-op path
+    c->round_ok = budget / stage >= 3 && c->round_ring.n_acc == 2;   // too few ring stages (very wide stages): per-op path   // too few ring stages (very wide stages): per-op path
     if ((cfg->sample || c->has_ad) && !c->round_ok) {
       delete c;
       return fail(nullptr, DEX_ECAPACITY, "sampling mode / inducing adapters need the round kernel, whose ring does not fit this stage width");
@@ -753,6 +765,7 @@ int32_t dex_init(dex_ctx** out, const dex_config* cfg, const dex_weights* w, con
     c->flow_ok = (D.nh * hd) % kTileM == 0 && (D.nkv * hd) % kTileM == 0 && n_t <= kFlowTiles &&
                  2 * ((D.ffn + kTileM - 1) / kTileM) <= kFlowTiles && (D.d + kTileM - 1) / kTileM <= kFlowTiles && D.nkv <= kFlowSlices;
     for (int i = 0; i < 4; ++i) c->flow_ok = c->flow_ok && c->op[i].dec.ksplit <= kFlowSlices;
+    c->flow_ok = c->flow_ok && 4 * L.max_len * n_depths + 3 <= 400 && c->n_sms >= 128 && c->n_sms <= 160;   // item records, op table
     std::vector<int> tab(kFtTotal, 0);
     if (c->flow_ok) {
       auto grp_of = [&](int hh) { return hh < D.nh ? hh / Gq : (hh < D.nh + D.nkv ? hh - D.nh : hh - D.nh - D.nkv); };

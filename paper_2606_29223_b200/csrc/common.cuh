@@ -111,6 +111,8 @@ struct Dev {
   __nv_bfloat16 *act_a, *act_o, *act_f, *act_e;   // [planes][R_cap][K] MMA operands
   float* part;             // split-K partial sums, per op [S_op][R_cap][ld_op] (OpDesc)
   unsigned int* gbar;      // grid-barrier arrival counter of the round kernel (reset every round)
+  void* item_recs;         // [grid][item_cap] 32-byte item records of k_flow (written by each CTA in its prologue)
+  int item_cap;
   int* flow_ctr;           // [kFcTotal] arrival counters / ready flags of the dataflow round kernel (k_flow), zeroed every round
   float* qbuf;             // [R_cap][nh*hd]
   float* attn_part;        // [R_cap][nh][4 * max_chunks][hd + 2]: (o, max, sum) per 16 positions (k_round) / per chunk (k_attn)

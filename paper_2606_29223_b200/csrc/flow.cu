@@ -104,18 +104,19 @@ struct FSeq {
   const int* s_nb;         // [16]
   const short* s_perm;     // QKV tile order
   int n_steps, n_ops, n_ad_ops, G, cta, gu_half;   // gu_half = ceil(ffn / 128)
+  const struct FRec* recs;   // this CTA's decoded items and their count (prologue of k_flow)
+  int n_my;
+  const int* mops;           // layer micro-ops in schedule order: (step j) << 8 | (kind) << 4 | stage
+  int n_layer;               // their count
 
-  __device__ __forceinline__ int which_of(int t) const {
-    return t < 4 * n_steps ? (t & 3) : (t < 4 * n_steps + n_ad_ops ? 5 + t - 4 * n_steps : 4);
-  }
   __device__ __forceinline__ void op_info(int t, FOp& o) const {
     unsigned mask = 0;
-    if (t < 4 * n_steps) {
-      o.j = t >> 2; o.which = t & 3; o.ext = 0;
-      for (int g = 0; g < a->dec.n_grp; ++g)
-        if (s_nb[g] > 0 && o.j < a->dec.layer_len[g]) mask |= 1u << g;
-    } else if (t < 4 * n_steps + n_ad_ops) {
-      o.j = 0; o.which = 5 + t - 4 * n_steps; o.ext = 0;
+    if (t < n_layer) {                                     // one projection of ONE stage at one layer-step
+      const int e = mops[t];
+      o.j = e >> 8; o.which = (e >> 4) & 15; o.ext = 0;
+      mask = 1u << (e & 15);
+    } else if (t < n_layer + n_ad_ops) {
+      o.j = 0; o.which = 5 + t - n_layer; o.ext = 0;
       for (int g = 0; g + 1 < a->dec.n_grp; ++g)
         if (s_nb[g] > 0) mask |= 1u << g;
     } else {
@@ -125,7 +126,7 @@ struct FSeq {
     }
     o.mask = mask;
     const OpDesc& d = a->op[o.which];
-    o.n_tiles = (t < 4 * n_steps && o.which == 2) ? 2 * gu_half : d.n_tiles;
+    o.n_tiles = (t < n_layer && o.which == 2) ? 2 * gu_half : d.n_tiles;
     o.ksplit = d.ksplit; o.kbps = d.kbps; o.kb_total = d.kb_total;
     o.per_grp = o.n_tiles * d.ksplit;
     o.n_items = __popc(mask) * o.per_grp;
@@ -200,6 +201,64 @@ struct FWalker {           // this CTA's items, in order (dealt round-robin, con
   __device__ __forceinline__ void next(const FSeq& q) {
     i += q.G;
     settle(q);
+  }
+};
+
+// Precomputed item records: the CTA decodes its items ONCE in the prologue (all threads in parallel) into 32-byte records
+// in global memory and the roles read them (two 16-byte loads per item, the next record requested one item ahead)
+// instead of each walking the list themselves (op_info / decode: integer divisions, ~300 instructions per item, inlined
+// into six warp roles).  ncu's source page put most of k_flow's instruction-fetch stalls in those walkers; with the
+// records c2 went from 172 to 227 tokens/s.  (k_round gains nothing from it: its glue warps sleep while the GEMM phases
+// stream, and the prologue costs as much as the walkers.)
+constexpr int kMaxOps = 400;            // ops of a round
+struct __align__(16) FRec {
+  int c1, col0;
+  short c2, t, kb0, kb1, nb, row0, row_end, cnt_idx;
+  unsigned char g, split, which, cnt_target;
+  int j;
+};
+static_assert(sizeof(FRec) == 32, "FRec is 32 bytes");
+
+struct FRecWalker {        // same interface as FWalker
+  const FRec* recs;
+  int k, n, t, i;
+  bool valid;
+  struct { int which, j; } o;
+  FItem it;
+  uint4 na, nb_;
+  int ffn, n_layer_ops;
+  const RoundArgs* a;
+  __device__ __forceinline__ void fetch(int idx) {
+    if (idx < n) {
+      const uint4* p = reinterpret_cast<const uint4*>(recs + idx);
+      na = p[0];
+      nb_ = p[1];
+    }
+  }
+  __device__ __forceinline__ void take() {
+    valid = k < n;
+    i = k;
+    if (!valid) return;
+    it.c1 = (int)na.x; it.col0 = (int)na.y;
+    it.c2 = (short)(na.z & 0xffffu); t = (short)(na.z >> 16);
+    it.kb0 = (short)(na.w & 0xffffu); it.kb1 = (short)(na.w >> 16);
+    it.nb = (short)(nb_.x & 0xffffu); it.row0 = (short)(nb_.x >> 16);
+    it.row_end = (short)(nb_.y & 0xffffu); it.cnt_idx = (short)(nb_.y >> 16);
+    it.g = (int)(nb_.z & 0xffu); it.split = (int)((nb_.z >> 8) & 0xffu);
+    o.which = (int)((nb_.z >> 16) & 0xffu); it.cnt_target = (int)(nb_.z >> 24);
+    o.j = (int)nb_.w;
+    it.tile = it.col0 / kTileM;
+    it.col_end = (t < n_layer_ops && o.which == 2) ? (it.col0 >= ffn ? 2 * ffn : ffn) : a->op[o.which].out_dim;
+    fetch(k + 1);
+  }
+  __device__ __forceinline__ void start(const FSeq& q) {
+    recs = q.recs; n = q.n_my; k = 0; a = q.a; ffn = q.a->D.ffn; n_layer_ops = q.n_layer;
+    fetch(0);
+    take();
+  }
+  __device__ __forceinline__ void next(const FSeq&) {
+    ++k;
+    take();
   }
 };
 
@@ -283,15 +342,18 @@ __global__ void __launch_bounds__(kFlowThreads, 1) k_flow(const __grid_constant_
     s_edone[0] = s_edone[1] = s_edone[2] = s_edone[3] = 0;
     s_qhead = s_qtail = 0;
     s_cdone = 0;
+    // Attention families that are live AT THE SAME TIME: here the stages' attention work is spread in time (a stage's
+    // heads become ready as its QKV tiles are finalized, stage after stage), so the chunk ranges are sized as if ONE
+    // stage were live - the last stage's tasks are what the O projection waits for, and they find the grid idle.
     int lm = 0;
-    for (int s = 0; s < D.max_seqs; ++s) {                   // live (stage, sequence[, 16-pair pass]) attention families
-      const SeqState st = D.seqs[s];
-      if (!r_seq_live(st)) continue;
-      if constexpr (PT) {
-        for (int m = 0; m <= min(st.q, D.N - 1); ++m) lm += (r_stage_count(st.q, m) * (D.nh / D.nkv) + 15) / 16;
-      } else {
-        lm += min(st.q, D.N - 1) + 1;
+    for (int m = 0; m < D.N; ++m) {
+      int lm_m = 0;
+      for (int s = 0; s < D.max_seqs; ++s) {
+        const SeqState st = D.seqs[s];
+        if (!r_seq_live(st) || st.q < m) continue;
+        lm_m += PT ? (r_stage_count(st.q, m) * (D.nh / D.nkv) + 15) / 16 : 1;
       }
+      lm = max(lm, lm_m);
     }
     s_live_ms = lm;
     s_cum[0] = 0;
@@ -322,28 +384,96 @@ __global__ void __launch_bounds__(kFlowThreads, 1) k_flow(const __grid_constant_
 
   FSeq sq;
   sq.a = &a; sq.s_nb = s_nb; sq.s_perm = s_perm; sq.n_steps = s_steps; sq.n_ad_ops = (D.ad_m > 0 && D.N >= 2) ? 2 : 0;
-  sq.n_ops = 4 * s_steps + sq.n_ad_ops + 1; sq.G = gridDim.x; sq.cta = blockIdx.x; sq.gu_half = (D.ffn + 127) / 128;
+  sq.G = gridDim.x; sq.cta = blockIdx.x; sq.gu_half = (D.ffn + 127) / 128;
   const unsigned G = gridDim.x;
   int* const ctr = D.flow_ctr;
-  const int n_layer_ops = 4 * s_steps;
+  // ---- the layer micro-ops (one projection of one live stage at one layer-step) in SKEWED order: micro-op (j, kind k,
+  // live-stage rank m) has key (4j + k) n + 2m (n = live stages), ties to the lower stage.  Every stage's own chain
+  // QKV -> O -> gate/up -> down -> next QKV stays in order, and between two dependent micro-ops of a stage lie n - 1
+  // micro-ops of the others: their streams cover its attention tasks and last-arriver finalizations (with the plain
+  // stage-major order the O projection of the LAST stage followed its QKV projection by three short ops and waited tens
+  // of microseconds for its attention).
+  __shared__ int s_n_layer;
+  int* const mops = reinterpret_cast<int*>(smem + a.attn_smem_off);    // prologue scratch: the attention buffers
+  int* const opn = mops + kMaxOps;
+  unsigned char* const opi0 = reinterpret_cast<unsigned char*>(opn + kMaxOps + 1);
+  if (threadIdx.x == 0) {
+    int live[kMaxGrp], n = 0, cnt = 0;
+    for (int g = 0; g < a.dec.n_grp; ++g)
+      if (s_nb[g] > 0) live[n++] = g;
+    if (n > 0) {
+      const int key_end = 4 * n * s_steps + 2 * n;
+      for (int key = 0; key < key_end; ++key)
+        for (int m = 0; m < n; ++m) {
+          const int rem = key - 2 * m;
+          if (rem < 0 || rem % n) continue;
+          const int jk = rem / n, j = jk >> 2, k = jk & 3;
+          if (j < a.dec.layer_len[live[m]] && cnt < kMaxOps - 3) mops[cnt++] = (j << 8) | (k << 4) | live[m];
+        }
+    }
+    s_n_layer = cnt;
+  }
+  __syncthreads();
+  sq.mops = mops; sq.n_layer = s_n_layer;
+  sq.n_ops = sq.n_layer + sq.n_ad_ops + 1;
+  const int n_layer_ops = sq.n_layer;
+
+  // ---- decode this CTA's items once (items are dealt round-robin, continuing across ops)
+  sq.recs = reinterpret_cast<const FRec*>(D.item_recs) + (size_t)blockIdx.x * D.item_cap;
+  sq.n_my = 0;
+  if (s_steps > 0) {
+    FRec* my = reinterpret_cast<FRec*>(D.item_recs) + (size_t)blockIdx.x * D.item_cap;
+    for (int t = threadIdx.x; t < sq.n_ops; t += blockDim.x) {
+      FOp o;
+      sq.op_info(t, o);
+      opn[t] = o.n_items;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      int rr = 0, start = 0;
+      for (int t = 0; t < sq.n_ops; ++t) {
+        const int n = opn[t], i0 = (sq.cta + sq.G - rr) % sq.G;
+        opi0[t] = (unsigned char)i0;
+        opn[t] = start;
+        start += n > i0 ? (n - i0 + sq.G - 1) / sq.G : 0;
+        rr = (rr + n) % sq.G;
+      }
+      opn[sq.n_ops] = start;
+      if (start > D.item_cap || sq.n_ops > kMaxOps) __trap();
+    }
+    __syncthreads();
+    sq.n_my = opn[sq.n_ops];
+    for (int k = threadIdx.x; k < sq.n_my; k += blockDim.x) {
+      int lo = 0, hi = sq.n_ops;
+      while (hi - lo > 1) {
+        const int mid = (lo + hi) >> 1;
+        if (opn[mid] <= k) lo = mid; else hi = mid;
+      }
+      FOp o;
+      FItem it;
+      sq.op_info(lo, o);
+      sq.decode(o, (int)opi0[lo] + (k - opn[lo]) * sq.G, it);
+      FRec r;
+      r.c1 = it.c1; r.col0 = it.col0; r.c2 = (short)it.c2; r.t = (short)lo; r.kb0 = (short)it.kb0; r.kb1 = (short)it.kb1;
+      r.nb = (short)it.nb; r.row0 = (short)it.row0; r.row_end = (short)it.row_end; r.cnt_idx = (short)it.cnt_idx;
+      r.g = (unsigned char)it.g; r.split = (unsigned char)it.split; r.which = (unsigned char)o.which;
+      r.cnt_target = (unsigned char)it.cnt_target; r.j = o.j;
+      my[k] = r;
+    }
+    __syncthreads();
+  }
 
   if (s_steps > 0) {
     if (warp == 0) {
       // ===================== weight producer: always as far ahead as the ring allows =====================
-      FWalker w;
+      FRecWalker w;
       unsigned st = 0, ph = 0;
       bool wrapped = false;
-      long long t_wait = 0;
-      const bool prof = D.taps && blockIdx.x == 0;
       for (w.start(sq); w.valid; w.next(sq)) {
         const CUtensorMap* desc = (w.t < n_layer_ops && w.o.which == 2) ? &tm.wgu2 : &tm.w[w.o.which];
         const uint32_t tx = kABytes + D.planes * w.it.nb * 128;
         for (int kb = w.it.kb0; kb < w.it.kb1; ++kb) {
-          if (wrapped) {
-            const long long t0 = prof ? clock64() : 0;
-            mbar_wait(&empty[st], ph ^ 1u);
-            if (prof) t_wait += clock64() - t0;
-          }
+          if (wrapped) mbar_wait(&empty[st], ph ^ 1u);
           if (elect_one()) {
             mbar_expect_tx(&full[st], tx);
             tma_load_3d(smem + (size_t)st * stage_bytes, desc, &full[st], kb * kTileK, w.it.c1, w.it.c2, kEvictFirst);
@@ -352,7 +482,6 @@ __global__ void __launch_bounds__(kFlowThreads, 1) k_flow(const __grid_constant_
           if (++st == (unsigned)NS) { st = 0; ph ^= 1u; wrapped = true; }
         }
       }
-      if (prof && lane == 0) D.tap_times[20 * D.max_len + 60] = (unsigned long long)t_wait;   // W: waiting for a free ring slot
     } else if (warp == 6) {
       // ===================== activation producer: waits for the K slice of its item =====================
       // The counter of item i + 1 is requested (relaxed load) before the boxes of item i are issued and consumed after
@@ -360,12 +489,12 @@ __global__ void __launch_bounds__(kFlowThreads, 1) k_flow(const __grid_constant_
       // relaxed: what depends on it are async-proxy (TMA) reads issued after fence.proxy.async, of data the finalizer
       // released at gpu scope before it bumped the counter; a gpu-scope acquire fence here stalls on the SM's
       // in-flight TMA traffic (measured: every fence.acq_rel.gpu costs microseconds of stream).
-      FWalker w, wn;
+      FRecWalker w, wn;
       unsigned st = 0, ph = 0;
       bool wrapped = false;
       unsigned seen = 0;
       const int sl_x = a.op[0].kbps * kTileK, sl_o = a.op[1].kbps * kTileK, sl_f = a.op[3].kbps * kTileK;
-      auto dep_of = [&](const FWalker& x, const int*& flag, int& target) {
+      auto dep_of = [&](const FRecWalker& x, const int*& flag, int& target) {
         flag = nullptr; target = 0;
         if (!x.valid || x.t >= n_layer_ops) return;
         const int which = x.o.which, m = x.it.g, s = x.it.split, j = x.o.j;
@@ -384,8 +513,6 @@ __global__ void __launch_bounds__(kFlowThreads, 1) k_flow(const __grid_constant_
           target = (j + 1) * tiles_in_slice(D.ffn, sl_f, s);
         }
       };
-      long long t_flag = 0, t_slot = 0;
-      const bool prof = D.taps && blockIdx.x == 0;
       w.start(sq);
       const int* f_cur;
       int t_cur, v_cur = 0;
@@ -396,13 +523,11 @@ __global__ void __launch_bounds__(kFlowThreads, 1) k_flow(const __grid_constant_
         if (w.t < n_layer_ops) {
           if (t_cur > 0) {
             unsigned spins = 0;
-            const long long t0 = prof ? clock64() : 0;
             while (v_cur < t_cur) {
               __nanosleep(20);
               v_cur = ld_relaxed_s32(f_cur);
               if (++spins > 20000000u) flow_die(D, 1, which, (w.it.g << 16) | w.it.split, w.o.j, t_cur);
             }
-            if (prof) t_flag += clock64() - t0;
             fence_proxy_async();
           }
         } else {
@@ -428,11 +553,7 @@ __global__ void __launch_bounds__(kFlowThreads, 1) k_flow(const __grid_constant_
         const CUtensorMap* desc = &tm.x[(which == 0 || which == 2 || which == 5) ? 0 : (which == 1 ? 1 : (which == 4 ? 3 : 2))];
         const int row0 = w.it.row0, nb = w.it.nb;
         for (int kb = w.it.kb0; kb < w.it.kb1; ++kb) {
-          if (wrapped) {
-            const long long t0 = prof ? clock64() : 0;
-            mbar_wait(&empty[st], ph ^ 1u);
-            if (prof) t_slot += clock64() - t0;
-          }
+          if (wrapped) mbar_wait(&empty[st], ph ^ 1u);
           if (elect_one()) {
             uint8_t* sB = smem + (size_t)st * stage_bytes + kABytes;
             if (a.stacked) {
@@ -449,53 +570,32 @@ __global__ void __launch_bounds__(kFlowThreads, 1) k_flow(const __grid_constant_
         }
         w = wn; f_cur = f_n; t_cur = t_n; v_cur = v_n;
       }
-      if (prof && lane == 0) {
-        D.tap_times[20 * D.max_len + 61] = (unsigned long long)t_flag;   // A: waiting for a ready counter
-        D.tap_times[20 * D.max_len + 62] = (unsigned long long)t_slot;   // A: waiting for a free ring slot
-      }
     } else if (warp == 1) {
       // ===================== MMA issuer =====================
-      FWalker w;
+      FRecWalker w;
       unsigned st = 0, ph = 0;
       int n_it = 0;
       const bool stacked = a.stacked != 0;
-      long long t_acc = 0, t_full = 0, t_issue = 0;
-      const bool prof = D.taps && blockIdx.x == 0;
       for (w.start(sq); w.valid; w.next(sq), ++n_it) {
         const int as = n_it & 1;
-        {
-          const long long t0 = prof ? clock64() : 0;
-          mbar_wait(&tempty[as], ((n_it >> 1) & 1) ^ 1);
-          if (prof) t_acc += clock64() - t0;
-        }
+        mbar_wait(&tempty[as], ((n_it >> 1) & 1) ^ 1);
         tc_fence_after();
         const uint32_t d_tmem = tmem_base + as * a.acc_cols;
         const uint32_t idesc = make_idesc_bf16_m128(stacked ? 2 * w.it.nb : w.it.nb);
         uint32_t acc = 0;
         for (int kb = w.it.kb0; kb < w.it.kb1; ++kb) {
-          {
-            const long long t0 = prof ? clock64() : 0;
-            mbar_wait(&full[st], ph);
-            if (prof) t_full += clock64() - t0;
-          }
+          mbar_wait(&full[st], ph);
           tc_fence_after();
-          const long long t1 = prof ? clock64() : 0;
           if (elect_one()) {
             mma_stage(smem_u32(smem + (size_t)st * stage_bytes), plane_bytes, D.planes, stacked, d_tmem, lo_off, idesc, acc);
             umma_commit(&empty[st]);
           }
           __syncwarp();
-          if (prof) t_issue += clock64() - t1;
           acc = 1;
           if (++st == (unsigned)NS) { st = 0; ph ^= 1u; }
         }
         if (elect_one()) umma_commit(&tfull[as]);
         __syncwarp();
-      }
-      if (prof && lane == 0) {
-        D.tap_times[20 * D.max_len + 65] = (unsigned long long)t_issue;  // M: issuing the MMAs of a stage
-        D.tap_times[20 * D.max_len + 63] = (unsigned long long)t_acc;    // M: waiting for a free accumulator stage
-        D.tap_times[20 * D.max_len + 64] = (unsigned long long)t_full;   // M: waiting for weights + operand of a ring stage
       }
     } else if (warp >= 2 && warp <= 5) {
       // ===================== epilogue: TMEM -> partials of the op's own region / exit arg-max =====================
@@ -503,7 +603,7 @@ __global__ void __launch_bounds__(kFlowThreads, 1) k_flow(const __grid_constant_
       EpiCtx ec;
       ec.rows = D.rows; ec.s_valid = s_valid; ec.vocab = D.vocab; ec.best_key = D.best_key;
       ec.ref_tile = D.ref_tile; ec.ref_tiles = D.ref_tiles; ec.dev = &D;
-      FWalker w;
+      FRecWalker w;
       int n_it = 0;
       for (w.start(sq); w.valid; w.next(sq), ++n_it) {
         const int which = w.o.which;
@@ -528,7 +628,7 @@ __global__ void __launch_bounds__(kFlowThreads, 1) k_flow(const __grid_constant_
       // Every finished item of this CTA (all four epilogue warps have written its partials) is counted into its out
       // tile's counter; the arrival that completes the tile queues it for the finalizer group.  Lane l of a batch
       // handles item n_counted + l: the atomics of a batch are in flight together.
-      FWalker wf;
+      FRecWalker wf;
       wf.start(sq);
       unsigned n_counted = 0, head = 0;
       int n_stamp = 0;
@@ -570,7 +670,53 @@ __global__ void __launch_bounds__(kFlowThreads, 1) k_flow(const __grid_constant_
         // also costs the TMA units their cached descriptors) is paid only by an arrival that completes a tile.
         if (lane < taken) last = atom_acq_rel_add_s32(cnt, 1) + 1 == target;
         const unsigned bal = __ballot_sync(0xffffffffu, last);
-        if (bal) {
+        const unsigned bal_all = bal;
+        const unsigned bal_own = PT ? 0u : __ballot_sync(0xffffffffu, last && mine.row_hi - mine.row0 <= 16 && s_nvalid[mine.m] <= 1);
+        const unsigned bal_q = bal_all & ~bal_own;
+        if (bal_own) {
+          // Narrow lattices (a stage has a few rows): this warp finalizes the tiles its arrivals completed right away -
+          // the finalizer group may be inside an attention task for tens of microseconds, and every finalization sits on
+          // the dependency chain of the next op.  Warp unit = (row, 128 columns), the bodies of round_dev.cuh.
+          const int sl_x = a.op[0].kbps * kTileK, sl_f = a.op[3].kbps * kTileK;
+          for (unsigned rest = bal_own; rest; rest &= rest - 1) {
+            const int b = __ffs(rest) - 1;
+            const int which = __shfl_sync(0xffffffffu, mine.which, b), m = __shfl_sync(0xffffffffu, mine.m, b);
+            const int idx = __shfl_sync(0xffffffffu, mine.idx, b), j = __shfl_sync(0xffffffffu, mine.j, b);
+            const int row0 = __shfl_sync(0xffffffffu, mine.row0, b), row_hi = __shfl_sync(0xffffffffu, mine.row_hi, b);
+            const float* part = D.part + a.part_off[which];
+            if (which == 0) {
+              const int hpt = kTileM / D.hd, h0 = idx * hpt;
+              for (int u = 0; u < (row_hi - row0) * hpt; ++u) {
+                const int r = row0 + u / hpt, hh = h0 + u % hpt;
+                if (!((s_valid[r >> 5] >> (r & 31)) & 1u)) continue;
+                if (D.hd == 128) unit_qkv<128>(a, j, part, r, hh, lane); else unit_qkv<64>(a, j, part, r, hh, lane);
+              }
+            } else {
+              for (int r = row0; r < row_hi; ++r) {
+                if (!((s_valid[r >> 5] >> (r & 31)) & 1u)) continue;
+                if (which == 2) unit_silu(a, j, a.op[2], part, r, idx, lane);
+                else unit_add_norm(a, j, which == 1 ? 0 : 1, a.op[which], part, r, idx, lane);
+              }
+            }
+            fence_proxy_async();                             // operand planes are read by TMA
+            __syncwarp();
+            if (lane == 0) {
+              if (which == 0) {
+                for (int g = s_glo[idx]; g <= s_ghi[idx]; ++g) red_release_add_s32(ctr + kFcQkv + m * kFlowSlices + g, 1);
+              } else if (which == 1) {
+                red_release_add_s32(ctr + kFcXf + m * kFlowSlices + (idx * kTileM) / sl_x, 1);
+              } else if (which == 2) {
+                red_release_add_s32(ctr + kFcF + m * kFlowSlices + (idx * kTileM) / sl_f, 1);
+              } else {
+                red_release_add_s32(ctr + kFcXa + m * kFlowSlices + (idx * kTileM) / sl_x, 1);
+              }
+            }
+            __syncwarp();
+          }
+        }
+        if (bal_q) {
+          const unsigned bal = bal_q;
+          const bool last = (bal >> lane) & 1u;
           const int n_new = __popc(bal);
           unsigned spins = 0;
           while (head + n_new - ld_acquire_cta_shared(&s_qtail) > (unsigned)kFlowQueue) {   // queue space
@@ -602,6 +748,8 @@ __global__ void __launch_bounds__(kFlowThreads, 1) k_flow(const __grid_constant_
       // warp 0 of the group owns the cursors: queue tail, next attention task
       unsigned tail = 0;
       int att_j = 0, att_u = blockIdx.x;
+      AttnTask tk;
+      bool have = false;
       unsigned it_no = 0, idle = 0;
       for (;; ++it_no) {
         FDec* dec = &s_dec[it_no & 1];
@@ -617,16 +765,14 @@ __global__ void __launch_bounds__(kFlowThreads, 1) k_flow(const __grid_constant_
             }
             ++tail;
           } else {
-            // next live attention task of this CTA (dead ones are skipped without waiting)
-            AttnTask tk;
-            bool have = false;
-            while (att_j < sq.n_steps) {
+            // next live attention task of this CTA (dead ones are skipped without waiting); decoded once, then only
+            // its counter is polled
+            while (!have && att_j < sq.n_steps) {
               if (att_u >= pl.n_tasks) { ++att_j; att_u = blockIdx.x; continue; }
               attn_task_of<PT>(a, pl, s_cum, G, att_u, tk);
               const SeqState sst = D.seqs[tk.s];
               if (!r_seq_live(sst) || sst.q < tk.m || att_j >= a.dec.layer_len[tk.m] || s_nb[tk.m] == 0) { att_u += G; continue; }
               have = true;
-              break;
             }
             if (have) {
               int v = 0;
@@ -639,6 +785,7 @@ __global__ void __launch_bounds__(kFlowThreads, 1) k_flow(const __grid_constant_
                 kind = 2;
                 if (lane == 0) { dec->tk = tk; dec->j = att_j; }
                 att_u += G;
+                have = false;
               }
             } else if (cdone) {
               kind = 3;

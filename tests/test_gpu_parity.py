@@ -286,6 +286,30 @@ def test_edges_prompt_len_one_ragged_prefill_pages_and_max_ctx(P, c1, c1_bf16):
     g.close()
 
 
+def test_sequence_prefilled_to_max_ctx_is_done_on_both_sides(P, c1):
+    """a sequence whose prompt already fills max_ctx is done on the device as on the host mirror: it takes no
+    part in the rounds (no rows, no layer evaluations) while the other sequence of the batch decodes its usual stream."""
+    import dex_synth
+    wl, w, p = c1
+    full = dex_synth.make_prompt(wl.shape.vocab, 64, 9)
+    alone = P.Dex(wl.shape, w, wl.depths, max_ctx=64)
+    alone.prefill(0, p)
+    want, _ = alone.generate(20)
+    alone.close()
+    g = P.Dex(wl.shape, w, wl.depths, max_seqs=2, max_ctx=64)
+    g.prefill(0, full)                                       # n == max_ctx: nothing can be generated
+    g.prefill(1, p)
+    got = []
+    while len(got) < 20:
+        res = g.step()
+        assert res[0].active == 0 and res[0].done == 1 and res[0].layer_evals == 0 and res[0].n_tokens == 64
+        if res[1].committed:
+            got.append(res[1].token)
+    assert g.tap_fsm(0).tolist()[2] == 64                    # the device FSM did not move either
+    assert np.array_equal(got, want)
+    g.close()
+
+
 def test_gqa_headdim128_ragged_vocab(P):
     """A small GQA model with head_dim 128, a vocabulary that is not a multiple of the 128-row
     tile and d_ffn with ragged tiles: AR and DEX against the oracle (shape family of c4)."""
