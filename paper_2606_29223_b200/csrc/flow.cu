@@ -743,6 +743,10 @@ __global__ void __launch_bounds__(kFlowThreads, 1) k_flow(const __grid_constant_
       constexpr int GT = kFT;
       AttnPlan pl;
       attn_plan<PT>(a, G, s_live_ms, s_cum, pl);
+      // A CTA runs its attention tasks in order, each waiting for its head's QKV counter: the order must follow the op
+      // order (stage-major within a layer-step).  k_round's heaviest-range-first deal puts tasks of LATER stages first,
+      // and such a task blocks one that an earlier op is waiting for: deadlock on lattices with more tasks than CTAs.
+      pl.lpt = 0;
       const int sl_x = a.op[0].kbps * kTileK, sl_f = a.op[3].kbps * kTileK, sl_o = a.op[1].kbps * kTileK;
       void* const asm_ = smem + a.attn_smem_off;
       // warp 0 of the group owns the cursors: queue tail, next attention task

@@ -672,6 +672,7 @@ __device__ __forceinline__ void attn_tile(const Dev& D, AttnSmem<HD>* sm, uint32
 // How the attention work of one layer-step is cut into tasks (shared by every CTA: same deterministic split).
 struct AttnPlan {
   int tail_own, n_body, CR, n_ranges, Gq, per_ms, fam, n_tasks;
+  int lpt;                 // pass tasks dealt heaviest range first (k_round); k_flow needs stage-major task order
 };
 struct AttnTask {
   int m, s, g, rg, pb_task;
@@ -697,13 +698,14 @@ __device__ __forceinline__ void attn_plan(const RoundArgs& a, int G, int n_live_
   p.per_ms = D.nkv * p.n_ranges;
   p.fam = PT ? cum[D.N] * D.nkv : 0;                         // cum[m]: (sequence, pass) slots of the stages before m (shared memory)
   p.n_tasks = PT ? p.fam * p.n_ranges : D.N * D.max_seqs * p.per_ms;
+  p.lpt = PT && p.n_tasks > G;                             // one wave: range fastest, as without pass tasks
 }
 template <bool PT>
 __device__ __forceinline__ void attn_task_of(const RoundArgs& a, const AttnPlan& p, const int* cum, int G, int u, AttnTask& t) {
   const Dev& D = a.D;
   t.pb_task = 0;
   if constexpr (PT) {
-    const bool lpt = p.n_tasks > G;                          // one wave: range fastest, as without pass tasks
+    const bool lpt = p.lpt != 0;
     t.rg = lpt ? p.n_ranges - 1 - u / p.fam : u % p.n_ranges;
     const int rem = lpt ? u % p.fam : u / p.n_ranges;
     const int psi = rem / D.nkv;

@@ -228,6 +228,25 @@ def test_c2_single_plane_dex_equals_ar(P, c2, rk):
     assert np.array_equal(out["dex"], out["ar"])
 
 
+def test_c3_flow_kernel_equals_round_kernel(P):
+    """k_flow on the N = 8 lattice of c3 at full size (pass tasks, 128 rows, 512-token context): same stream as k_round."""
+    import dex_synth
+    import torch
+    wl = dex_synth.workload("c3")
+    w = dex_synth.make_weights(wl.shape, wl.weight_seed, threads=16)
+    wd = {k: v.cuda() for k, v in w.items()}
+    p = dex_synth.make_prompt(wl.shape.vocab, wl.prompt_len, wl.prompt_seed)
+    out = {}
+    for rk in (1, 2):
+        g = P.Dex(wl.shape, wd, wl.depths, max_ctx=wl.prompt_len + 32, round_kernel=rk)
+        g.prefill(0, p)
+        out[rk], _ = g.generate(16)
+        g.close()
+    del wd
+    torch.cuda.empty_cache()
+    assert np.array_equal(out[1], out[2])
+
+
 def test_c2_sampling_dex_equals_ar(P, c2):
     """Sampling-mode DECS at the 7B shape: GPU DEX stream == GPU AR stream (same Gumbel rows), differs from greedy."""
     import dex_synth

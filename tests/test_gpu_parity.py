@@ -310,6 +310,24 @@ def test_sequence_prefilled_to_max_ctx_is_done_on_both_sides(P, c1):
     g.close()
 
 
+def test_flow_kernel_more_attention_tasks_than_ctas(P, c1):
+    """k_flow (round_kernel = 2) on a wide lattice with a long context: more attention tasks than CTAs.  Its CTAs run
+    their tasks in order, each waiting for its head's QKV counter, so the tasks must be dealt stage-major; with
+    k_round's heaviest-range-first deal this configuration deadlocked (round 2).  Streams must equal k_round's."""
+    import dex_synth
+    wl, w, _ = c1
+    X = tuple(range(1, 9))
+    p = dex_synth.make_prompt(wl.shape.vocab, 300, 17)
+    out = {}
+    for rk in (1, 2):
+        g = P.Dex(wl.shape, w, X, max_ctx=360, page_size=64, round_kernel=rk)
+        g.prefill(0, p)
+        toks, recs = g.generate(24)
+        out[rk] = (toks.tolist(), [r["match_k"] for r in recs])
+        g.close()
+    assert out[1] == out[2]
+
+
 def test_gqa_headdim128_ragged_vocab(P):
     """A small GQA model with head_dim 128, a vocabulary that is not a multiple of the 128-row
     tile and d_ffn with ragged tiles: AR and DEX against the oracle (shape family of c4)."""
