@@ -220,6 +220,22 @@ int32_t dex_debug_phase_us(dex_ctx* ctx, float* out8);
  * through the per-op kernels (2: phase breakdown even when round_kernel = 1).  on < 0: read only. */
 int32_t dex_profile(dex_ctx* ctx, int32_t on, double* phase_us_acc8, double* counters8);
 
+/* The weight-streaming GEMM of the layer segment (north_star (a); the k_gemm kernel of dex_step's per-op path) through an
+ * entry point that ALLOCATES NOTHING and needs no context - for callers that cannot call cudaMalloc (code under CUDA graph
+ * capture, tight serving loops, harnesses that forbid it):
+ *     y[rows, out] (f32) = x[rows, k] (f32) . W[out, k]^T (bf16),  the same tiles and fixed K split as the context path.
+ * w_dev: device, bf16 [out_dim, k_dim] row-major, 16-byte aligned; x_dev: device f32 [rows, k_dim]; y_dev: device f32
+ * [rows, out_dim] (written); act_planes: 1 (x enters the MMA as bf16) or 2 (bf16 hi + lo pair, reading R23); stream:
+ * cudaStream_t.  The work is enqueued on the stream, not synchronised.  The kernel's scratch (operand planes, row table,
+ * split-K partials) is ONE static device array of 10 MiB + 8 KiB that every GPU loading the library holds until exit.
+ * Limits: rows <= 32, k_dim <= 16384 (a multiple of 8), out_dim <= 262144 and
+ * ceil(k_dim / 512) * round16(rows) * round4(out_dim) <= 2 Mi floats; DEX_ECAPACITY beyond them, DEX_EINVAL for null /
+ * misaligned pointers or bad sizes, DEX_ECUDA if a CUDA call fails (message: dex_last_error(NULL)).  Every call shares the
+ * array: calls on one stream are ordered, calls that OVERLAP on the GPU (several streams or threads) race on it.  Calls
+ * no cudaMalloc / cudaFree or allocating library routine. */
+int32_t dex_gemm_noalloc(const void* w_dev, const float* x_dev, int32_t rows, int32_t out_dim, int32_t k_dim,
+                         int32_t act_planes, float* y_dev, void* cuda_stream);
+
 int32_t dex_destroy(dex_ctx* ctx);
 const char* dex_last_error(const dex_ctx* ctx);   /* ctx may be NULL: last global error */
 

@@ -56,6 +56,7 @@ _SIGNATURES = {
     "dex_debug_gemm": (C.c_int32, [C.c_void_p, C.c_int32, C.c_int32, C.POINTER(C.c_float), C.c_int32, C.POINTER(C.c_float)]),
     "dex_debug_phase_us": (C.c_int32, [C.c_void_p, C.POINTER(C.c_float)]),
     "dex_profile": (C.c_int32, [C.c_void_p, C.c_int32, C.POINTER(C.c_double), C.POINTER(C.c_double)]),
+    "dex_gemm_noalloc": (C.c_int32, [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p]),
     "dex_destroy": (C.c_int32, [C.c_void_p]),
     "dex_last_error": (C.c_char_p, [C.c_void_p]),
 }
@@ -154,6 +155,11 @@ def dex_profile(ctx, on):
     ph, ct = np.zeros(8, dtype=np.float64), np.zeros(8, dtype=np.float64)
     _check(lib().dex_profile(ctx, on, ph.ctypes.data_as(C.POINTER(C.c_double)), ct.ctypes.data_as(C.POINTER(C.c_double))), ctx)
     return ph, ct
+
+
+def dex_gemm_noalloc(w_ptr, x_ptr, rows, out_dim, k_dim, act_planes, y_ptr, stream_ptr):
+    """y = x . W^T through the allocation-free entry point; all pointers are DEVICE addresses (ints)."""
+    _check(lib().dex_gemm_noalloc(w_ptr, x_ptr, rows, out_dim, k_dim, act_planes, y_ptr, stream_ptr))
 
 
 def dex_destroy(ctx):

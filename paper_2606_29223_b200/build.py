@@ -6,7 +6,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libdex_b200.so")
-SOURCES = ["gemm.cu", "round.cu", "flow.cu", "kernels.cu", "api.cu"]
+SOURCES = ["gemm.cu", "round.cu", "flow.cu", "kernels.cu", "api.cu", "noalloc.cu"]
 HEADERS = ["common.cuh", "ptx.cuh", "gemm_dev.cuh", "round_dev.cuh", os.path.join("..", "..", "include", "dex.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "--use_fast_math=false"]

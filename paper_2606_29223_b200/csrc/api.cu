@@ -595,6 +595,11 @@ void collect_phase_times(dex_ctx* c) {
 
 }  // namespace
 
+namespace dexk {
+// for entry points outside this file (noalloc.cu): the string dex_last_error(NULL) returns
+void set_global_error(const char* msg) { g_last_error = msg ? msg : ""; }
+}  // namespace dexk
+
 // =============================================================================================
 extern "C" {
 
