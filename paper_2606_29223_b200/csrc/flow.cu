@@ -22,17 +22,25 @@
 //     of one stage are covered by the other stages' streams: depth-parallel stages hide each other's latency.
 // Only the tail of the round (inducing adapters, exit head) keeps grid barriers.
 //
-//   warp 0      weight producer (TMA, always ahead)         warp 6      activation producer (waits on slice counters)
-//   warp 1      tcgen05.mma issuer, owns TMEM               warps 7-10  finalizer group: finalizes completed tiles,
-//   warps 2-5   epilogue: TMEM -> split-K partials / arg-max            runs attention tasks
-//   warp 11     counter: counts this CTA's finished items into the tile counters (one atomic per item, a batch of up
+//   warp 0      weight producer (TMA, always ahead)         warp 1      activation producer (waits on slice counters)
+//   warp 8      tcgen05.mma issuer, owns TMEM               warps 2, 3, 10, 11  finalizer group: finalizes completed
+//   warps 4-7   epilogue: TMEM -> split-K partials / arg-max            tiles, runs attention tasks
+//   warp 9      counter: counts this CTA's finished items into the tile counters (one atomic per item, a batch of up
 //               to 32 in flight), queues the tiles it completed for the finalizer group
+//   (which warp takes which role follows the SM's four schedulers: see kWarp* below)
 #include "round_dev.cuh"
 
 namespace dexk {
 
 constexpr int kFlowThreads = 384;
-constexpr int kFT = 128;             // finalizer group threads (warps 7-10)
+constexpr int kFT = 128;             // finalizer group threads
+// Warp roles.  Warps are dealt to the SM's four schedulers by warp % 4.  The finalizer warps run attention MMAs and
+// split-K sums WHILE the pipeline streams, so they must not share a scheduler with the single-issuer pipeline warps:
+//   scheduler 0: weight producer (0), epilogue (4), MMA issuer (8)      scheduler 2: finalizer (2), epilogue (6), finalizer (10)
+//   scheduler 1: activation producer (1), epilogue (5), counter (9)     scheduler 3: finalizer (3), epilogue (7), finalizer (11)
+// (epilogue warp w reads TMEM lanes 32 (w % 4) .. +31: one per scheduler in any case).
+constexpr int kWarpW = 0, kWarpA = 1, kWarpM = 8, kWarpC = 9, kWarpE0 = 4;
+__device__ __forceinline__ int flow_fin_index(int warp) { return warp == 2 ? 0 : (warp == 3 ? 1 : (warp == 10 ? 2 : (warp == 11 ? 3 : -1))); }
 
 // ---------------------------------------------------------------- small helpers
 __device__ __forceinline__ int ld_acquire_s32(const int* p) {
@@ -372,7 +380,7 @@ __global__ void __launch_bounds__(kFlowThreads, 1) k_flow(const __grid_constant_
     for (int i = 0; i < 4; ++i) tma_prefetch_desc(&tm.x[i]);
     tma_prefetch_desc(&tm.wgu2);
   }
-  if (warp == 1) {
+  if (warp == kWarpM) {
     tmem_alloc(tmem_slot, 2 * a.acc_cols);
     tmem_relinquish();
   }
@@ -464,7 +472,7 @@ __global__ void __launch_bounds__(kFlowThreads, 1) k_flow(const __grid_constant_
   }
 
   if (s_steps > 0) {
-    if (warp == 0) {
+    if (warp == kWarpW) {
       // ===================== weight producer: always as far ahead as the ring allows =====================
       FRecWalker w;
       unsigned st = 0, ph = 0;
@@ -482,7 +490,7 @@ __global__ void __launch_bounds__(kFlowThreads, 1) k_flow(const __grid_constant_
           if (++st == (unsigned)NS) { st = 0; ph ^= 1u; wrapped = true; }
         }
       }
-    } else if (warp == 6) {
+    } else if (warp == kWarpA) {
       // ===================== activation producer: waits for the K slice of its item =====================
       // The counter of item i + 1 is requested (relaxed load) before the boxes of item i are issued and consumed after
       // them, so its L2 round trip (microseconds under the weight stream) is off the critical path.  The load is
@@ -570,7 +578,7 @@ __global__ void __launch_bounds__(kFlowThreads, 1) k_flow(const __grid_constant_
         }
         w = wn; f_cur = f_n; t_cur = t_n; v_cur = v_n;
       }
-    } else if (warp == 1) {
+    } else if (warp == kWarpM) {
       // ===================== MMA issuer =====================
       FRecWalker w;
       unsigned st = 0, ph = 0;
@@ -597,7 +605,7 @@ __global__ void __launch_bounds__(kFlowThreads, 1) k_flow(const __grid_constant_
         if (elect_one()) umma_commit(&tfull[as]);
         __syncwarp();
       }
-    } else if (warp >= 2 && warp <= 5) {
+    } else if (warp >= kWarpE0 && warp < kWarpE0 + 4) {
       // ===================== epilogue: TMEM -> partials of the op's own region / exit arg-max =====================
       const int quarter = warp & 3;
       EpiCtx ec;
@@ -623,7 +631,7 @@ __global__ void __launch_bounds__(kFlowThreads, 1) k_flow(const __grid_constant_
           red_release_cta_shared_add(&s_edone[quarter], 1u); // this warp's partials of the item are written
         }
       }
-    } else if (warp == 11) {
+    } else if (warp == kWarpC) {
       // ===================== counter warp =====================
       // Every finished item of this CTA (all four epilogue warps have written its partials) is counted into its out
       // tile's counter; the arrival that completes the tile queues it for the finalizer group.  Lane l of a batch
@@ -737,9 +745,9 @@ __global__ void __launch_bounds__(kFlowThreads, 1) k_flow(const __grid_constant_
       __syncwarp();
       if (lane == 0) asm volatile("st.release.cta.shared.u32 [%0], %1;\n" ::"r"(smem_u32(&s_cdone)), "r"(1u) : "memory");
       if (D.taps && blockIdx.x == 0 && lane == 0 && n_stamp < 20 * D.max_len + 60) D.tap_times[n_stamp] = (unsigned long long)clock64();
-    } else if (warp >= 7) {
+    } else if (flow_fin_index(warp) >= 0) {
       // ===================== finalizer group (warps 7-10) =====================
-      const int we = warp - 7, tid_f = we * 32 + lane;
+      const int we = flow_fin_index(warp), tid_f = we * 32 + lane;
       constexpr int GT = kFT;
       AttnPlan pl;
       attn_plan<PT>(a, G, s_live_ms, s_cum, pl);
@@ -874,7 +882,7 @@ __global__ void __launch_bounds__(kFlowThreads, 1) k_flow(const __grid_constant_
 
   tc_fence_before();
   __syncthreads();
-  if (warp == 1) tmem_dealloc(tmem_base, 2 * a.acc_cols);
+  if (warp == kWarpM) tmem_dealloc(tmem_base, 2 * a.acc_cols);
 }
 
 cudaError_t flow_init() {
