@@ -886,9 +886,9 @@ __global__ void __launch_bounds__(kFlowThreads, 1) k_flow(const __grid_constant_
 }
 
 cudaError_t flow_init() {
-  cudaError_t e = cudaFuncSetAttribute(k_flow<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024);
+  cudaError_t e = cudaFuncSetAttribute(k_flow<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 223 * 1024);
   if (e != cudaSuccess) return e;
-  return cudaFuncSetAttribute(k_flow<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024);
+  return cudaFuncSetAttribute(k_flow<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 223 * 1024);
 }
 
 // Cooperative launch: all CTAs must be co-resident (they wait on one another's counters).

@@ -328,6 +328,37 @@ def test_flow_kernel_more_attention_tasks_than_ctas(P, c1):
     assert out[1] == out[2]
 
 
+def test_256_row_single_plane_stages_run_the_round_kernel(P):
+    """The c5 launch geometry (4 sequences x N = 8 -> 256-row stage 0, head_dim 128, act_planes = 1) must fit the round
+    kernel's shared-memory ring: ONE segment-GEMM launch per round in the library's own counters (dex_profile), not the
+    4 |Pi| launches of the per-op fallback - a budget change once made this fall back silently (round 2).  Also
+    DEX == AR on that path."""
+    import dex_synth
+    sh = dex_synth.ModelShape("mini-hd128-8L", 8, 512, 4, 4, 128, 1024, 1000)
+    w = dex_synth.make_weights(sh, 91)
+    X, S = tuple(range(1, 9)), 4
+    prompts = [dex_synth.make_prompt(sh.vocab, 40 + 7 * s, 92, seq=s) for s in range(S)]
+    streams = {}
+    for name, depths in (("dex", X), ("ar", (sh.n_layers,))):
+        g = P.Dex(sh, w, depths, max_seqs=S, max_ctx=128, act_planes=1, page_size=64)
+        for s in range(S):
+            g.prefill(s, prompts[s])
+        g.profile(0)
+        got = [[] for _ in range(S)]
+        rounds = 0
+        while min(len(t) for t in got) < 10:
+            res = g.step()
+            rounds += 1
+            for s in range(S):
+                if res[s].committed and len(got[s]) < 10:
+                    got[s].append(res[s].token)
+        _, ct = g.profile(-1)
+        assert ct[0] == rounds and ct[2] == rounds, (name, ct[:3].tolist(), rounds)   # one k_round launch per round
+        streams[name] = got
+        g.close()
+    assert streams["dex"] == streams["ar"]
+
+
 def test_gqa_headdim128_ragged_vocab(P):
     """A small GQA model with head_dim 128, a vocabulary that is not a multiple of the 128-row
     tile and d_ffn with ragged tiles: AR and DEX against the oracle (shape family of c4)."""
