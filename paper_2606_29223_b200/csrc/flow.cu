@@ -12,14 +12,15 @@
 //     tile b and up tile b are counted together; the weights stay in their [2][ffn][d] layout, the tensor map views
 //     them as [2L][ffn][d]);
 //   * a finished tile bumps the READY counter of the consumer's K slice (an item's K range: 8 K-blocks = 512
-//     columns); the activation producer of a consuming item polls exactly the slice it needs (ld.acquire.gpu), so
-//     consumers start while the producing op is still streaming.  Item orders are chosen for that: QKV by KV head
+//     columns); the activation producer of a consuming item polls exactly the slice it needs (relaxed loads, requested
+//     one item ahead), so consumers start while the producing op is still streaming.  Item orders are chosen for that: QKV by KV head
 //     (q, k, v tiles of a head adjacent) -> attention of the first heads overlaps the rest of the QKV stream; O and
 //     down split-major (early splits need early heads / early gate-up pairs); gate/up pair-major;
 //   * attention tasks wait for the QKV counter of their KV head group, the last merger of a (row, head) bumps the
 //     ready counter of the O operand slice;
-//   * with several live stages (DEX rounds) the ops are stage-major, so the O -> gate/up and down -> QKV dependencies
-//     of one stage are covered by the other stages' streams: depth-parallel stages hide each other's latency.
+//   * with several live stages (DEX rounds) an op is one projection of ONE stage and the ops are SKEWED across stages
+//     (see the micro-op schedule in the kernel), so between two dependent projections of a stage lie the streams of the
+//     other stages: depth-parallel stages hide each other's latency.
 // Only the tail of the round (inducing adapters, exit head) keeps grid barriers.
 //
 //   warp 0      weight producer (TMA, always ahead)         warp 1      activation producer (waits on slice counters)
