@@ -65,6 +65,21 @@ def ncu_traffic_ratio():
     return (dram / alg if alg > 0 else None), os.path.relpath(files[-1], ROOT)
 
 
+def ncu_tensor_pipe(workload):
+    """sm__pipe_tensor_cycles_active of the dominant kernel from the committed ncu capture of this workload (SURVEY 8(d):
+    to be reported where stages are wide); None if no capture exists for it."""
+    import csv
+    try:
+        with open(os.path.join(ROOT, "profiles", "tensor_pipe_r2.csv")) as f:
+            for row in csv.DictReader(f):
+                if row["workload"] == workload:
+                    return {"active_pct": float(row["sm__pipe_tensor_cycles_active_pct"]), "kernel": row["kernel"],
+                            "source": "NOT a counter of this run: " + row["source"]}
+    except Exception:
+        pass
+    return None
+
+
 # ------------------------------------------------------------------------------------------------
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
@@ -325,6 +340,7 @@ def bench_dex(args):
                                        f"committed ncu --set full capture {ratio_src} (c2), x this run's algorithmic bytes "
                                        "per launch") if ratio else None,
                     "lm_head_restream_bytes_per_launch": ct[6] / max(1, k_launches),
+                    "tensor_pipe": ncu_tensor_pipe(wl.key),
                     "launches": int(k_launches), "avg_launch_us": k_us / max(1, k_launches),
                     "algorithmic_bytes_per_launch": k_bytes / max(1, k_launches),
                     "share_of_step": k_us / max(1e-9, ph[7] if ph[7] > 0 else sum(ph[:6])),

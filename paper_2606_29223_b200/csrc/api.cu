@@ -537,13 +537,10 @@ void account_round(dex_ctx* c) {
   double wbytes = 0;
   int gemm_launches = 0;
   for (int j = 0; j < D.max_len; ++j) {
-    bool any = false;
     for (int m = 0; m < D.N; ++m)
       if (live[m] && j < c->dec_plan.layer_len[m]) {
-        any = true;
         for (int i = 0; i < 4; ++i) wbytes += 2.0 * c->op[i].dec.out_dim * c->op[i].dec.k_dim;
       }
-    (void)any;
     gemm_launches += 4;
   }
   if (c->has_ad)   // every live non-final stage streams its adapter once per round

@@ -74,10 +74,10 @@ def test_7b_width_long_context_ar(P, wide7b):
     d.close()
 
 
-@pytest.mark.parametrize("rk", [1, 0])
+@pytest.mark.parametrize("rk", [1, 0, 2])
 def test_7b_width_long_context_dex_trace(P, wide7b, rk):
-    """X = {1,2,3,4} at a 640-token context: every round against the oracle's trace (tests/trace_util.py), both launch
-    paths; then GPU DEX stream == GPU AR stream."""
+    """X = {1,2,3,4} at a 640-token context: every round against the oracle's trace (tests/trace_util.py), all three launch
+    paths (k_round, per-op kernels, k_flow); then GPU DEX stream == GPU AR stream."""
     from trace_util import gpu_trace, compare_with_oracle
     sh, w, p, om, st = wide7b
     X, T = (1, 2, 3, 4), 3
