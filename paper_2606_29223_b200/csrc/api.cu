@@ -194,7 +194,7 @@ struct Layout {
 };
 enum Buf {
   B_SEQS, B_TOKENS, B_B, B_PT, B_ROWS, B_GNB, B_ENB, B_KEY, B_REFT, B_CMD, B_SS, B_ACNT, B_KPOOL, B_VPOOL, B_KSLOT, B_VSLOT,
-  B_XCUR, B_XFRONT, B_ACTA, B_ACTO, B_ACTF, B_ACTE, B_PART, B_QBUF, B_APART, B_ROPE, B_TAPH, B_DBG, B_GBAR, B_TAPT, B_FCTR, B_FTAB, B_ITEMS, B_COUNT
+  B_XCUR, B_XFRONT, B_ACTA, B_ACTO, B_ACTF, B_ACTE, B_PART, B_QBUF, B_APART, B_ROPE, B_TAPH, B_DBG, B_GBAR, B_TAPT, B_FCTR, B_FTAB, B_ITEMS, B_EMAP, B_COUNT
 };
 
 void make_layout(const dex_config& c, const int32_t* depths, int n, Layout& L) {
@@ -310,6 +310,7 @@ void make_layout(const dex_config& c, const int32_t* depths, int n, Layout& L) {
     L.item_cap = (int)(items / 128 + 4 * L.max_len * n + 3 + 16);   // + one per (op, stage) for the round-robin remainders
   }
   sz[B_ITEMS] = (size_t)32 * L.item_cap * 160;              // up to 160 CTAs
+  sz[B_EMAP] = sizeof(int) * R;
   sz[B_FCTR] = sizeof(int) * kFcTotal;
   sz[B_FTAB] = sizeof(int) * kFtTotal;
   size_t off = 0;
@@ -398,6 +399,7 @@ int run_gemm(dex_ctx* c, int which, const OpDesc& o, const CUtensorMap& tmX, con
   a.ref_tile = c->D.ref_tile;
   a.ref_tiles = c->D.ref_tiles;
   a.vocab = c->D.vocab;
+  a.exit_map = c->D.exit_map;
   if (which == 4) {   // the LM head is one [V, d] matrix: every exit chunk streams "layer" 0
     for (int g = 0; g < kMaxGrp; ++g) a.plan.layer_lo[g] = 0;
   }
@@ -551,20 +553,14 @@ void account_round(dex_ctx* c) {
   c->counters[1] += mega ? 7.0 : 2 + 10.0 * D.max_len + 1 + 1 + 3;
   c->counters[2] += mega ? 1 : gemm_launches;
   c->counters[3] += wbytes;
-  // algorithmic: the LM head once per round; the kernel re-streams it once per LIVE exit chunk (chunks of
-  // exit_chunk rows; 2 at N = 8 when more than 64 rows are live) - that re-stream is traffic, reported separately
-  int max_end = 0;
-  for (int m = 0; m < D.N; ++m) {
-    int ext = 0;
-    const int cap = cap_of(D.N, m);
-    for (int s = 0; s < c->cfg.max_seqs; ++s) {
-      const HostSeq& hs = c->seqs[s];
-      if (!hs.active || hs.done || hs.q < m) continue;
-      ext = std::max(ext, s * cap + (m == hs.q ? 1 : (1 << (hs.q - 1 - m))));
-    }
-    if (ext > 0) max_end = std::max(max_end, c->dec_plan.row_base[m] + ext);
+  // algorithmic: the LM head once per round; the kernel re-streams it once per further exit chunk of
+  // exit_chunk VALID rows (2 chunks only at N = 8, q = 7: 128 rows) - that re-stream is traffic, reported separately
+  long long n_valid = 0;                              // rows decoded this round = 2^q per live sequence (sparse lattice: an upper bound)
+  for (int s = 0; s < c->cfg.max_seqs; ++s) {
+    const HostSeq& hs = c->seqs[s];
+    if (hs.active && !hs.done) n_valid += 1ll << std::min(hs.q, D.N - 1);
   }
-  const int live_chunks = (max_end + D.exit_chunk - 1) / D.exit_chunk;
+  const int live_chunks = (int)((n_valid + D.exit_chunk - 1) / D.exit_chunk);   // the exit head works on DENSE rows (Dev::exit_map)
   c->counters[4] += 2.0 * c->op[4].dec.out_dim * c->op[4].dec.k_dim;
   c->counters[6] += 2.0 * c->op[4].dec.out_dim * c->op[4].dec.k_dim * std::max(0, live_chunks - 1);
   c->counters[5] += kv;
@@ -681,6 +677,7 @@ int32_t dex_init(dex_ctx** out, const dex_config* cfg, const dex_weights* w, con
   D.part = WSP(float, B_PART); D.qbuf = WSP(float, B_QBUF); D.attn_part = WSP(float, B_APART);
   D.rope = WSP(float2, B_ROPE); D.tap_hidden = cfg->debug_taps ? WSP(float, B_TAPH) : nullptr;
   D.gbar = WSP(unsigned int, B_GBAR);
+  D.exit_map = WSP(int, B_EMAP);
   D.flow_ctr = WSP(int, B_FCTR);
   D.item_recs = WSP(void, B_ITEMS);
   D.item_cap = L.item_cap;

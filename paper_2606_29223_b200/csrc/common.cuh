@@ -45,7 +45,8 @@ struct RowInfo {
   int is_ref;              // final-depth anchor node 2^{N-1}-1: never masked (Alg. 2 lines 1-4)
   int n_mask;              // DECS: tokens proposed by shallower nodes of the same slot chain
   int mask_tok[kMaxAnc];
-  int pad[4];
+  int exit_row;            // dense index of this row among the round's valid rows: its row of the exit operand act_e
+  int pad[3];
 };
 static_assert(sizeof(RowInfo) == 32 * 4, "RowInfo is 128 bytes");
 
@@ -107,7 +108,9 @@ struct Dev {
   int* attn_cnt;           // [R_cap][nh] chunk partials written (last writer merges them)
   RowInfo* rows;           // [R_cap]
   int* grp_nb;             // [kMaxGrp] live row extent per decode/prefill group (multiple of 16)
-  int* exit_nb;            // [kMaxGrp] live row extent per exit chunk
+  int* exit_nb;            // [kMaxGrp] live row extent per exit chunk (of the DENSE exit rows)
+  int* exit_map;           // [R_cap] dense exit row -> lattice row (-1 beyond the round's valid rows).  The exit head works on
+                           // dense rows, so a round streams the LM head once per exit_chunk VALID rows, not per row slot
   __nv_bfloat16 *act_a, *act_o, *act_f, *act_e;   // [planes][R_cap][K] MMA operands
   float* part;             // split-K partial sums, per op [S_op][R_cap][ld_op] (OpDesc)
   unsigned int* gbar;      // grid-barrier arrival counter of the round kernel (reset every round)
@@ -237,6 +240,7 @@ struct GemmArgs {
   float2* ref_tile;
   int ref_tiles;
   int vocab;
+  const int* exit_map;     // mode 1: dense exit row -> lattice row
 };
 
 // One projection kind (Y = X . W^T) and its fixed split of K: the split depends on the operator

@@ -611,7 +611,7 @@ __global__ void __launch_bounds__(kFlowThreads, 1) k_flow(const __grid_constant_
       const int quarter = warp & 3;
       EpiCtx ec;
       ec.rows = D.rows; ec.s_valid = s_valid; ec.vocab = D.vocab; ec.best_key = D.best_key;
-      ec.ref_tile = D.ref_tile; ec.ref_tiles = D.ref_tiles; ec.dev = &D;
+      ec.ref_tile = D.ref_tile; ec.ref_tiles = D.ref_tiles; ec.dev = &D; ec.exit_map = D.exit_map;
       FRecWalker w;
       int n_it = 0;
       for (w.start(sq); w.valid; w.next(sq), ++n_it) {

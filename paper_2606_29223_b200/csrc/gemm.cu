@@ -185,7 +185,7 @@ k_gemm(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CUtensor
     EpiCtx ec;
     ec.mode = a.mode; ec.rows = a.rows; ec.s_valid = s_valid; ec.part = a.part; ec.part_ld = a.part_ld;
     ec.split_stride = a.part_split_stride; ec.out_dim = a.out_dim; ec.vocab = a.vocab; ec.best_key = a.best_key;
-    ec.ref_tile = a.ref_tile; ec.ref_tiles = a.ref_tiles; ec.dev = nullptr;
+    ec.ref_tile = a.ref_tile; ec.ref_tiles = a.ref_tiles; ec.dev = nullptr; ec.exit_map = a.exit_map;
     int n_it = 0;
     for (int item = blockIdx.x; item < n_items; item += gridDim.x, ++n_it) {
       Item it = decode_item(a, item, live_g, live_nb);

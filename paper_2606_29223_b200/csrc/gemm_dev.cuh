@@ -21,6 +21,7 @@ struct EpiCtx {
   float2* ref_tile;
   int ref_tiles;
   const Dev* dev;          // sampling mode only (k_round): deferred norm scale, temperature, seed
+  const int* exit_map;     // mode 1: the operand rows are DENSE exit rows; exit_map[row] = lattice row (-1: none)
 };
 
 // One ring stage: (kTileK/16) MMAs of M=128, K=16 into d_tmem.  Activation planes (bf16 hi / lo, R23):
@@ -80,14 +81,17 @@ __device__ __forceinline__ void epilogue_item(const EpiCtx& e, uint32_t t_addr, 
     } else {
       // sampling mode (Alg. 2 line 13): the logit needs its deferred RMSNorm scale before the noise is added;
       // lane i computes the scale of row c0 + i once per block of 16 rows
+      // the operand rows of the exit head are dense exit rows: lane i looks up the lattice row of row c0 + i
+      int lr_lane = -1;
+      if (lane < 16 && row0 + c0 + lane < row_end) lr_lane = e.exit_map[row0 + c0 + lane];
       float inv_lane = 1.f;
       const bool sampling = e.dev != nullptr && e.dev->sample;
-      if (sampling && lane < 16 && row0 + c0 + lane < row_end) inv_lane = inv_rms(*e.dev, row0 + c0 + lane) * e.dev->inv_tau;
+      if (sampling && lr_lane >= 0) inv_lane = inv_rms(*e.dev, lr_lane) * e.dev->inv_tau;
 #pragma unroll
       for (int i = 0; i < 16; ++i) {
-        const int rr = row0 + c0 + i;
+        const int rr = __shfl_sync(0xffffffffu, lr_lane, i);
         const float inv_i = __shfl_sync(0xffffffffu, inv_lane, i);
-        if (rr >= row_end || !((e.s_valid[rr >> 5] >> (rr & 31)) & 1u)) continue;   // warp-uniform
+        if (rr < 0) continue;                                                        // warp-uniform
         const RowInfo* ri = &e.rows[rr];
         float val = __uint_as_float(v[i]);
         if (sampling) val = val * inv_i + gumbel_noise(e.dev->sample_seed, ri->seq, ri->pos + 1, col);

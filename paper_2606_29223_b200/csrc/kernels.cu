@@ -72,14 +72,17 @@ __device__ __forceinline__ int round16(int v) { return (v + 15) & ~15; }
 __device__ __forceinline__ int stage_count(int q, int m) { return m > q ? 0 : (m == q ? 1 : (1 << (q - 1 - m))); }
 
 // ------------------------------------------------------------------------------------------
-// a0: expand bookkeeping.  One thread per row slot of the decode plan.
-__global__ void k_rows_decode(Dev D, Plan plan) {
-  const int r = blockIdx.x * blockDim.x + threadIdx.x;
-  for (int i = r; i < kFcTotal; i += gridDim.x * blockDim.x) D.flow_ctr[i] = 0;   // k_flow: arrival counters / ready flags
+// a0: expand bookkeeping.  ONE block, one thread per row slot of the decode plan (R_cap <= 1024): the valid rows are
+// ranked with a block-wide scan, which gives every row its DENSE exit row (the exit head then streams the LM head once
+// per exit_chunk valid rows instead of once per exit_chunk row slots: at N = 8 the slots of a low-q round span both
+// chunks although a handful of rows are live).
+__global__ void __launch_bounds__(1024) k_rows_decode(Dev D, Plan plan) {
+  __shared__ int s_wcnt[32];
+  const int r = threadIdx.x;
+  for (int i = r; i < kFcTotal; i += blockDim.x) D.flow_ctr[i] = 0;   // k_flow: arrival counters / ready flags
   if (r == 0) {
     *D.gbar = 0u;                                     // grid-barrier counter of this round's k_round
-    // live row extent of every stage group and of every exit chunk
-    int max_end = 0;
+    // live row extent of every stage group
     for (int m = 0; m < kMaxGrp; ++m) {
       int ext = 0;
       if (m < D.N) {
@@ -88,22 +91,17 @@ __global__ void k_rows_decode(Dev D, Plan plan) {
           const SeqState st = D.seqs[s];
           if (seq_live(st) && st.q >= m) ext = max(ext, s * cap + stage_count(st.q, m));
         }
-        if (ext > 0) max_end = max(max_end, plan.row_base[m] + ext);
       }
       D.grp_nb[m] = round16(ext);
     }
-    for (int c = 0; c < kMaxGrp; ++c) {
-      int e = min(D.exit_chunk, max_end - D.exit_chunk * c);
-      D.exit_nb[c] = e > 0 ? round16(e) : 0;
-    }
   }
-  if (r >= D.R_cap) return;
-  D.best_key[r] = 0ull;
+  const bool in_range = r < D.R_cap;
+  if (in_range) D.best_key[r] = 0ull;
   RowInfo ri;
   ri.valid = 0;
   ri.seq = 0; ri.node = -1; ri.pos = -1; ri.grp = 0; ri.slot = 0; ri.n_paged = 0; ri.n_anc = 0;   // a clean dead row
   ri.parent_row = -1; ri.tok_in = 0; ri.is_ref = 0; ri.n_mask = 0;
-  if (r < D.R_dec) {
+  if (in_range && r < D.R_dec) {
     int m = 0;
     while (m + 1 < D.N && r >= plan.row_base[m + 1]) ++m;
     const int cap = cap_of(D.N, m);
@@ -162,7 +160,28 @@ __global__ void k_rows_decode(Dev D, Plan plan) {
       }
     }
   }
-  D.rows[r] = ri;
+  // dense rank of the valid rows (ascending row index) = exit row
+  const int lane = threadIdx.x & 31, wp = threadIdx.x >> 5;
+  const unsigned bal = __ballot_sync(0xffffffffu, ri.valid != 0);
+  if (lane == 0) s_wcnt[wp] = __popc(bal);
+  __syncthreads();
+  int base = 0, total = 0;
+  for (int w = 0; w < (int)(blockDim.x >> 5); ++w) {
+    base += w < wp ? s_wcnt[w] : 0;
+    total += s_wcnt[w];
+  }
+  const int rank = base + __popc(bal & ((1u << lane) - 1u));
+  ri.exit_row = ri.valid ? rank : 0;
+  ri.pad[0] = ri.pad[1] = ri.pad[2] = 0;
+  if (in_range) {
+    D.rows[r] = ri;
+    if (ri.valid) D.exit_map[rank] = r;
+    if (r >= total) D.exit_map[r] = -1;
+  }
+  if (r < kMaxGrp) {                                  // live extent of every exit chunk of the dense rows
+    const int e = min(D.exit_chunk, total - D.exit_chunk * r);
+    D.exit_nb[r] = e > 0 ? round16(e) : 0;
+  }
 }
 
 // Prefill rows: positions p0 .. p0+R-1 of the prompt as one causal chunk.
@@ -192,6 +211,8 @@ __global__ void k_rows_prefill(Dev D, int seq, int p0, int R) {
     ri.is_ref = 0;
     ri.n_mask = 0;
   }
+  ri.exit_row = r;                                    // no exit op in prefill; keeps the last norm's (unused) operand row in range
+  D.exit_map[r] = -1;
   D.rows[r] = ri;
 }
 
@@ -296,7 +317,7 @@ __global__ void __launch_bounds__(1024) k_add_norm(Dev D, Plan plan, int step, i
       ss = sumsq4(v);
       if (mode == 1 && D.taps) *reinterpret_cast<float4*>(D.tap_hidden + ((size_t)r * D.max_len + step) * D.d + i) = v;
       const float4 wv = ld4(w + i);
-      split_store4(dst, ps, (size_t)r * D.d + i, make_float4(v.x * wv.x, v.y * wv.y, v.z * wv.z, v.w * wv.w), D.planes);
+      split_store4(dst, ps, (size_t)(dst == D.act_e ? ri.exit_row : r) * D.d + i, make_float4(v.x * wv.x, v.y * wv.y, v.z * wv.z, v.w * wv.w), D.planes);
     }
     ss = warp_sum(ss);
     if (lane == 0) D.ss_part[(size_t)r * kSsSeg + seg] = ss;
@@ -807,7 +828,7 @@ __global__ void k_tap_logits(Dev D, int row, float* out) {
   const int v = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), lane = threadIdx.x & 31;
   if (v >= D.vocab) return;
   const __nv_bfloat16* w = D.lm_head + (size_t)v * D.d;
-  const __nv_bfloat16* e = D.act_e + (size_t)row * D.d;
+  const __nv_bfloat16* e = D.act_e + (size_t)D.rows[row].exit_row * D.d;
   const size_t ps = (size_t)D.R_cap * D.d;
   float acc = 0.f;
   for (int i = lane; i < D.d; i += 32) {
@@ -839,6 +860,8 @@ __global__ void k_debug_rows(Dev D, int R) {
   ri.seq = 0; ri.node = -1; ri.pos = 0; ri.grp = 0; ri.slot = -1; ri.n_paged = 0; ri.n_anc = 0;
   ri.parent_row = -1; ri.tok_in = 0; ri.is_ref = 0; ri.n_mask = 0;
   for (int i = 0; i < kMaxAnc; ++i) ri.anc[i] = 0, ri.mask_tok[i] = -1;
+  ri.exit_row = r;
+  D.exit_map[r] = -1;
   D.rows[r] = ri;
 }
 __global__ void k_debug_split(const float* x, __nv_bfloat16* dst, int rows, int k, size_t plane_stride, int planes) {
@@ -875,7 +898,8 @@ cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, cudaStream
 }
 
 cudaError_t launch_rows_decode(const Dev& D, const Plan& p, cudaStream_t st) {
-  k_rows_decode<<<(D.R_cap + 127) / 128, 128, 0, st>>>(D, p);
+  if (D.R_cap > 1024) return cudaErrorInvalidValue;
+  k_rows_decode<<<1, 1024, 0, st>>>(D, p);
   DEX_LAUNCH_CHECK();
 }
 cudaError_t launch_rows_prefill(const Dev& D, int seq, int p0, int R, cudaStream_t st) {

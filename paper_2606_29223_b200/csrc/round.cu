@@ -206,7 +206,7 @@ __global__ void __launch_bounds__(kMaxThreads, 1) k_round(const __grid_constant_
       const int gw = blockIdx.x * kGlueWarps + we, n_gw = gridDim.x * kGlueWarps;
       EpiCtx ec;
       ec.rows = D.rows; ec.s_valid = s_valid; ec.part = D.part; ec.vocab = D.vocab; ec.best_key = D.best_key;
-      ec.ref_tile = D.ref_tile; ec.ref_tiles = D.ref_tiles; ec.dev = &D;
+      ec.ref_tile = D.ref_tile; ec.ref_tiles = D.ref_tiles; ec.dev = &D; ec.exit_map = D.exit_map;
       Walker w;
       w.start(sq);
       int n_it = 0;

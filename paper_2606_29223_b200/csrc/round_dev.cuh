@@ -211,7 +211,7 @@ __device__ __forceinline__ void unit_add_norm(const RoundArgs& a, int j, int mod
   const Dev& D = a.D;
   // the row table, x and the partials are loaded together (addresses depend on r only); w needs the layer
   const RowInfo* ri = &D.rows[r];
-  const int valid = ri->valid, grp = ri->grp;
+  const int valid = ri->valid, grp = ri->grp, exit_row = ri->exit_row;
   const int i = seg * 128 + lane * 4;
   const bool in = i < D.d;
   float* x = D.x_cur + (size_t)r * D.d + (in ? i : 0);
@@ -242,7 +242,8 @@ __device__ __forceinline__ void unit_add_norm(const RoundArgs& a, int j, int mod
     *reinterpret_cast<float4*>(x) = v;
     ss = sumsq4(v);
     if (mode == 1 && D.taps) *reinterpret_cast<float4*>(D.tap_hidden + ((size_t)r * D.max_len + j) * D.d + i) = v;
-    r_split_store4(dst, (size_t)D.R_cap * D.d, (size_t)r * D.d + i, make_float4(v.x * wv.x, v.y * wv.y, v.z * wv.z, v.w * wv.w),
+    // the exit operand is indexed by the row's DENSE exit row (Dev::exit_map)
+    r_split_store4(dst, (size_t)D.R_cap * D.d, (size_t)(dst == D.act_e ? exit_row : r) * D.d + i, make_float4(v.x * wv.x, v.y * wv.y, v.z * wv.z, v.w * wv.w),
                    D.planes);
   }
   ss = r_warp_sum(ss);
@@ -344,7 +345,7 @@ static __device__ void glue_ad2(const RoundArgs& a, const OpDesc& op, int gw, in
       const float4 v = make_float4(xv.x + al * (sv[0].x + bv.x), xv.y + al * (sv[0].y + bv.y), xv.z + al * (sv[0].z + bv.z),
                                    xv.w + al * (sv[0].w + bv.w));
       ss = sumsq4(v);
-      r_split_store4(D.act_e, (size_t)D.R_cap * D.d, (size_t)r * D.d + i, make_float4(v.x * wv.x, v.y * wv.y, v.z * wv.z, v.w * wv.w),
+      r_split_store4(D.act_e, (size_t)D.R_cap * D.d, (size_t)ri->exit_row * D.d + i, make_float4(v.x * wv.x, v.y * wv.y, v.z * wv.z, v.w * wv.w),
                      D.planes);
     }
     ss = r_warp_sum(ss);
