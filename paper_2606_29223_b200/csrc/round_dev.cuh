@@ -505,6 +505,9 @@ struct AttnSmem {
   __nv_bfloat16 ql[kAttnPairs][HD + 8];
   int ppos[kAttnPairs];                         // position of the pair's row; -1: not in this pass
   int prow[kAttnPairs], phead[kAttnPairs];
+  int rpos[kAttnPairs];                         // per LATTICE ROW of the pass (row rl = pair / Gq): its position and the slot
+  int rslot[kAttnPairs][kMaxAnc + 1];           // that holds private position n_paged + i (ancestor slots, then its own): read
+                                                // once per task, so the private-tile loop has ONE dependent load per row
   int n_vrow;                                   // sparse lattice (R26): the expanded rows of the task's (stage, sequence)
   short vrow[128];
 };
@@ -816,6 +819,14 @@ __device__ void attn_run(const RoundArgs& a, const AttnPlan& pl, const AttnTask&
       sm->ppos[pi] = pos;
       sm->prow[pi] = r;
       sm->phead[pi] = h;
+      if (pi < np && (pb + pi) % Gq == 0) {                  // first pair of a lattice row: the row's private-suffix table
+        const int rl = pi / Gq;
+        const RowInfo* ri = &D.rows[r];
+        const int n_anc = ri->n_anc, own = ri->slot;
+        sm->rpos[rl] = ri->pos;
+#pragma unroll
+        for (int i = 0; i <= kMaxAnc; ++i) sm->rslot[rl][i] = (i < n_anc && i < kMaxAnc) ? ri->anc[i] : own;
+      }
     }
     for (int c = ca; c < cb; ++c) {
       const int buf = (c - ca) & 1, c0 = c * kChunk;
@@ -865,15 +876,13 @@ __device__ void attn_run(const RoundArgs& a, const AttnPlan& pl, const AttnTask&
           }
           const uint32_t kbt = smem_u32(sm->kv[tb][0]), vbt = smem_u32(sm->kv[tb][1]);
           for (int rl = rank; rl < n_rl; rl += nk) {
-            const int r = row_of(pb / Gq + rl);
-            const RowInfo* ri = &D.rows[r];
-            const int pos = ri->pos;
+            const int pos = sm->rpos[rl];
             if (pos < p0) continue;                        // the row does not see this tile (warp-uniform)
             const int i_hi = min(pos - p0, 15);
             for (int id = lane; id < (i_hi - i_lo + 1) * CPR; id += 32) {
               const int i = i_lo + id / CPR, cj = id % CPR, pl = trow + i;
               const int ai = p0 + i - n_paged;
-              const int slot = (ai < ri->n_anc) ? ri->anc[ai] : ri->slot;
+              const int slot = sm->rslot[rl][min(ai, kMaxAnc)];
               const size_t so = slot_off(D, s, slot, layer) + (size_t)g * HD + cj * 8;
               const int dj = (cj ^ (pl & 7)) * 8;
               *reinterpret_cast<uint4*>(&sm->kv[tb][0][pl * HD + dj]) = *reinterpret_cast<const uint4*>(D.kslot + so);
