@@ -315,6 +315,7 @@ __global__ void __launch_bounds__(kFlowThreads, 1) k_flow(const __grid_constant_
   __shared__ int s_qtarget[kFlowSlices];
   __shared__ int s_ao_cnt[kFlowSlices];
   __shared__ FDec s_dec[2];
+  __shared__ SeqState s_seq[8];          // the round's FSM snapshot
   __shared__ FJob s_queue[kFlowQueue];
   __shared__ unsigned s_qhead, s_qtail;  // jobs pushed by the counter warp / taken by the finalizer group
   __shared__ unsigned s_cdone;           // the counter warp has counted every layer-step item of this CTA
@@ -322,6 +323,12 @@ __global__ void __launch_bounds__(kFlowThreads, 1) k_flow(const __grid_constant_
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   if (threadIdx.x < 32) s_valid[threadIdx.x] = 0;
+  if (threadIdx.x >= 32 && threadIdx.x < 40) {
+    const int s_ = threadIdx.x - 32;
+    SeqState z;
+    z.active = 0; z.q = 0; z.ctx_len = 0; z.n_tok = 0; z.last_tok = 0; z.pending = 0; z.done = 1; z.pad = 0;
+    s_seq[s_] = s_ < D.max_seqs ? D.seqs[s_] : z;
+  }
   if (threadIdx.x < kMaxGrp) s_nvalid[threadIdx.x] = 0;
   __syncthreads();
   for (int r = threadIdx.x; r < D.R_cap; r += blockDim.x)
@@ -783,7 +790,7 @@ __global__ void __launch_bounds__(kFlowThreads, 1) k_flow(const __grid_constant_
             while (!have && att_j < sq.n_steps) {
               if (att_u >= pl.n_tasks) { ++att_j; att_u = blockIdx.x; continue; }
               attn_task_of<PT>(a, pl, s_cum, G, att_u, tk);
-              const SeqState sst = D.seqs[tk.s];
+              const SeqState sst = s_seq[tk.s];
               if (!r_seq_live(sst) || sst.q < tk.m || att_j >= a.dec.layer_len[tk.m] || s_nb[tk.m] == 0) { att_u += G; continue; }
               have = true;
             }
@@ -844,8 +851,8 @@ __global__ void __launch_bounds__(kFlowThreads, 1) k_flow(const __grid_constant_
           const int j = dec->j;
           if (tid_f < kFlowSlices) s_ao_cnt[tid_f] = 0;
           bar_f<GT>();
-          if (D.hd == 128) attn_run<128, GT, PT>(a, pl, tk, j, tid_f, lane, we, reinterpret_cast<AttnSmem<128>*>(asm_), s_ao_cnt, sl_o);
-          else attn_run<64, GT, PT>(a, pl, tk, j, tid_f, lane, we, reinterpret_cast<AttnSmem<64>*>(asm_), s_ao_cnt, sl_o);
+          if (D.hd == 128) attn_run<128, GT, PT>(a, pl, tk, j, tid_f, lane, we, reinterpret_cast<AttnSmem<128>*>(asm_), s_ao_cnt, sl_o, s_seq);
+          else attn_run<64, GT, PT>(a, pl, tk, j, tid_f, lane, we, reinterpret_cast<AttnSmem<64>*>(asm_), s_ao_cnt, sl_o, s_seq);
           fence_proxy_async();                               // act_o is read by TMA
           bar_f<GT>();
           if (tid_f < kFlowSlices) {

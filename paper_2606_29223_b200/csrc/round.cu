@@ -49,9 +49,16 @@ __global__ void __launch_bounds__(kMaxThreads, 1) k_round(const __grid_constant_
   __shared__ int s_cum[kMaxGrp + 1];
   __shared__ int s_steps;
   __shared__ unsigned s_seen;
+  __shared__ SeqState s_seq[8];          // the round's FSM snapshot (attention tasks read it instead of global memory)
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   if (threadIdx.x < 32) s_valid[threadIdx.x] = 0;
+  if (threadIdx.x >= 32 && threadIdx.x < 40) {
+    const int s_ = threadIdx.x - 32;
+    SeqState z;
+    z.active = 0; z.q = 0; z.ctx_len = 0; z.n_tok = 0; z.last_tok = 0; z.pending = 0; z.done = 1; z.pad = 0;
+    s_seq[s_] = s_ < D.max_seqs ? D.seqs[s_] : z;
+  }
   __syncthreads();
   for (int r = threadIdx.x; r < D.R_cap; r += blockDim.x)
     if (D.rows[r].valid) atomicOr(&s_valid[r >> 5], 1u << (r & 31));
@@ -244,8 +251,8 @@ __global__ void __launch_bounds__(kMaxThreads, 1) k_round(const __grid_constant_
         ++gb; grid_bar<GT>(D.gbar, gb * G, tid_e, &s_seen, gb); stamp();
         {
           void* asm_ = smem + a.attn_smem_off;
-          if (D.hd == 128) glue_attention<128, GT, PT>(a, j, tid_e, lane, we, blockIdx.x, G, reinterpret_cast<AttnSmem<128>*>(asm_), s_live_ms, s_cum);
-          else glue_attention<64, GT, PT>(a, j, tid_e, lane, we, blockIdx.x, G, reinterpret_cast<AttnSmem<64>*>(asm_), s_live_ms, s_cum);
+          if (D.hd == 128) glue_attention<128, GT, PT>(a, j, tid_e, lane, we, blockIdx.x, G, reinterpret_cast<AttnSmem<128>*>(asm_), s_live_ms, s_cum, s_seq);
+          else glue_attention<64, GT, PT>(a, j, tid_e, lane, we, blockIdx.x, G, reinterpret_cast<AttnSmem<64>*>(asm_), s_live_ms, s_cum, s_seq);
         }
         stamp();
         ++gb; grid_bar<GT>(D.gbar, gb * G, tid_e, &s_seen, gb); stamp();

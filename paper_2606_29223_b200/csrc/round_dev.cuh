@@ -731,7 +731,7 @@ __device__ __forceinline__ void attn_task_of(const RoundArgs& a, const AttnPlan&
 // only, else nullptr): shared counters of the (row, head) pairs this task merged, per ao_slice_cols columns of act_o.
 template <int HD, int GT, bool PT>
 __device__ void attn_run(const RoundArgs& a, const AttnPlan& pl, const AttnTask& tk, int j, int tid_e, int lane, int we,
-                         AttnSmem<HD>* sm, int* s_ao_cnt, int ao_slice_cols) {
+                         AttnSmem<HD>* sm, int* s_ao_cnt, int ao_slice_cols, const SeqState* seq_sm) {
   constexpr int CPR = HD / 8;                                // 16-byte pieces per K/V row
   constexpr int kEpiThreads = GT;
   const Dev& D = a.D;
@@ -739,7 +739,7 @@ __device__ void attn_run(const RoundArgs& a, const AttnPlan& pl, const AttnTask&
   const bool tail_own = pl.tail_own != 0;
   const int n_body = pl.n_body, CR = pl.CR, n_ranges = pl.n_ranges, Gq = pl.Gq;
   const size_t kv_stride = (size_t)D.nkv * HD;
-  const SeqState st = D.seqs[s];
+  const SeqState st = seq_sm[s];                            // the round's FSM snapshot in shared memory (constant for the round)
   if (!r_seq_live(st) || st.q < m || j >= a.dec.layer_len[m]) return;
   const bool is_tail = tail_own && rg == n_ranges - 1;
   const int ca = is_tail ? n_body : rg * CR;
@@ -905,14 +905,18 @@ __device__ void attn_run(const RoundArgs& a, const AttnPlan& pl, const AttnTask&
       const int mine = min(cb, pos / kChunk + 1) - ca;     // chunks of this range visible to the row
       if (mine <= 0) continue;
       const int nc = pos / kChunk + 1;
+      // this range holds EVERY chunk the row sees: sole writer, no counter (the CTA barrier above already orders this
+      // CTA's sub-partial stores before the merge's loads) - saves the atomic's round trip on the lattice rounds, whose
+      // (stage, head) families fill the grid with one range each
+      const bool sole = mine == nc;
       int old = 0;
-      if (lane == 0)                                         // release our sub-partials, acquire the other ranges'
+      if (!sole && lane == 0)                                // release our sub-partials, acquire the other ranges'
         asm volatile("atom.acq_rel.gpu.global.add.s32 %0, [%1], %2;\n" : "=r"(old) : "l"(&D.attn_cnt[r * D.nh + h]), "r"(mine) : "memory");
       old = __shfl_sync(0xffffffffu, old, 0);
-      if (old + mine == nc) {
+      if (sole || old + mine == nc) {
         attn_merge<HD>(D, r, h, pos / 16 + 1, lane);           // reads with ld.global.cg (L2)
         if (lane == 0) {
-          D.attn_cnt[r * D.nh + h] = 0;
+          if (!sole) D.attn_cnt[r * D.nh + h] = 0;
           if (s_ao_cnt) atomicAdd(&s_ao_cnt[(h * HD) / ao_slice_cols], 1);   // k_flow: merged (row, head) pairs per O-operand slice
         }
       }
@@ -923,13 +927,13 @@ __device__ void attn_run(const RoundArgs& a, const AttnPlan& pl, const AttnTask&
 
 template <int HD, int GT, bool PT>
 __device__ void glue_attention(const RoundArgs& a, int j, int tid_e, int lane, int we, int cta, int G,
-                               AttnSmem<HD>* sm, int n_live_ms, const int* cum) {
+                               AttnSmem<HD>* sm, int n_live_ms, const int* cum, const SeqState* seq_sm) {
   AttnPlan pl;
   attn_plan<PT>(a, G, n_live_ms, cum, pl);
   for (int u = cta; u < pl.n_tasks; u += G) {
     AttnTask tk;
     attn_task_of<PT>(a, pl, cum, G, u, tk);
-    attn_run<HD, GT, PT>(a, pl, tk, j, tid_e, lane, we, sm, nullptr, 1);
+    attn_run<HD, GT, PT>(a, pl, tk, j, tid_e, lane, we, sm, nullptr, 1, seq_sm);
   }
 }
 
