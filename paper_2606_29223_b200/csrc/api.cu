@@ -699,9 +699,11 @@ int32_t dex_init(dex_ctx** out, const dex_config* cfg, const dex_weights* w, con
     // the round kernel also carves its attention scratch out of dynamic shared memory: fewer ring stages
     const size_t stage = 16384 + (size_t)cfg->act_planes * c->round_ring.x_cap * 128;
     const size_t attn = (round_attn_smem(cfg->head_dim) + 1023) / 1024 * 1024;
-    // 227 KB per block minus k_flow's static shared memory (< 4 KB) and alignment slack.  (219 KB, as this stood for part
-    // of round 2, left a 256-row single-plane stage one byte short of 3 ring stages: c5 fell back to the per-op path.)
-    const size_t budget = 222 * 1024 - attn - 2048;
+    // 227 KB per block (232448 B) minus the kernels' static shared memory (k_round: row cache, 4.8 KB; k_flow: 3.8 KB)
+    // and alignment slack: the dynamic request is at most budget constant + 511 B, the kernels' limits are 222 / 223 KB.
+    // (219 KB, as this stood for part of round 2, left a 256-row single-plane stage short of 3 ring stages: c5 fell
+    // back to the per-op path; at 221 KB it has 148480 B for 3 x 49152.)
+    const size_t budget = 221 * 1024 - attn - 2048;
     c->round_ok = budget / stage >= 3 && c->round_ring.n_acc == 2;   // too few ring stages (very wide stages): per-op path   // too few ring stages (very wide stages): per-op path
     if ((cfg->sample || c->has_ad) && !c->round_ok) {
       delete c;

@@ -49,6 +49,7 @@ __global__ void __launch_bounds__(kMaxThreads, 1) k_round(const __grid_constant_
   __shared__ int s_cum[kMaxGrp + 1];
   __shared__ int s_steps;
   __shared__ unsigned s_seen;
+  __shared__ RowLite s_row[kRowCache];   // per-row record of the glue units (round_dev.cuh)
   __shared__ SeqState s_seq[8];          // the round's FSM snapshot (attention tasks read it instead of global memory)
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -60,8 +61,12 @@ __global__ void __launch_bounds__(kMaxThreads, 1) k_round(const __grid_constant_
     s_seq[s_] = s_ < D.max_seqs ? D.seqs[s_] : z;
   }
   __syncthreads();
-  for (int r = threadIdx.x; r < D.R_cap; r += blockDim.x)
-    if (D.rows[r].valid) atomicOr(&s_valid[r >> 5], 1u << (r & 31));
+  for (int r = threadIdx.x; r < D.R_cap; r += blockDim.x) {
+    const RowInfo ri = D.rows[r];
+    if (ri.valid) atomicOr(&s_valid[r >> 5], 1u << (r & 31));
+    if (r < kRowCache) s_row[r] = row_lite_of(ri);
+  }
+  const RowLite* const rc = D.R_cap <= kRowCache ? s_row : nullptr;
   if (threadIdx.x == 0) {
     int steps = 0;
     for (int g = 0; g < 8; ++g) {
@@ -246,7 +251,7 @@ __global__ void __launch_bounds__(kMaxThreads, 1) k_round(const __grid_constant_
       for (int j = 0; j < sq.n_steps; ++j) {
         run_items(4 * j); stamp();
         ++gb; grid_bar<GT>(D.gbar, gb * G, tid_e, &s_seen, gb); stamp();
-        if (D.hd == 128) glue_qkv_finalize<128>(a, j, gw, n_gw, lane); else glue_qkv_finalize<64>(a, j, gw, n_gw, lane);
+        if (D.hd == 128) glue_qkv_finalize<128>(a, j, gw, n_gw, lane, rc); else glue_qkv_finalize<64>(a, j, gw, n_gw, lane, rc);
         stamp();
         ++gb; grid_bar<GT>(D.gbar, gb * G, tid_e, &s_seen, gb); stamp();
         {
@@ -258,7 +263,7 @@ __global__ void __launch_bounds__(kMaxThreads, 1) k_round(const __grid_constant_
         ++gb; grid_bar<GT>(D.gbar, gb * G, tid_e, &s_seen, gb); stamp();
         run_items(4 * j + 1); stamp();
         ++gb; grid_bar<GT>(D.gbar, gb * G, tid_e, &s_seen, gb); stamp();
-        glue_add_norm(a, j, 0, a.op[1], gw, n_gw, lane);
+        glue_add_norm(a, j, 0, a.op[1], gw, n_gw, lane, rc);
         stamp();
         ++gb; grid_bar<GT>(D.gbar, gb * G, tid_e, &s_seen, gb); stamp();
         run_items(4 * j + 2); stamp();
@@ -268,7 +273,7 @@ __global__ void __launch_bounds__(kMaxThreads, 1) k_round(const __grid_constant_
         ++gb; grid_bar<GT>(D.gbar, gb * G, tid_e, &s_seen, gb); stamp();
         run_items(4 * j + 3); stamp();
         ++gb; grid_bar<GT>(D.gbar, gb * G, tid_e, &s_seen, gb); stamp();
-        glue_add_norm(a, j, 1, a.op[3], gw, n_gw, lane);
+        glue_add_norm(a, j, 1, a.op[3], gw, n_gw, lane, rc);
         stamp();
         ++gb; grid_bar<GT>(D.gbar, gb * G, tid_e, &s_seen, gb); stamp();
       }
@@ -298,9 +303,9 @@ __global__ void __launch_bounds__(kMaxThreads, 1) k_round(const __grid_constant_
 size_t round_attn_smem(int hd) { return hd == 128 ? sizeof(AttnSmem<128>) : sizeof(AttnSmem<64>); }
 
 cudaError_t round_init() {
-  cudaError_t e = cudaFuncSetAttribute(k_round<kRoundThreads, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024);
+  cudaError_t e = cudaFuncSetAttribute(k_round<kRoundThreads, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 222 * 1024);
   if (e != cudaSuccess) return e;
-  return cudaFuncSetAttribute(k_round<kRoundThreads, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024);
+  return cudaFuncSetAttribute(k_round<kRoundThreads, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 222 * 1024);
 }
 
 // Cooperative launch: all CTAs must be co-resident (they meet at grid barriers).

@@ -194,6 +194,39 @@ __device__ __forceinline__ void grid_bar(unsigned* gbar, unsigned target, int ti
   bar_epi<GT>();
 }
 
+// ---------------------------------------------------------------- per-row record cached in shared memory
+// The glue units need a row's (valid, stage, sequence, slot, position, exit row) before they can address anything that
+// depends on the layer or the position (norm weights, RoPE table, slot K/V): read from the row table in global memory
+// that is one more dependent L2 round trip per phase under the weight stream.  k_round copies the fields into shared
+// memory once per round (8 bytes per row); callers without the cache (k_flow) pass nullptr.
+struct RowLite {
+  int pos;
+  unsigned bits;           // valid | grp << 1 | seq << 4 | slot << 8 | exit_row << 16
+};
+constexpr int kRowCache = 544;   // rows cached (R_cap of every supported lattice: 4 x 128 + 16 slack + 16)
+struct RowView {
+  int valid, grp, seq, slot, pos, exit_row;
+};
+__device__ __forceinline__ RowLite row_lite_of(const RowInfo& ri) {
+  RowLite l;
+  l.pos = ri.pos;
+  l.bits = (ri.valid ? 1u : 0u) | ((unsigned)ri.grp & 7u) << 1 | ((unsigned)ri.seq & 15u) << 4 | ((unsigned)ri.slot & 255u) << 8 |
+           ((unsigned)ri.exit_row & 65535u) << 16;
+  return l;
+}
+__device__ __forceinline__ RowView row_view(const Dev& D, const RowLite* cache, int r) {
+  RowView v;
+  if (cache != nullptr) {
+    const RowLite l = cache[r];
+    v.valid = l.bits & 1u; v.grp = (l.bits >> 1) & 7u; v.seq = (l.bits >> 4) & 15u; v.slot = (l.bits >> 8) & 255u;
+    v.exit_row = l.bits >> 16; v.pos = l.pos;
+  } else {
+    const RowInfo* ri = &D.rows[r];
+    v.valid = ri->valid; v.grp = ri->grp; v.seq = ri->seq; v.slot = ri->slot; v.pos = ri->pos; v.exit_row = ri->exit_row;
+  }
+  return v;
+}
+
 // ---------------------------------------------------------------- glue phases (epilogue group)
 __device__ __forceinline__ float r_warp_sum(float v) {
 #pragma unroll
@@ -207,11 +240,12 @@ __device__ __forceinline__ float r_warp_sum(float v) {
 // 128-element segment).  mode 0: after o_proj (w = norm_ffn[l] -> act_a); mode 1: after down_proj (next layer's
 // attention norm -> act_a, or the shared final norm -> act_e).
 __device__ __forceinline__ void unit_add_norm(const RoundArgs& a, int j, int mode, const OpDesc& op, const float* part, int r, int seg,
-                                              int lane) {
+                                              int lane, const RowLite* rc = nullptr) {
   const Dev& D = a.D;
-  // the row table, x and the partials are loaded together (addresses depend on r only); w needs the layer
-  const RowInfo* ri = &D.rows[r];
-  const int valid = ri->valid, grp = ri->grp, exit_row = ri->exit_row;
+  // the row table, x and the partials are loaded together (addresses depend on r only); w needs the layer (with the
+  // shared-memory row cache it is known at once and w joins the same batch of loads)
+  const RowView rv = row_view(D, rc, r);
+  const int valid = rv.valid, grp = rv.grp, exit_row = rv.exit_row;
   const int i = seg * 128 + lane * 4;
   const bool in = i < D.d;
   float* x = D.x_cur + (size_t)r * D.d + (in ? i : 0);
@@ -249,12 +283,12 @@ __device__ __forceinline__ void unit_add_norm(const RoundArgs& a, int j, int mod
   ss = r_warp_sum(ss);
   if (lane == 0) D.ss_part[(size_t)r * kSsSeg + seg] = ss;
 }
-static __device__ void glue_add_norm(const RoundArgs& a, int j, int mode, const OpDesc& op, int gw, int n_gw, int lane) {
+static __device__ void glue_add_norm(const RoundArgs& a, int j, int mode, const OpDesc& op, int gw, int n_gw, int lane, const RowLite* rc) {
   const Dev& D = a.D;
   const int n_seg = (D.d + 127) / 128;
   for (int u = gw; u < D.R_dec * n_seg; u += n_gw) {
     const int r = u / n_seg, seg = u - r * n_seg;
-    unit_add_norm(a, j, mode, op, D.part, r, seg, lane);
+    unit_add_norm(a, j, mode, op, D.part, r, seg, lane, rc);
   }
 }
 
@@ -418,15 +452,16 @@ __device__ __forceinline__ void attn_merge(const Dev& D, int r, int h, int n_sub
 // Phase Q (warp = (row, head of the fused QKV output)): split-K sum, deferred RMSNorm scale, RoPE (rotate-half,
 // R13); query heads -> fp32 qbuf, key / value heads -> bf16 into the row's branch-private slot.
 template <int HD>
-__device__ __forceinline__ void unit_qkv(const RoundArgs& a, int j, const float* part, int r, int hh, int lane) {
+__device__ __forceinline__ void unit_qkv(const RoundArgs& a, int j, const float* part, int r, int hh, int lane,
+                                         const RowLite* rc = nullptr) {
   constexpr int DPL = HD / 32, HH = HD / 2;
   const Dev& D = a.D;
   const OpDesc& op = a.op[0];
-  const RowInfo* ri = &D.rows[r];
-  if (!ri->valid) return;
-  const int m = ri->grp;
+  const RowView rv = row_view(D, rc, r);
+  if (!rv.valid) return;
+  const int m = rv.grp;
   if (j >= a.dec.layer_len[m]) return;
-  const int layer = a.dec.layer_lo[m] + j, pos = ri->pos;
+  const int layer = a.dec.layer_lo[m] + j, pos = rv.pos;
   const float inv = inv_rms(D, r);
   const int d0 = lane * DPL;
   const float* p = part + (size_t)r * op.part_ld + (size_t)hh * HD + d0;
@@ -465,18 +500,18 @@ __device__ __forceinline__ void unit_qkv(const RoundArgs& a, int j, const float*
     for (int t = 0; t < DPL; ++t) q[t] = o[t];
   } else {
     const int g = is_v ? hh - D.nh - D.nkv : hh - D.nh;
-    __nv_bfloat16* dst = (is_v ? D.vslot : D.kslot) + slot_off(D, ri->seq, ri->slot, layer) + (size_t)g * HD + d0;
+    __nv_bfloat16* dst = (is_v ? D.vslot : D.kslot) + slot_off(D, rv.seq, rv.slot, layer) + (size_t)g * HD + d0;
 #pragma unroll
     for (int t = 0; t < DPL; ++t) dst[t] = __float2bfloat16_rn(o[t]);
   }
 }
 template <int HD>
-__device__ void glue_qkv_finalize(const RoundArgs& a, int j, int gw, int n_gw, int lane) {
+__device__ void glue_qkv_finalize(const RoundArgs& a, int j, int gw, int n_gw, int lane, const RowLite* rc) {
   const Dev& D = a.D;
   const int heads = D.nh + 2 * D.nkv;
   for (int u = gw; u < D.R_dec * heads; u += n_gw) {
     const int r = u / heads, hh = u - r * heads;
-    unit_qkv<HD>(a, j, D.part, r, hh, lane);
+    unit_qkv<HD>(a, j, D.part, r, hh, lane, rc);
   }
 }
 
