@@ -195,3 +195,51 @@ def test_13b_width_four_sequences_256_row_stages(P):
     a.close()
     del wd
     torch.cuda.empty_cache()
+
+
+def test_c2_full_model_at_the_bench_context(P):
+    """BASELINE.json:configs[1] at FULL size in the configuration bench.py times: the Llama-2-7B shape with all 32 layers,
+    X = {8,16,24,32}, the bench's own 512-token prompt (same seed).  The oracle prefills the prompt in its whole-sequence
+    form (oracle.ar.prefill_matrix, pinned to the position-wise prefill), then
+      * AR (X = {L}): two tokens, every one of the 32 layers' hidden states, the logits through the debug recompute AND the
+        fused exit's own per-block maxima, the anchor top-2, the tokens (teacher-forced, R17);
+      * DEX: the first commit (4 rounds, 15 lattice nodes) against the oracle's Alg. 1 trace with the GPU's exit decisions
+        forced (R17b): nodes, rows per stage, layer evaluations, stage-boundary hidden states, the commit."""
+    import dex_synth
+    import torch
+    from oracle import OracleModel, ar_greedy, dex_decode
+    from trace_util import gpu_trace, check_ref_blocks, rel_err, HID_TOL, LOGIT_TOL, MARGIN
+    wl = dex_synth.workload("c2")
+    w = dex_synth.make_weights(wl.shape, wl.weight_seed, threads=16)
+    p = dex_synth.make_prompt(wl.shape.vocab, wl.prompt_len, wl.prompt_seed)
+    om = OracleModel(wl.shape, w, dtype=np.float32, kv_round="bf16")
+    st = _oracle_state(om, p)
+    wd = {k: v.cuda() for k, v in w.items()}
+    L = wl.shape.n_layers
+    # ---- AR
+    T = 2
+    ar = ar_greedy(om, p, T, keep_hidden=True, keep_logits=True, state=_copy_state(st))
+    d = P.Dex(wl.shape, wd, (L,), max_ctx=wl.prompt_len + 16, debug_taps=1, use_graph=0)
+    d.prefill(0, p)
+    for t in range(T):
+        r = d.step(0)[0]
+        h = d.tap_hidden(0)
+        for l in range(L):
+            assert rel_err(h[l], ar["hidden"][t][l]) < HID_TOL, (t, l)
+        assert np.abs(d.tap_logits() - ar["logits"][t]).max() < LOGIT_TOL
+        check_ref_blocks(d.tap_ref_blocks(), ar["logits"][t])
+        assert abs(r.ref_top1 - ar["top1"][t]) < LOGIT_TOL and abs(r.ref_top2 - ar["top2"][t]) < LOGIT_TOL
+        if r.token != ar["tokens"][t]:
+            assert ar["top1"][t] - ar["top2"][t] < MARGIN
+        d.collapse(0, 0, int(ar["tokens"][t]))
+    d.close()
+    # ---- DEX, first commit
+    g = P.Dex(wl.shape, wd, wl.depths, max_ctx=wl.prompt_len + 16, debug_taps=1, use_graph=0)
+    g.prefill(0, p)
+    recs = gpu_trace(g, 1)
+    g.close()
+    force_u = {(ri, i): t for ri, rec in enumerate(recs) for i, t in rec["u"].items()}
+    od = dex_decode(om, p, 1, wl.depths, trace=True, force_u=force_u, state=_copy_state(st))
+    _trace_check(recs, od, 15)
+    del wd
+    torch.cuda.empty_cache()
