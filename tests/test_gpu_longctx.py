@@ -98,8 +98,14 @@ def test_7b_width_long_context_dex_trace(P, wide7b, rk):
     assert np.array_equal(ar_gpu, dex_tokens)
 
 
-def _trace_check(recs, od, n_min):
+def _trace_check(recs, od, n_min, margin_mid=None):
+    """margin_mid: the oracle logit gap below which an INTERMEDIATE exit decision (a non-final node's candidate) may differ;
+    default = the 1e-2 of the committed-token rule (reading R17b).  The final-depth anchor (the committed token) is always
+    held to 1e-2."""
     import trace_util as tu
+    margin_mid = tu.MARGIN if margin_mid is None else margin_mid
+    n_lvl = max(gr["q"] for gr in recs) + 1
+    ref_node = (1 << (n_lvl - 1)) - 1
     assert len(od["rounds"]) == len(recs)
     n_nodes = n_forced = 0
     for ri, (gr, o) in enumerate(zip(recs, od["rounds"])):
@@ -110,7 +116,7 @@ def _trace_check(recs, od, n_min):
             assert tu.rel_err(gr["h"][i], o["h_out"][i]) < tu.HID_TOL, (ri, i)
         for i, (own, tok, gap) in o.get("u_forced", {}).items():
             n_forced += 1
-            assert gap < tu.MARGIN, (ri, i, gap)
+            assert gap < (tu.MARGIN if (i == ref_node and o["committed"]) else margin_mid), (ri, i, gap)
         if o["committed"]:
             assert gr["token"] == o["token"] and gr["k"] == o["match_k"], ri
             assert abs(gr["top1"] - o["ref_top1"]) < tu.LOGIT_TOL and abs(gr["top2"] - o["ref_top2"]) < tu.LOGIT_TOL
@@ -204,7 +210,8 @@ def test_c2_full_model_at_the_bench_context(P):
       * AR (X = {L}): two tokens, every one of the 32 layers' hidden states, the logits through the debug recompute AND the
         fused exit's own per-block maxima, the anchor top-2, the tokens (teacher-forced, R17);
       * DEX: the first commit (4 rounds, 15 lattice nodes) against the oracle's Alg. 1 trace with the GPU's exit decisions
-        forced (R17b): nodes, rows per stage, layer evaluations, stage-boundary hidden states, the commit."""
+        forced (R17b): nodes, rows per stage, layer evaluations, stage-boundary hidden states, the commit;
+      * the same for the c3 lattice (X every 4 layers, N = 8: 8 rounds, 255 nodes) on the same tensors and prompt."""
     import dex_synth
     import torch
     from oracle import OracleModel, ar_greedy, dex_decode
@@ -241,5 +248,108 @@ def test_c2_full_model_at_the_bench_context(P):
     force_u = {(ri, i): t for ri, rec in enumerate(recs) for i, t in rec["u"].items()}
     od = dex_decode(om, p, 1, wl.depths, trace=True, force_u=force_u, state=_copy_state(st))
     _trace_check(recs, od, 15)
+    # ---- the c3 lattice on the same tensors and prompt (BASELINE.json:configs[2]: X every 4 layers, N = 8): the first
+    #      commit = 8 rounds up to 128 rows, 255 nodes, pass-task attention, both exit chunks on the last round
+    X3 = dex_synth.workload("c3").depths
+    g = P.Dex(wl.shape, wd, X3, max_ctx=wl.prompt_len + 16, debug_taps=1, use_graph=0)
+    g.prefill(0, p)
+    recs = gpu_trace(g, 1)
+    g.close()
+    force_u = {(ri, i): t for ri, rec in enumerate(recs) for i, t in rec["u"].items()}
+    od = dex_decode(om, p, 1, X3, trace=True, force_u=force_u, state=_copy_state(st))
+    _trace_check(recs, od, 255)
     del wd
     torch.cuda.empty_cache()
+
+
+def test_c4_full_model_at_the_bench_context(P):
+    """BASELINE.json:configs[3] at FULL size: the Llama-3-8B shape (32 layers, GQA 32/8, ffn 14336, V = 128256, RoPE theta
+    5e5), X every 4 layers (N = 8), the bench's own 2048-token prompt (33 attention chunks, 16 committed pages).  One AR
+    token (all 32 layers' hidden states, logits through the recompute and through the fused exit's own maxima over 4008
+    blocks, anchor top-2) and the first DEX commit (8 rounds, 255 nodes, pass-task attention over the long context, the
+    1002-tile exit head on both exit chunks) against the oracle's trace.  The oracle's prefill takes about a minute."""
+    import dex_synth
+    import torch
+    from oracle import OracleModel, ar_greedy, dex_decode
+    from trace_util import gpu_trace, check_ref_blocks, rel_err, HID_TOL, LOGIT_TOL, MARGIN
+    wl = dex_synth.workload("c4")
+    w = dex_synth.make_weights(wl.shape, wl.weight_seed, threads=16)
+    p = dex_synth.make_prompt(wl.shape.vocab, wl.prompt_len, wl.prompt_seed)
+    om = OracleModel(wl.shape, w, dtype=np.float32, kv_round="bf16")
+    st = _oracle_state(om, p)
+    wd = {k: v.cuda() for k, v in w.items()}
+    L = wl.shape.n_layers
+    ar = ar_greedy(om, p, 1, keep_hidden=True, keep_logits=True, state=_copy_state(st))
+    d = P.Dex(wl.shape, wd, (L,), max_ctx=wl.prompt_len + 16, debug_taps=1, use_graph=0)
+    d.prefill(0, p)
+    r = d.step(0)[0]
+    h = d.tap_hidden(0)
+    for l in range(L):
+        assert rel_err(h[l], ar["hidden"][0][l]) < HID_TOL, l
+    assert np.abs(d.tap_logits() - ar["logits"][0]).max() < LOGIT_TOL
+    check_ref_blocks(d.tap_ref_blocks(), ar["logits"][0])
+    assert abs(r.ref_top1 - ar["top1"][0]) < LOGIT_TOL and abs(r.ref_top2 - ar["top2"][0]) < LOGIT_TOL
+    if r.token != ar["tokens"][0]:
+        assert ar["top1"][0] - ar["top2"][0] < MARGIN
+    d.close()
+    g = P.Dex(wl.shape, wd, wl.depths, max_ctx=wl.prompt_len + 16, debug_taps=1, use_graph=0)
+    g.prefill(0, p)
+    recs = gpu_trace(g, 1)
+    g.close()
+    force_u = {(ri, i): t for ri, rec in enumerate(recs) for i, t in rec["u"].items()}
+    od = dex_decode(om, p, 1, wl.depths, trace=True, force_u=force_u, state=_copy_state(st))
+    _trace_check(recs, od, 255)
+    del wd
+    torch.cuda.empty_cache()
+
+
+@pytest.fixture(scope="module")
+def c5_full():
+    import dex_synth
+    from oracle import OracleModel
+    wl = dex_synth.workload("c5")
+    w = dex_synth.make_weights(wl.shape, wl.weight_seed, threads=16)
+    prompts = [dex_synth.make_prompt(wl.shape.vocab, wl.prompt_len, wl.prompt_seed, seq=s) for s in range(wl.n_seqs)]
+    om = OracleModel(wl.shape, w, dtype=np.float32, kv_round="bf16")
+    return wl, w, prompts, om, _oracle_state(om, prompts[3])
+
+
+@pytest.mark.parametrize("planes", [2, 1])
+def test_c5_full_model_at_the_bench_context(P, c5_full, planes):
+    """BASELINE.json:configs[4] at FULL size: the Llama-2-13B shape (40 layers), X every 5 layers (N = 8), FOUR sequences
+    with their own 1024-token prompts batched into the same launches (256-row stage 0, 512 exit rows).  Sequence 3 is
+    checked against the oracle's Alg. 1 trace for its first commit (8 rounds, 255 nodes) while all four step together.
+    planes = 2: two-plane activations (the per-op launch path: a 256-row two-plane stage does not fit k_round's ring):
+    every clause at its stated tolerance.  planes = 1: the k_round configuration of the c5 bench line (plain bf16
+    activations, what north_star's "bf16 tensor-core GEMMs" literally are): hidden states, counts and the committed token
+    at their tolerances, but an INTERMEDIATE exit decision may differ from the oracle's up to the logit tolerance
+    (5e-2; seen: one node of 255 at an oracle gap of 0.017) - which is why two planes are the default (reading R23)."""
+    import torch
+    from oracle import dex_decode
+    wl, w, prompts, om, st3 = c5_full
+    wd = {k: v.cuda() for k, v in w.items()}
+    S, X, N = wl.n_seqs, wl.depths, len(wl.depths)
+    g = P.Dex(wl.shape, wd, X, max_seqs=S, max_ctx=wl.prompt_len + 16, debug_taps=1, use_graph=0, act_planes=planes)
+    for s in range(S):
+        g.prefill(s, prompts[s])
+    recs = []
+    for _ in range(N):
+        res = g.step(0)
+        r = res[3]
+        q = r.q_before
+        B = g.tap_B(3)
+        nodes = list(range((1 << q) - 1, (2 << q) - 1))
+        rec = dict(q=q, rows=list(r.rows_per_stage)[:N], evals=int(r.layer_evals), nodes=nodes,
+                   u={i: int(B[i]) for i in nodes}, h={i: g.tap_hidden(i, 3)[-1].copy() for i in nodes}, committed=0)
+        if r.match_k >= 0:
+            rec.update(committed=1, token=int(r.token), k=int(r.match_k), top1=float(r.ref_top1), top2=float(r.ref_top2))
+        recs.append(rec)
+        for s in range(S):
+            if res[s].match_k >= 0:
+                g.collapse(s, res[s].match_k, res[s].token)
+    g.close()
+    del wd
+    torch.cuda.empty_cache()
+    force_u = {(ri, i): t for ri, rec in enumerate(recs) for i, t in rec["u"].items()}
+    od = dex_decode(om, prompts[3], 1, X, trace=True, force_u=force_u, state=_copy_state(st3))
+    _trace_check(recs, od, 255, margin_mid=None if planes == 2 else 5e-2)
