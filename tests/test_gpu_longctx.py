@@ -209,9 +209,11 @@ def test_c2_full_model_at_the_bench_context(P):
     form (oracle.ar.prefill_matrix, pinned to the position-wise prefill), then
       * AR (X = {L}): two tokens, every one of the 32 layers' hidden states, the logits through the debug recompute AND the
         fused exit's own per-block maxima, the anchor top-2, the tokens (teacher-forced, R17);
-      * DEX: the first commit (4 rounds, 15 lattice nodes) against the oracle's Alg. 1 trace with the GPU's exit decisions
+      * DEX: the first three commits (the first = 4 rounds, 15 lattice nodes; then collapse and the re-rooted lattice)
+        against the oracle's Alg. 1 trace with the GPU's exit decisions
         forced (R17b): nodes, rows per stage, layer evaluations, stage-boundary hidden states, the commit;
-      * the same for the c3 lattice (X every 4 layers, N = 8: 8 rounds, 255 nodes) on the same tensors and prompt."""
+      * the same for the c3 lattice (X every 4 layers, N = 8: 8 rounds, 255 nodes, then a second commit) on the same
+        tensors and prompt."""
     import dex_synth
     import torch
     from oracle import OracleModel, ar_greedy, dex_decode
@@ -243,21 +245,22 @@ def test_c2_full_model_at_the_bench_context(P):
     # ---- DEX, first commit
     g = P.Dex(wl.shape, wd, wl.depths, max_ctx=wl.prompt_len + 16, debug_taps=1, use_graph=0)
     g.prefill(0, p)
-    recs = gpu_trace(g, 1)
+    recs = gpu_trace(g, 3)                                   # three commits: collapse and the re-rooted lattice included
     g.close()
     force_u = {(ri, i): t for ri, rec in enumerate(recs) for i, t in rec["u"].items()}
-    od = dex_decode(om, p, 1, wl.depths, trace=True, force_u=force_u, state=_copy_state(st))
-    _trace_check(recs, od, 15)
+    od = dex_decode(om, p, 3, wl.depths, trace=True, force_u=force_u, state=_copy_state(st))
+    _trace_check(recs, od, 15 + 2)
+    assert [r_["fsm_after"][0] for r_ in recs if r_["committed"]] == [o["q_after"] for o in od["rounds"] if o["committed"]]
     # ---- the c3 lattice on the same tensors and prompt (BASELINE.json:configs[2]: X every 4 layers, N = 8): the first
     #      commit = 8 rounds up to 128 rows, 255 nodes, pass-task attention, both exit chunks on the last round
     X3 = dex_synth.workload("c3").depths
     g = P.Dex(wl.shape, wd, X3, max_ctx=wl.prompt_len + 16, debug_taps=1, use_graph=0)
     g.prefill(0, p)
-    recs = gpu_trace(g, 1)
+    recs = gpu_trace(g, 2)                                   # two commits
     g.close()
     force_u = {(ri, i): t for ri, rec in enumerate(recs) for i, t in rec["u"].items()}
-    od = dex_decode(om, p, 1, X3, trace=True, force_u=force_u, state=_copy_state(st))
-    _trace_check(recs, od, 255)
+    od = dex_decode(om, p, 2, X3, trace=True, force_u=force_u, state=_copy_state(st))
+    _trace_check(recs, od, 255 + 1)
     del wd
     torch.cuda.empty_cache()
 
