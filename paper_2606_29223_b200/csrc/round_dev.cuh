@@ -532,10 +532,12 @@ __device__ void glue_qkv_finalize(const RoundArgs& a, int j, int gw, int n_gw, i
 // commit, page after) and whatever else shares the MMA: DEX stream == AR stream (H3).  When all chunks of
 // (row, head) are written, the last writer merges the sub-partials in ascending position order.
 constexpr int kAttnPairs = 16;       // pairs per pass of a task (the M of the MMAs)
+constexpr int kPageCache = 96;       // chunks of a range whose page index is cached in shared memory (longer ranges: table lookups)
 
 template <int HD>
 struct AttnSmem {
-  __nv_bfloat16 kv[2][2][kChunk * HD];          // [buffer][K / V][row][dim], 16-byte pieces swizzled: j ^ (row & 7)
+  __nv_bfloat16 kv[2][2][kChunk * HD];          // eight tile buffers of [K / V][16 positions][dim] (attn_run: NB per warp),
+                                                // 16-byte pieces swizzled: j ^ (row & 7)
   __nv_bfloat16 qh[kAttnPairs][HD + 8];         // q hi / lo planes (row stride padded: conflict-free fragment loads)
   __nv_bfloat16 ql[kAttnPairs][HD + 8];
   int ppos[kAttnPairs];                         // position of the pair's row; -1: not in this pass
@@ -545,6 +547,8 @@ struct AttnSmem {
                                                 // once per task, so the private-tile loop has ONE dependent load per row
   int n_vrow;                                   // sparse lattice (R26): the expanded rows of the task's (stage, sequence)
   short vrow[128];
+  int unit_ctr;                                 // next work unit of the pass (claimed per warp)
+  int cpage[kPageCache];                        // page of every 64-position chunk of the task's range
 };
 
 __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc) {
@@ -769,6 +773,8 @@ __device__ void attn_run(const RoundArgs& a, const AttnPlan& pl, const AttnTask&
                          AttnSmem<HD>* sm, int* s_ao_cnt, int ao_slice_cols, const SeqState* seq_sm) {
   constexpr int CPR = HD / 8;                                // 16-byte pieces per K/V row
   constexpr int kEpiThreads = GT;
+  constexpr int NW = GT / 32, NB = NW >= 8 ? 1 : 2;          // warps of the group; 16-position tile buffers per warp
+  static_assert(NW * NB <= 8, "the K/V staging area holds eight 16-position tile pairs");
   const Dev& D = a.D;
   const int m = tk.m, s = tk.s, g = tk.g, rg = tk.rg, pb_task = tk.pb_task;
   const bool tail_own = pl.tail_own != 0;
@@ -807,30 +813,64 @@ __device__ void attn_run(const RoundArgs& a, const AttnPlan& pl, const AttnTask&
 
   for (int pb = pb_task; pb < (PT ? min(n_pairs, pb_task + kAttnPairs) : n_pairs); pb += kAttnPairs) {
     const int np = min(kAttnPairs, n_pairs - pb);
-    auto stage = [&](int c, int buf) {
-      const int c0 = c * kChunk;
-      const int n_rows = min(kChunk, n_paged - c0);        // committed rows of the chunk (one page: page_size % 64 == 0)
-      if (n_rows > 0) {
-        const size_t base = page_off(D, s, layer, c0) + (size_t)g * HD;
-        for (int id = tid_e; id < n_rows * CPR; id += kEpiThreads) {
-          const int pl = id / CPR, cj = id - pl * CPR;
-          const int dj = (cj ^ (pl & 7)) * 8;
-          cp_async16(&sm->kv[buf][0][pl * HD + dj], D.kpool + base + (size_t)pl * kv_stride + cj * 8);
-          cp_async16(&sm->kv[buf][1][pl * HD + dj], D.vpool + base + (size_t)pl * kv_stride + cj * 8);
+    // ---- work units of the pass.  The range's 16-position tiles [4 ca, 4 cb) are independent of one another: every
+    // (tile, pair) writes a sub-partial of its own and the merge below adds them in position order, so which warp runs
+    // a tile, and when, cannot change a bit (H3).  Each warp owns NB tile buffers (K and V of 16 positions, 64 KB for
+    // the group), claims units from a shared counter, loads the tile with cp.async and computes it on its own: no
+    // CTA-wide barrier inside the loop, and the 8 warps' loads are in flight under one another's MMAs (the chunk-wide
+    // double buffer had ONE 32 KB stage in flight per CTA and was bound by its latency).
+    //   shared tile  (all 16 positions committed): one attn_tile over every pair of the pass
+    //   private unit (tile, rank of nk): the tile holds private positions; the unit takes lattice rows rank, rank + nk, ...
+    //     one at a time, patching the row's ancestor / own K/V rows (from their slots) into its copy of the tile IN PLACE.
+    //     Rows above the row's own position keep finite data (zeros or an earlier row's patch): they are masked and
+    //     enter the P.V MMA with weight 0.  Private units come first in the claim order (they are the long ones).
+    const int T0 = ca * 4;
+    const int T_end = min(cb * 4, (st.ctx_len + st.q) / 16 + 1);          // no row sees a tile beyond ctx_len + q
+    const int T_sh = min(T_end, max(T0, n_paged / 16));                    // tiles [T0, T_sh) are fully committed
+    const int n_priv = T_end - T_sh;
+    const int n_rl = (np + Gq - 1) / Gq;
+    const int nk = n_priv > 0 ? max(1, min(n_rl, NW / n_priv)) : 1;
+    const int n_pu = n_priv * nk;
+    const int n_units = n_pu + (T_sh - T0);
+    if (tid_e == 0) sm->unit_ctr = 0;
+    for (int i = tid_e; i < min(cb - ca, kPageCache); i += kEpiThreads)     // page of every chunk of the range (one per chunk:
+      sm->cpage[i] = D.page_table[s * D.pages_per_seq + ((ca + i) * kChunk) / D.page_size];   // page_size % 64 == 0)
+    bar_epi<GT>();
+    auto claim = [&]() {
+      int u = 0;
+      if (lane == 0) u = atomicAdd(&sm->unit_ctr, 1);
+      return __shfl_sync(0xffffffffu, u, 0);
+    };
+    auto tile_of = [&](int u) { return u < n_pu ? T_sh + u / nk : T0 + (u - n_pu); };
+    auto kbuf = [&](int b) { return &sm->kv[0][0][0] + (size_t)((we * NB + b) * 2) * (16 * HD); };
+    auto load_unit = [&](int u, int b) {                  // committed rows of the unit's tile -> the warp's buffer b, zeros above
+      if (u < n_units) {
+        const int T = tile_of(u), p0 = T * 16, ci = T / 4 - ca;
+        const int n_rows = max(0, min(16, n_paged - p0));
+        __nv_bfloat16* kd = kbuf(b);
+        __nv_bfloat16* vd = kd + 16 * HD;
+        if (n_rows > 0) {
+          const int pg = ci < kPageCache ? sm->cpage[ci] : D.page_table[s * D.pages_per_seq + p0 / D.page_size];
+          const size_t base = (size_t)layer * kv_layer_elems(D) + (size_t)pg * kv_page_elems(D) + (size_t)(p0 % D.page_size) * kv_stride + (size_t)g * HD;
+          for (int id = lane; id < n_rows * CPR; id += 32) {
+            const int pl = id / CPR, cj = id - pl * CPR;
+            const int dj = (cj ^ (pl & 7)) * 8;
+            cp_async16(kd + pl * HD + dj, D.kpool + base + (size_t)pl * kv_stride + cj * 8);
+            cp_async16(vd + pl * HD + dj, D.vpool + base + (size_t)pl * kv_stride + cj * 8);
+          }
         }
-      }
-      if (n_rows < kChunk) {                               // rows past the committed prefix: zeros (a masked position
-        const int z0 = max(n_rows, 0);                     // still enters the P.V MMA with weight 0: keep it finite)
-        for (int id = tid_e; id < (kChunk - z0) * CPR; id += kEpiThreads) {
-          const int pl = z0 + id / CPR, cj = id % CPR;
-          *reinterpret_cast<uint4*>(&sm->kv[buf][0][pl * HD + cj * 8]) = make_uint4(0u, 0u, 0u, 0u);
-          *reinterpret_cast<uint4*>(&sm->kv[buf][1][pl * HD + cj * 8]) = make_uint4(0u, 0u, 0u, 0u);
+        for (int id = lane; id < (16 - n_rows) * CPR; id += 32) {
+          const int pl = n_rows + id / CPR, cj = id % CPR;
+          *reinterpret_cast<uint4*>(kd + pl * HD + cj * 8) = make_uint4(0u, 0u, 0u, 0u);
+          *reinterpret_cast<uint4*>(vd + pl * HD + cj * 8) = make_uint4(0u, 0u, 0u, 0u);
         }
       }
       cp_async_commit();
     };
-    stage(ca, 0);
-    // ---- q of the pass's pairs (phase Q wrote it) -> bf16 hi / lo planes, in flight together with the first chunk
+    int u0 = claim(), u1 = n_units;
+    load_unit(u0, 0);
+    if (NB == 2) { u1 = claim(); load_unit(u1, 1); }
+    // ---- q of the pass's pairs (phase Q wrote it) -> bf16 hi / lo planes, in flight together with the first tiles
     for (int id = tid_e; id < kAttnPairs * HD; id += kEpiThreads) {
       const int pi = id / HD, t = id - pi * HD;
       float v = 0.f;
@@ -863,74 +903,46 @@ __device__ void attn_run(const RoundArgs& a, const AttnPlan& pl, const AttnTask&
         for (int i = 0; i <= kMaxAnc; ++i) sm->rslot[rl][i] = (i < n_anc && i < kMaxAnc) ? ri->anc[i] : own;
       }
     }
-    for (int c = ca; c < cb; ++c) {
-      const int buf = (c - ca) & 1, c0 = c * kChunk;
-      if (c + 1 < cb) stage(c + 1, buf ^ 1);
-      else cp_async_commit();
-      cp_async_wait<1>();
-      bar_epi<GT>();                                         // chunk c staged by all threads; q planes written
+    bar_epi<GT>();                                           // q planes and the row tables are written
+    for (int k = 0;; ++k) {
+      const int b = NB == 2 ? (k & 1) : 0;
+      const int u = b ? u1 : u0;
+      if (u >= n_units) break;                               // claims only grow: nothing later is valid either
+      cp_async_wait<NB - 1>();
+      __syncwarp();
       {
-        const uint32_t kb = smem_u32(sm->kv[buf][0]), vb = smem_u32(sm->kv[buf][1]);
-        const int t_shared = max(0, min(4, (n_paged - c0) / 16));   // tiles whose 16 positions are all committed:
-        if (we < t_shared) attn_tile<HD>(D, sm, kb, vb, we * 16, c, we, 0, np, lane);   // every pair shares them
-        // tiles that hold private positions: warp t owns tile t of the staged chunk and takes lattice rows one at a
-        // time, patching the row's ancestor / own K/V rows (from their slots) into the tile IN PLACE at their
-        // positions.  Rows above the row's own position keep finite data (zeros or an earlier row's patch): they
-        // are masked and enter the P.V MMA with weight 0.  No CTA-wide synchronisation: tiles are disjoint.
-        // On the LAST chunk of the range the other staging buffer is idle: warps 4-7 copy the committed rows of a
-        // private tile into a 16-row slot of it and share the tile's lattice rows with the owner (same
-        // instructions on the same tile contents -> same bits, H3).
-        const int n_rl = (np + Gq - 1) / Gq;
-        const int t_hi = min(3, (st.ctx_len + st.q - c0) / 16);     // last tile a row of this sequence can see
-        const int n_pt = t_hi - t_shared + 1;                         // tiles with private positions
-        const bool par = c == cb - 1 && n_rl > 1 && n_pt >= 1 && GT / 32 >= 8;
-        int t = -1, rank = 0, nk = 1, tb = buf, trow = 0;
-        if (we >= t_shared && we < 4) {
-          t = we; trow = t * 16;
-          if (par && t <= t_hi) nk = 1 + (4 - (t - t_shared) + n_pt - 1) / n_pt;
-        } else if (par && we >= 4 && we < 8) {
-          const int h = we - 4;
-          t = t_shared + h % n_pt; rank = 1 + h / n_pt; nk = 1 + (4 - (t - t_shared) + n_pt - 1) / n_pt;
-          tb = buf ^ 1; trow = h * 16;
-        }
-        if (t >= 0) {
-          const int p0 = c0 + t * 16;
+        const int T = tile_of(u), c = T >> 2, t = T & 3, p0 = T * 16;
+        __nv_bfloat16* kd = kbuf(b);
+        const uint32_t kbt = smem_u32(kd), vbt = smem_u32(kd + 16 * HD);
+        if (u >= n_pu) {
+          attn_tile<HD>(D, sm, kbt, vbt, 0, c, t, 0, np, lane);   // every pair shares a committed tile
+        } else {
           const int i_lo = max(n_paged - p0, 0);
-          if (tb != buf) {                                 // helper: committed rows of the tile, zeros above
-            for (int id = lane; id < 16 * CPR; id += 32) {
-              const int i = id / CPR, cj = id % CPR;
-              uint4 kk = make_uint4(0u, 0u, 0u, 0u), vv = kk;
-              if (i < i_lo) {
-                kk = *reinterpret_cast<const uint4*>(&sm->kv[buf][0][(t * 16 + i) * HD + cj * 8]);
-                vv = *reinterpret_cast<const uint4*>(&sm->kv[buf][1][(t * 16 + i) * HD + cj * 8]);
-              }
-              *reinterpret_cast<uint4*>(&sm->kv[tb][0][(trow + i) * HD + cj * 8]) = kk;
-              *reinterpret_cast<uint4*>(&sm->kv[tb][1][(trow + i) * HD + cj * 8]) = vv;
-            }
-            __syncwarp();
-          }
-          const uint32_t kbt = smem_u32(sm->kv[tb][0]), vbt = smem_u32(sm->kv[tb][1]);
-          for (int rl = rank; rl < n_rl; rl += nk) {
+          for (int rl = u % nk; rl < n_rl; rl += nk) {
             const int pos = sm->rpos[rl];
             if (pos < p0) continue;                        // the row does not see this tile (warp-uniform)
             const int i_hi = min(pos - p0, 15);
             for (int id = lane; id < (i_hi - i_lo + 1) * CPR; id += 32) {
-              const int i = i_lo + id / CPR, cj = id % CPR, pl = trow + i;
+              const int i = i_lo + id / CPR, cj = id % CPR;
               const int ai = p0 + i - n_paged;
               const int slot = sm->rslot[rl][min(ai, kMaxAnc)];
               const size_t so = slot_off(D, s, slot, layer) + (size_t)g * HD + cj * 8;
-              const int dj = (cj ^ (pl & 7)) * 8;
-              *reinterpret_cast<uint4*>(&sm->kv[tb][0][pl * HD + dj]) = *reinterpret_cast<const uint4*>(D.kslot + so);
-              *reinterpret_cast<uint4*>(&sm->kv[tb][1][pl * HD + dj]) = *reinterpret_cast<const uint4*>(D.vslot + so);
+              const int dj = (cj ^ (i & 7)) * 8;
+              *reinterpret_cast<uint4*>(kd + i * HD + dj) = *reinterpret_cast<const uint4*>(D.kslot + so);
+              *reinterpret_cast<uint4*>(kd + 16 * HD + i * HD + dj) = *reinterpret_cast<const uint4*>(D.vslot + so);
             }
             __syncwarp();
-            attn_tile<HD>(D, sm, kbt, vbt, trow, c, t, rl * Gq, min(np, (rl + 1) * Gq), lane);
+            attn_tile<HD>(D, sm, kbt, vbt, 0, c, t, rl * Gq, min(np, (rl + 1) * Gq), lane);
             __syncwarp();
           }
         }
       }
-      bar_epi<GT>();                                         // kv buffer free for chunk c + 2
+      __syncwarp();                                          // every lane is done with buffer b before it is refilled
+      const int un = claim();
+      load_unit(un, b);
+      if (b) u1 = un; else u0 = un;
     }
+    cp_async_wait<0>();
     // ---- all sub-partials of this pass are written: count the chunks in; the last writer of (row, head) merges
     bar_epi<GT>();                                           // orders every warp's sub-partial stores before the counter's release
     for (int pi = we; pi < np; pi += GT / 32) {
